@@ -1,0 +1,91 @@
+"""ctypes wrapper over the double-precision CPU oracle (TEST INFRASTRUCTURE).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs import this.  It never imports the CUDA binding.  Inputs of any float dtype are
+widened to float64 exactly; see psdf_oracle.cpp for what is computed and the citations.
+"""
+from __future__ import annotations
+
+import ctypes
+from dataclasses import dataclass
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(_build.build())
+        dp = ctypes.POINTER(ctypes.c_double)
+        ip = ctypes.POINTER(ctypes.c_int)
+        _lib.psdf_oracle_eval.restype = ctypes.c_int
+        _lib.psdf_oracle_eval.argtypes = [dp, ctypes.c_int, dp, dp, ctypes.POINTER(ctypes.c_uint8),
+                                          ctypes.c_int, ctypes.c_int, dp, ctypes.c_int, dp, dp, dp,
+                                          dp, ip, ip, ctypes.c_double, ctypes.c_int]
+        _lib.psdf_oracle_max_threads.restype = ctypes.c_int
+    return _lib
+
+
+def max_threads() -> int:
+    return int(lib().psdf_oracle_max_threads())
+
+
+@dataclass
+class OracleResult:
+    value: np.ndarray          # [N] f64   phi (eq.6)
+    grad: np.ndarray           # [N,3] f64 d phi / d(x,y,theta)
+    per_obstacle: np.ndarray   # [N,M] f64 sd^i (eq.23), +inf for empty rows (or None)
+    margin: np.ndarray         # [N] f64   reading G9
+    winner: np.ndarray         # [N] i32   argmin obstacle row (-1: none)
+    branch: np.ndarray         # [N] i32   1 separated / 0 not separated, of the winner
+
+
+def _p(a, ct):
+    return a.ctypes.data_as(ctypes.POINTER(ct)) if a is not None else None
+
+
+def evaluate(footprint, A, B, S, poses, per_obstacle=False, window=0.01, nthreads=0) -> OracleResult:
+    fp = np.ascontiguousarray(footprint, dtype=np.float64)
+    A = np.ascontiguousarray(A, dtype=np.float64)
+    B = np.ascontiguousarray(B, dtype=np.float64)
+    S = np.ascontiguousarray(S, dtype=np.uint8)
+    poses = np.ascontiguousarray(poses, dtype=np.float64).reshape(-1, 3)
+    V, (M, E), N = fp.shape[0], S.shape, poses.shape[0]
+    assert fp.shape == (V, 2) and A.shape == (M, E, 2) and B.shape == (M, E, 2)
+    value = np.empty(N)
+    grad = np.empty((N, 3))
+    per = np.empty((N, M)) if per_obstacle else None
+    margin = np.empty(N)
+    winner = np.empty(N, dtype=np.int32)
+    branch = np.empty(N, dtype=np.int32)
+    rc = lib().psdf_oracle_eval(_p(fp, ctypes.c_double), V, _p(A, ctypes.c_double),
+                                _p(B, ctypes.c_double), _p(S, ctypes.c_uint8), M, E,
+                                _p(poses, ctypes.c_double), N, _p(value, ctypes.c_double),
+                                _p(grad, ctypes.c_double), _p(per, ctypes.c_double),
+                                _p(margin, ctypes.c_double), _p(winner, ctypes.c_int),
+                                _p(branch, ctypes.c_int), float(window), int(nthreads))
+    if rc != 0:
+        raise ValueError("psdf_oracle_eval: bad arguments")
+    return OracleResult(value, grad, per, margin, winner, branch)
+
+
+def evaluate_value_only(footprint, A, B, S, poses, nthreads=0) -> np.ndarray:
+    """Plain-double pass only (no duals): what bench.py times as the CPU baseline."""
+    fp = np.ascontiguousarray(footprint, dtype=np.float64)
+    A = np.ascontiguousarray(A, dtype=np.float64)
+    B = np.ascontiguousarray(B, dtype=np.float64)
+    S = np.ascontiguousarray(S, dtype=np.uint8)
+    poses = np.ascontiguousarray(poses, dtype=np.float64).reshape(-1, 3)
+    V, (M, E), N = fp.shape[0], S.shape, poses.shape[0]
+    value = np.empty(N)
+    rc = lib().psdf_oracle_eval(_p(fp, ctypes.c_double), V, _p(A, ctypes.c_double),
+                                _p(B, ctypes.c_double), _p(S, ctypes.c_uint8), M, E,
+                                _p(poses, ctypes.c_double), N, _p(value, ctypes.c_double),
+                                None, None, None, None, None, 0.01, int(nthreads))
+    if rc != 0:
+        raise ValueError("psdf_oracle_eval: bad arguments")
+    return value

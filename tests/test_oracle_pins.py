@@ -1,0 +1,179 @@
+"""Pins the oracle to things other than itself (③): hand-worked closed forms of the
+definition (5a-c), the Minkowski-difference definition, dense brute force, finite
+differences.  CPU only."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import psdf_oracle as O
+from paper_2607_04310_b200 import workloads as W
+from tests import geom_ref as G
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")
+ENV = {"sqrt": math.sqrt, "cos": math.cos, "sin": math.sin, "pi": math.pi, "__builtins__": {}}
+FP = {"rect": W.rectangle(0.6, 0.4), "sq": W.rectangle(1.0, 1.0)}
+
+
+def _num(tok):
+    return float(eval(tok, ENV))
+
+
+def _poly(spec):
+    t = spec.split()
+    if t[0] == "box":
+        x0, x1, y0, y1 = map(float, t[1:])
+        return np.array([[x0, y0], [x1, y0], [x1, y1], [x0, y1]])
+    v = np.array(list(map(float, t[1:]))).reshape(-1, 2)
+    return v
+
+
+def _scene(polys, E=None, M_extra=0):
+    E = E or max(len(p) for p in polys)
+    M = len(polys) + M_extra
+    A = np.full((M, E, 2), 7.5)
+    B = np.full((M, E, 2), -3.25)
+    S = np.zeros((M, E), np.uint8)
+    for i, p in enumerate(polys):
+        k = len(p)
+        A[i, :k], B[i, :k], S[i, :k] = p, np.roll(p, -1, axis=0), 1
+    return A, B, S
+
+
+def _cases():
+    out = []
+    for line in open(GOLD):
+        if line.startswith("#") or not line.strip():
+            continue
+        f = [x.strip() for x in line.split("|")]
+        out.append(f)
+    return out
+
+
+@pytest.mark.parametrize("case", _cases(), ids=lambda c: c[0])
+def test_closed_forms(case):
+    cid, fpn, pose, obst, val, grad, per, _ = case
+    pose = [_num(t) for t in pose.split()]
+    polys = [_poly(s) for s in obst.split(";")]
+    A, B, S = _scene(polys)
+    r = O.evaluate(FP[fpn], A, B, S, [pose], per_obstacle=True, window=-1.0)
+    assert abs(r.value[0] - _num(val)) < 1e-12, cid
+    if grad != "-":
+        g = [_num(t) for t in grad.split()]
+        assert np.allclose(r.grad[0], g, atol=1e-12), cid
+        assert r.margin[0] > 1e-4
+    else:
+        assert r.margin[0] <= 1e-12          # listed "value only" because of a tie
+    if per != "-":
+        for k, tok in enumerate(per.split(None, 1)):
+            if tok.strip() != "-":
+                assert abs(r.per_obstacle[0, k] - _num(tok)) < 1e-12
+
+
+def test_axis_aligned_box_box_formula():
+    """General closed form: gap sqrt(gx^2+gy^2) / overlap -min(ox,oy) for axis-aligned boxes."""
+    rng = np.random.default_rng(7)
+    for _ in range(300):
+        w, h = rng.uniform(0.2, 2, 2)
+        fp = W.rectangle(w, h)
+        px, py = rng.uniform(-3, 3, 2)
+        x0, y0 = rng.uniform(-3, 3, 2)
+        x1, y1 = x0 + rng.uniform(0.2, 2), y0 + rng.uniform(0.2, 2)
+        A, B, S = _scene([_poly(f"box {x0} {x1} {y0} {y1}")])
+        th = rng.choice([0.0, math.pi])                     # half-turn keeps it axis-aligned
+        got = O.evaluate(fp, A, B, S, [(px, py, th)]).value[0]
+        gx = max(x0 - (px + w / 2), (px - w / 2) - x1)
+        gy = max(y0 - (py + h / 2), (py - h / 2) - y1)
+        if gx > 0 or gy > 0:
+            want = math.hypot(max(gx, 0), max(gy, 0))
+        else:
+            want = -min(-gx, -gy)
+        assert abs(got - want) < 1e-12
+
+
+def _random_case(rng, penetrate=None):
+    V = int(rng.integers(3, 9))
+    fp = W.convex_kgon(rng, V, rng.uniform(0.3, 1.0))
+    k = int(rng.integers(3, 9))
+    ob = W.place(W.convex_kgon(rng, k, rng.uniform(0.3, 1.5)), rng.uniform(-2.5, 2.5, 2), 0.0)
+    pose = np.array([rng.uniform(-1, 1), rng.uniform(-1, 1), rng.uniform(-math.pi, math.pi)])
+    return fp, ob, pose
+
+
+def test_minkowski_definition_random():
+    """sd of eqs.(5a-c) == signed distance of the origin to the Minkowski difference.
+    Pins pools (14)-(16), SAT (17)-(22) and the selection (23) jointly, both signs."""
+    rng = np.random.default_rng(11)
+    npos = nneg = 0
+    for _ in range(1500):
+        fp, ob, pose = _random_case(rng)
+        A, B, S = _scene([ob], E=10)
+        got = O.evaluate(fp, A, B, S, [pose]).value[0]
+        want = G.sd_minkowski(G.posed(fp, pose), ob)
+        assert abs(got - want) < 1e-11, (got, want)
+        npos += got > 0
+        nneg += got < 0
+    assert npos > 200 and nneg > 200
+
+
+def test_bruteforce_tiny():
+    rng = np.random.default_rng(13)
+    seen = {True: 0, False: 0}
+    for _ in range(40):
+        fp, ob, pose = _random_case(rng)
+        A, B, S = _scene([ob], E=10)
+        got = O.evaluate(fp, A, B, S, [pose]).value[0]
+        rw = G.posed(fp, pose)
+        if got > 0:
+            ub = G.dist_bruteforce(rw, ob)                  # from above, error <= ~perimeter/k
+            assert got - 1e-12 <= ub <= got + 5e-3
+        else:
+            ub = G.pen_bruteforce(rw, ob)                   # from above, error O(angle step)
+            assert -got - 1e-12 <= ub <= -got + 1e-3
+        seen[got > 0] += 1
+    assert seen[True] >= 5 and seen[False] >= 5
+
+
+def test_finite_difference_gradient():
+    """Central differences (h=1e-6, double) where the margin allows (reading G9)."""
+    w = W.make_config(2)
+    r = O.evaluate(w.footprint, w.A, w.B, w.S, w.poses)
+    rng = np.random.default_rng(17)
+    extra = np.stack([rng.uniform(0, 20, 400), rng.uniform(0, 20, 400),
+                      rng.uniform(-math.pi, math.pi, 400)], axis=1)
+    poses = np.concatenate([w.poses.astype(np.float64), extra])
+    r = O.evaluate(w.footprint, w.A, w.B, w.S, poses)
+    h = 1e-6
+    ok = (r.margin > 1e-4) & (np.abs(r.value) > 1e-3)
+    assert ok.mean() > 0.8
+    fd = np.empty((len(poses), 3))
+    for k in range(3):
+        d = np.zeros(3)
+        d[k] = h
+        fd[:, k] = (O.evaluate_value_only(w.footprint, w.A, w.B, w.S, poses + d)
+                    - O.evaluate_value_only(w.footprint, w.A, w.B, w.S, poses - d)) / (2 * h)
+    err = np.abs(fd - r.grad)[ok]
+    assert err.max() < 2e-5, err.max()
+    # both branches were exercised
+    assert (r.value[ok] < 0).sum() > 20 and (r.value[ok] > 0).sum() > 20
+
+
+def test_gradient_closed_form_witness():
+    """|grad_p phi| = 1 on both branches away from ties (unit gradient)."""
+    w = W.make_config(3, n_traj=64)
+    r = O.evaluate(w.footprint, w.A, w.B, w.S, w.poses)
+    ok = (r.margin > 1e-4) & (np.abs(r.value) > 1e-3)
+    gn = np.hypot(r.grad[ok, 0], r.grad[ok, 1])
+    assert np.abs(gn - 1.0).max() < 1e-9
+    rmax = np.hypot(w.footprint[:, 0], w.footprint[:, 1]).max()
+    sep = ok & (r.value > 0)
+    assert np.abs(r.grad[sep, 2]).max() <= rmax + 1e-9      # witness lies on the robot
+
+
+def test_window_mode_equals_full_duals():
+    w = W.make_config(2)
+    a = O.evaluate(w.footprint, w.A, w.B, w.S, w.poses, window=-1.0)
+    b = O.evaluate(w.footprint, w.A, w.B, w.S, w.poses, window=0.01)
+    assert np.array_equal(a.value, b.value) and np.array_equal(a.grad, b.grad)
+    assert np.array_equal(np.minimum(a.margin, 0.01), b.margin)
