@@ -1,0 +1,111 @@
+/* psdf.h — C ABI of the B200-native PSDF hot path (arxiv/paper_2607_04310).
+ *
+ * What is computed (citations are PAPER.md line numbers, /root/reference/PAPER.md):
+ *   the polygonal signed distance function
+ *       phi(x, E) = min_i sd(P0(x), P^i)                               eq.(6)
+ *   of a convex robot footprint posed at x = (p, theta),
+ *       P0(x) = { R(theta) v + p | v in co(V0) }                       eq.(9)
+ *   against the convex obstacle components encoded in the padded edge tensors
+ *       A, B in R^{M x E x 2},  S in {0,1}^{M x E}                     eq.(10)
+ *   where sd = dist - pen (eqs.(5a-c)) is evaluated exactly: point-to-
+ *   segment minima over both vertex/edge pools when separated (eqs.(12)-(16),
+ *   PAPER.md:153-177), SAT minimum overlap over both polygons' edge normals when not
+ *   (eqs.(17)-(22)), selected by eq.(23); together
+ *   with the state gradient d phi / d(x, y, theta), here the analytic
+ *   gradient at the arg-min witness instead of an autodiff backward pass.
+ *
+ * Conventions.  Row-major, float32, metres / radians.  Every function returns a
+ * psdf_status (0 ok, <0 error); nothing throws, aborts or prints.  On error the outputs
+ * are untouched.  "device" pointers are CUDA device memory of the current device,
+ * "host" pointers ordinary host memory.  `cuda_stream` is a cudaStream_t passed as
+ * void* (NULL = legacy default stream).  The caller owns every I/O buffer and the stream;
+ * the library copies the scene at create/update and owns that copy.
+ *
+ * Thread-safety: calls that use the same psdf_scene must be ordered on ONE stream (the
+ * scene carries a small device workspace); different scenes are independent.
+ */
+#ifndef PSDF_H_
+#define PSDF_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct psdf_scene psdf_scene; /* opaque; owns packed device scene + workspace + graph */
+
+typedef enum {
+  PSDF_OK = 0,
+  PSDF_ERR_INVALID_ARG = -1, /* null pointer, V outside [3,16], E<3, M<1, N<0 */
+  PSDF_ERR_DEGENERATE = -2,  /* violates Assumption 1: edge shorter than 1e-6 m,
+                                non-empty row with <3 valid edges, row that is not a closed
+                                convex polygon, footprint not convex counter-clockwise */
+  PSDF_ERR_CAPACITY = -3,    /* N > max_poses given at create */
+  PSDF_ERR_CUDA = -4,        /* a CUDA call failed (psdf_last_cuda_error() has the code) */
+  PSDF_ERR_ALLOC = -5
+} psdf_status;
+
+typedef enum { PSDF_MEM_HOST = 0, PSDF_MEM_DEVICE = 1 } psdf_mem;
+
+/* EncodeEdges + upload (Alg.1 l.1-4; eq.(10)).
+ *   footprint  host [V,2]   robot vertices in the robot-local frame, CCW
+ *   A, B       [M,E,2]      edge start / end points, world frame; `where` says host or device
+ *   S          [M,E] uint8  1 = valid edge, 0 = padded entry (any position, any garbage
+ *                           in A/B there); a row with no valid entry is an absent obstacle
+ *   max_poses  capacity for N in later psdf_eval / psdf_eval_host calls
+ * Valid entries of a row, in slot order, must form one closed convex polygon
+ * (B_j == A_next bitwise), either orientation.  Blocks until the upload has finished. */
+psdf_status psdf_create_scene(const float* footprint, int V, const float* A, const float* B,
+                              const uint8_t* S, int M, int E, psdf_mem where, int max_poses,
+                              void* cuda_stream, psdf_scene** out);
+
+/* Perception update: same (M,E), new values only.  On error the old scene
+ * stays in force.  Blocks until the upload has finished. */
+psdf_status psdf_update_scene(psdf_scene* scene, const float* A, const float* B, const uint8_t* S,
+                              psdf_mem where, void* cuda_stream);
+
+/* Batched evaluation (Alg.1 l.5-7), asynchronous on `cuda_stream`:
+ * no host synchronisation, no allocation.
+ *   poses         device [N,3]  (x, y, theta) per pose
+ *   value         device [N]    phi                                    eq.(6)
+ *   grad          device [N,3]  (d phi/dx, d phi/dy, d phi/dtheta), PLUS sign (the paper's
+ *                               J_g = -grad);  NULL = value-only
+ *   per_obstacle  device [N,M]  sd^i per obstacle row (eq.23), +INF for a row with no valid
+ *                               edge;  NULL = not wanted
+ * No valid obstacle at all: value=+INF, grad=0.  Non-finite pose: NaN outputs.
+ * At ties / kinks the gradient is that of one of the tied branches. */
+psdf_status psdf_eval(psdf_scene* scene, const float* poses, int N, float* value, float* grad,
+                      float* per_obstacle, void* cuda_stream);
+
+/* MPC-sized path: same semantics with HOST buffers.  Copies the poses into the scene's
+ * pinned staging buffer, replays a captured CUDA graph {H2D, kernel, D2H} on the scene's
+ * own stream, synchronises, copies the results out.  grad / per_obstacle may be NULL. */
+psdf_status psdf_eval_host(psdf_scene* scene, const float* poses, int N, float* value, float* grad,
+                           float* per_obstacle);
+
+/* MPC coefficient epilogue (Alg.1 l.7-11; eqs.(26)-(28)):
+ * for each stage s writes coeff[s] = [ h_s - gamma_s ; J_g,s ] with h_s = phi_s - d_min,
+ * J_g,s = -grad phi_s, gamma_s = 0.5 (r_max + phi_s) rho_theta^2 + rho_p rho_theta,
+ * r_max = max_l |v_l|.  coeff: host [N,4].  Same graph path as psdf_eval_host. */
+psdf_status psdf_mpc_coeffs_host(psdf_scene* scene, const float* poses, int N, float d_min,
+                                 float rho_p, float rho_theta, float* coeff);
+
+void psdf_destroy_scene(psdf_scene* scene);
+
+/* Introspection (no CUDA work). */
+int psdf_scene_num_obstacles(const psdf_scene* scene);   /* rows with >=1 valid edge */
+int psdf_scene_num_edges(const psdf_scene* scene);       /* total valid edges */
+int psdf_last_cuda_error(void);                          /* cudaError_t of the last failure */
+long long psdf_kernel_launches(void);                    /* kernels launched by this library */
+const char* psdf_status_string(psdf_status status);
+const char* psdf_version(void);
+
+/* Measurement helper: FP32 FMA-only micro-kernel, returns achieved TFLOP/s on the
+ * current device (used by bench.py for the measured FP32 roofline denominator). */
+psdf_status psdf_measure_fp32_peak(int iters, void* cuda_stream, double* tflops_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PSDF_H_ */

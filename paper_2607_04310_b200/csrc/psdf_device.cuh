@@ -1,0 +1,211 @@
+// Device-side PSDF arithmetic for sm_100a (no code shared with oracle/).
+//
+// Formulation (equivalent to PAPER.md eqs.(11)-(23) by rigid-motion
+// invariance and one-sided SAT):
+//   * pose-relative world frame: r_l = R(theta) v_l (posed robot vertex minus p) and
+//     a_j = A_j - p; rotation is applied to the footprint once per pose instead of to
+//     every obstacle endpoint (eq.(11) PAPER.md:141-145 moved onto eq.(9));
+//   * obstacle edge j has unit tangent t_j, inward unit normal n_j = rot90(t_j) (CCW),
+//     half length h_j; robot edge l has rotated tangent T_l, inward normal N_l;
+//   * per (l, j):  sigma = (r_l - a_j).n_j, tau_m = (r_l - a_j).t_j - h_j   (pool 1,
+//     eqs.(12)-(14) PAPER.md:153-167) and sigma' = (a_j - r_l).N_l,
+//     tau'_m = (a_j - r_l).T_l - h_l (pool 2, eq.(15));
+//     point-to-segment d^2 = sigma^2 + (max(|tau_m|, h) - h)^2  (eq.(13) with the clamp
+//     of eq.(12) written around the edge midpoint);
+//   * SAT (eqs.(17)-(22) PAPER.md:181-217), one-sided: face depth G_j = max_l sigma,
+//     G'_l = max_j sigma'; depth^i = min over the faces of both polygons; separated^i
+//     <=> depth^i < 0 (eq.21); pen = depth^i otherwise (eq.22) — the "other side" term of
+//     eq.(20) can never be the minimum;
+//   * phi = -max_i depth^i if any depth^i >= 0 else sqrt(min over everything of d^2)
+//     (eqs.(23),(6) PAPER.md:221-225, 93-95).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace psdf {
+
+constexpr int kMaxV = 16;
+constexpr float kInf = __builtin_huge_valf();
+
+// One packed valid edge, 32 bytes (two float4): built in double at scene creation (H0).
+struct __align__(16) EdgeRec {
+  float ax, ay;   // edge start A_j, world frame (the obstacle vertex of eq.(15))
+  float tx, ty;   // unit tangent; inward normal is (-ty, tx)
+  float h;        // half length |B-A|/2
+  int last;       // -1, or the obstacle row index if this is the row's last valid edge
+  int slot;       // packed obstacle index (0..Mv-1)
+  float pad;
+};
+
+// Footprint constants (pose independent), passed by value as a kernel parameter so that
+// the unrolled loops read them as constant-bank operands.
+struct Footprint {
+  float vx[kMaxV], vy[kMaxV];   // vertices v_l (robot-local)
+  float tx[kMaxV], ty[kMaxV];   // unit edge tangents t~_l of E_l = [v_l, v_{l+1}]
+  float h[kMaxV];               // half lengths
+  float cN[kMaxV];              // v_l . n~_l      (n~_l = rot90(t~_l), inward)
+  float cT[kMaxV];              // v_l . t~_l + h_l
+  float rmax;                   // max_l |v_l|  (Prop.1)
+};
+
+// Per-pose state: posed footprint in registers (H1).
+template <int V>
+struct Posed {
+  float px, py;
+  float rx[V], ry[V];   // r_l = R v_l
+  float Tx[V], Ty[V];   // T_l = R t~_l
+};
+
+template <int V>
+__device__ __forceinline__ void pose_setup(const Footprint& fp, float x, float y, float th, Posed<V>& P) {
+  float s, c;
+  sincosf(th, &s, &c);                       // full-accuracy (not __sincosf): reading G13
+  P.px = x;
+  P.py = y;
+#pragma unroll
+  for (int l = 0; l < V; ++l) {
+    P.rx[l] = c * fp.vx[l] - s * fp.vy[l];
+    P.ry[l] = s * fp.vx[l] + c * fp.vy[l];
+    P.Tx[l] = c * fp.tx[l] - s * fp.ty[l];
+    P.Ty[l] = s * fp.tx[l] + c * fp.ty[l];
+  }
+}
+
+// Scan accumulators for the obstacle currently being traversed.
+template <int V>
+struct ObstacleAcc {
+  float gR[V];   // G'_l = max_j sigma'   (robot faces)
+  float gO;      // min_j G_j             (obstacle faces)
+  __device__ __forceinline__ void reset() {
+#pragma unroll
+    for (int l = 0; l < V; ++l) gR[l] = -kInf;
+    gO = kInf;
+  }
+  __device__ __forceinline__ float depth() const {
+    float d = gO;
+#pragma unroll
+    for (int l = 0; l < V; ++l) d = fminf(d, gR[l]);
+    return d;
+  }
+};
+
+// Hot inner step H2-H5 for one packed edge against all V robot vertices/edges.
+// minD2 is min-updated with the 2V point-to-segment candidates of this edge.
+template <int V>
+__device__ __forceinline__ void edge_step(const Footprint& fp, const Posed<V>& P, const float4 e0,
+                                          const float h, ObstacleAcc<V>& acc, float& minD2) {
+  const float ax = e0.x - P.px, ay = e0.y - P.py;   // H2: a_j = A_j - p
+  const float tx = e0.z, ty = e0.w;
+  const float cn = fmaf(ay, tx, -ax * ty);          // a_j . n_j,  n_j = (-ty, tx)
+  const float ct = fmaf(ax, tx, fmaf(ay, ty, h));   // a_j . t_j + h_j
+  float gj = -kInf;
+  float m = minD2;
+#pragma unroll
+  for (int l = 0; l < V; ++l) {
+    // pool 1 + obstacle axis j
+    const float sig = fmaf(P.ry[l], tx, fmaf(-P.rx[l], ty, -cn));
+    const float tau = fmaf(P.rx[l], tx, fmaf(P.ry[l], ty, -ct));
+    const float e1 = fmaxf(fabsf(tau), h) - h;
+    const float d1 = fmaf(e1, e1, sig * sig);
+    gj = fmaxf(gj, sig);
+    // pool 2 + robot axis l
+    const float sigp = fmaf(ay, P.Tx[l], fmaf(-ax, P.Ty[l], -fp.cN[l]));
+    const float taup = fmaf(ax, P.Tx[l], fmaf(ay, P.Ty[l], -fp.cT[l]));
+    const float e2 = fmaxf(fabsf(taup), fp.h[l]) - fp.h[l];
+    const float d2 = fmaf(e2, e2, sigp * sigp);
+    acc.gR[l] = fmaxf(acc.gR[l], sigp);
+    m = fminf(fminf(m, d1), d2);
+  }
+  acc.gO = fminf(acc.gO, gj);
+  minD2 = m;
+}
+
+// Order-preserving float -> uint32 key (works for negatives and +-inf).
+__device__ __forceinline__ uint32_t fkey(float f) {
+  uint32_t u = __float_as_uint(f);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float fkey_inv(uint32_t k) {
+  return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
+}
+
+// H8: analytic gradient at the arg-min witness of obstacle [e_begin, e_end), re-evaluated
+// with full witness tracking (only the winning obstacle: 1/M of the scan work).
+//   separated:   n = unit vector from the obstacle witness to the robot witness, c = robot
+//                witness (pose-relative);   not separated: n = push-out normal of the
+//                minimum-overlap face, c = deepest vertex.   grad = (n_x, n_y, c x n).
+template <int V>
+__device__ __forceinline__ void witness_gradient(const Footprint& fp, const Posed<V>& P,
+                                                 const EdgeRec* __restrict__ edges, int e_begin,
+                                                 int e_end, bool separated, float* g) {
+  float nx = 0.f, ny = 0.f, cx = 0.f, cy = 0.f;
+  if (separated) {
+    float best = kInf;
+    for (int k = e_begin; k < e_end; ++k) {
+      const float4 e0 = __ldg(reinterpret_cast<const float4*>(edges + k));
+      const float h = __ldg(&edges[k].h);
+      const float ax = e0.x - P.px, ay = e0.y - P.py, tx = e0.z, ty = e0.w;
+#pragma unroll
+      for (int l = 0; l < V; ++l) {
+        const float dx = P.rx[l] - ax, dy = P.ry[l] - ay;
+        {  // pool 1: robot vertex l -> obstacle edge k.  (w - Q) = sig n + ex t
+          const float sig = dy * tx - dx * ty;
+          const float tm = fmaf(dx, tx, dy * ty) - h;
+          const float ex = copysignf(fmaxf(fabsf(tm), h) - h, tm);
+          const float d2 = fmaf(ex, ex, sig * sig);
+          if (d2 < best) {
+            best = d2;
+            const float inv = rsqrtf(fmaxf(d2, 1e-30f));
+            nx = (ex * tx - sig * ty) * inv;
+            ny = (ex * ty + sig * tx) * inv;
+            cx = P.rx[l];
+            cy = P.ry[l];
+          }
+        }
+        {  // pool 2: obstacle vertex a_k -> robot edge l.  (a - Q) = sig' N + ex' T
+          const float Tx = P.Tx[l], Ty = P.Ty[l];
+          const float sig = -(dy * Tx - dx * Ty);
+          const float tm = -fmaf(dx, Tx, dy * Ty) - fp.h[l];
+          const float ex = copysignf(fmaxf(fabsf(tm), fp.h[l]) - fp.h[l], tm);
+          const float d2 = fmaf(ex, ex, sig * sig);
+          if (d2 < best) {
+            best = d2;
+            const float inv = rsqrtf(fmaxf(d2, 1e-30f));
+            const float ux = (ex * Tx - sig * Ty), uy = (ex * Ty + sig * Tx);  // a - Q
+            nx = -ux * inv;
+            ny = -uy * inv;
+            cx = ax - ux;
+            cy = ay - uy;
+          }
+        }
+      }
+    }
+  } else {
+    float best = kInf;       // minimum face depth
+    float gR[V], gcx[V], gcy[V];
+#pragma unroll
+    for (int l = 0; l < V; ++l) { gR[l] = -kInf; gcx[l] = 0.f; gcy[l] = 0.f; }
+    for (int k = e_begin; k < e_end; ++k) {
+      const float4 e0 = __ldg(reinterpret_cast<const float4*>(edges + k));
+      const float ax = e0.x - P.px, ay = e0.y - P.py, tx = e0.z, ty = e0.w;
+      float gj = -kInf, wx = 0.f, wy = 0.f;
+#pragma unroll
+      for (int l = 0; l < V; ++l) {
+        const float dx = P.rx[l] - ax, dy = P.ry[l] - ay;
+        const float sig = dy * tx - dx * ty;
+        if (sig > gj) { gj = sig; wx = P.rx[l]; wy = P.ry[l]; }
+        const float sigp = -(dy * P.Tx[l] - dx * P.Ty[l]);
+        if (sigp > gR[l]) { gR[l] = sigp; gcx[l] = ax; gcy[l] = ay; }
+      }
+      if (gj < best) { best = gj; nx = ty; ny = -tx; cx = wx; cy = wy; }   // n = -n_in
+    }
+#pragma unroll
+    for (int l = 0; l < V; ++l)
+      if (gR[l] < best) { best = gR[l]; nx = -P.Ty[l]; ny = P.Tx[l]; cx = gcx[l]; cy = gcy[l]; }
+  }
+  g[0] = nx;
+  g[1] = ny;
+  g[2] = cx * ny - cy * nx;
+}
+
+}  // namespace psdf

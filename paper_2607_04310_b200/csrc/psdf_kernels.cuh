@@ -1,0 +1,229 @@
+// PSDF kernels for sm_100a: the tile-scan kernel (one thread per pose, packed edges staged
+// through shared memory with cp.async and broadcast to all poses of the CTA) and the
+// lane-split kernel (K lanes per pose, obstacles split across lanes, warp-shuffle arg-min)
+// for MPC-sized batches.  See DESIGN.md §6.
+#pragma once
+#include "psdf_device.cuh"
+
+namespace psdf {
+
+constexpr int kTileEdges = 128;    // records per shared-memory tile (4 KB), double buffered
+constexpr int kMaxChunks = 64;
+
+enum Mode : int { kGrad = 1, kPerObs = 2, kCoeff = 4 };
+
+struct EvalParams {
+  const EdgeRec* edges;        // [n_edges] packed valid edges, grouped by obstacle
+  const int* row_begin;        // [Mv+1] packed obstacle -> first edge
+  const int* empty_rows;       // [n_empty] obstacle rows with no valid edge
+  const float* poses;          // [N,3]
+  float* value;                // [N]
+  float* grad;                 // [N,3] or null
+  float* per_obs;              // [N,M_rows] or null
+  float* coeff;                // [N,4] or null (kCoeff)
+  unsigned long long* ws_depth;  // [max_poses] cross-chunk arg-max keys (clean = 0)
+  unsigned long long* ws_d2;     // [max_poses] cross-chunk arg-min keys (clean = ~0)
+  unsigned int* ws_count;        // [pose tiles] arrival counters (clean = 0)
+  int n_edges, Mv, M_rows, n_empty, N;
+  int n_chunks;
+  int lanes;                   // lane-split kernel: lanes per pose (power of two <= 32)
+  float d_min, rho_p, rho_theta;
+  int chunk_begin[kMaxChunks + 1];   // edge offsets of the obstacle chunks
+};
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  unsigned s = static_cast<unsigned>(__cvta_generic_to_shared(smem));
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N_>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N_)); }
+
+// H6-H8 tail shared by both kernels: value, gradient (or MPC coefficients), stores.
+template <int V, int MODE>
+__device__ __forceinline__ void finalize_pose(const Footprint& fp, const EvalParams& p, const Posed<V>& P,
+                                              int n, float th, float value, int slot, bool separated) {
+  const bool finite = isfinite(P.px) && isfinite(P.py) && isfinite(th);
+  float g[3] = {0.f, 0.f, 0.f};
+  if (!finite) {
+    value = __int_as_float(0x7fc00000);
+    g[0] = g[1] = g[2] = value;
+  } else if (slot < 0) {
+    value = kInf;                                  // no valid obstacle at all
+  } else if (MODE & (kGrad | kCoeff)) {
+    witness_gradient<V>(fp, P, p.edges, __ldg(p.row_begin + slot), __ldg(p.row_begin + slot + 1),
+                        separated, g);
+  }
+  p.value[n] = value;
+  if (MODE & kGrad) {
+    p.grad[3 * n + 0] = g[0];
+    p.grad[3 * n + 1] = g[1];
+    p.grad[3 * n + 2] = g[2];
+  }
+  if (MODE & kCoeff) {
+    // [h_s - gamma_s ; J_g,s], eqs.(26)-(28) PAPER.md:247-268; J_g = -grad phi.
+    const float gamma = 0.5f * (fp.rmax + value) * p.rho_theta * p.rho_theta + p.rho_p * p.rho_theta;
+    reinterpret_cast<float4*>(p.coeff)[n] = make_float4(value - p.d_min - gamma, -g[0], -g[1], -g[2]);
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// Tile-scan kernel.  grid = (pose tiles, obstacle chunks), block = BD threads = BD poses.
+template <int V, int MODE>
+__global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ Footprint fp,
+                                                        const __grid_constant__ EvalParams p) {
+  __shared__ float4 tile[2][kTileEdges * 2];
+  __shared__ int s_is_last;
+  const int tid = threadIdx.x, bd = blockDim.x;
+  const int n_raw = blockIdx.x * bd + tid;
+  const int n = min(n_raw, p.N - 1);               // tail threads recompute the last pose
+  const float x = __ldg(p.poses + 3 * n), y = __ldg(p.poses + 3 * n + 1), th = __ldg(p.poses + 3 * n + 2);
+  Posed<V> P;
+  pose_setup<V>(fp, x, y, th, P);
+
+  const int cb = p.chunk_begin[blockIdx.y], ce = p.chunk_begin[blockIdx.y + 1];
+  const int n_tiles = (ce - cb + kTileEdges - 1) / kTileEdges;
+  const float4* gsrc = reinterpret_cast<const float4*>(p.edges);
+
+  auto issue = [&](int t) {
+    const int e0 = cb + t * kTileEdges;
+    const int cnt = min(kTileEdges, ce - e0) * 2;  // float4 count
+    for (int i = tid; i < cnt; i += bd) cp_async16(&tile[t & 1][i], gsrc + 2 * (size_t)e0 + i);
+    cp_async_commit();
+  };
+
+  ObstacleAcc<V> acc;
+  acc.reset();
+  float minD2 = kInf, prevD2 = kInf, maxDepth = -kInf;
+  int idD2 = -1, idDepth = -1;
+
+  if (n_tiles > 0) issue(0);
+  for (int t = 0; t < n_tiles; ++t) {
+    if (t + 1 < n_tiles) {
+      issue(t + 1);
+      cp_async_wait<1>();
+    } else {
+      cp_async_wait<0>();
+    }
+    __syncthreads();
+    const float4* buf = tile[t & 1];
+    const int cnt = min(kTileEdges, ce - (cb + t * kTileEdges));
+#pragma unroll 1
+    for (int k = 0; k < cnt; ++k) {
+      const float4 e0 = buf[2 * k];
+      const float4 e1 = buf[2 * k + 1];
+      edge_step<V>(fp, P, e0, e1.x, acc, minD2);
+      const int last = __float_as_int(e1.y);
+      if (last >= 0) {                             // uniform: end of an obstacle (H6, H7)
+        const int slot = __float_as_int(e1.z);
+        const float depth = acc.depth();
+        if (MODE & kPerObs) {
+          if (n_raw < p.N)
+            p.per_obs[(size_t)n * p.M_rows + last] = depth >= 0.f ? -depth : sqrtf(minD2);
+          if (minD2 < prevD2) { prevD2 = minD2; idD2 = slot; }
+          minD2 = kInf;
+        } else if (MODE & (kGrad | kCoeff)) {
+          if (minD2 < prevD2) { prevD2 = minD2; idD2 = slot; }
+        }
+        if (depth > maxDepth) { maxDepth = depth; idDepth = slot; }
+        acc.reset();
+      }
+    }
+    __syncthreads();
+  }
+  if (MODE & kPerObs) {
+    minD2 = prevD2;
+    if (blockIdx.y == 0 && n_raw < p.N)
+      for (int r = 0; r < p.n_empty; ++r) p.per_obs[(size_t)n * p.M_rows + __ldg(p.empty_rows + r)] = kInf;
+  } else if (!(MODE & (kGrad | kCoeff))) {
+    idD2 = minD2 < kInf ? 0 : -1;                  // value-only: winner id not tracked
+  }
+
+  if (p.n_chunks > 1) {
+    // cross-chunk arg-min/arg-max through 64-bit keys; the last CTA to arrive finalises.
+    if (n_raw < p.N) {
+      if (idDepth >= 0)
+        atomicMax(p.ws_depth + n, ((unsigned long long)fkey(maxDepth) << 32) | (0xffffffffu - (unsigned)idDepth));
+      if (idD2 >= 0)
+        atomicMin(p.ws_d2 + n, ((unsigned long long)__float_as_uint(minD2) << 32) | (unsigned)idD2);
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) s_is_last = (atomicAdd(p.ws_count + blockIdx.x, 1u) == (unsigned)p.n_chunks - 1u);
+    __syncthreads();
+    if (!s_is_last) return;
+    __threadfence();
+    if (tid == 0) p.ws_count[blockIdx.x] = 0u;     // leave the workspace clean for the next call
+    if (n_raw >= p.N) return;
+    const unsigned long long kd = __ldcg(p.ws_depth + n), k2 = __ldcg(p.ws_d2 + n);
+    p.ws_depth[n] = 0ull;
+    p.ws_d2[n] = ~0ull;
+    maxDepth = kd ? fkey_inv((uint32_t)(kd >> 32)) : -kInf;
+    idDepth = kd ? (int)(0xffffffffu - (uint32_t)kd) : -1;
+    minD2 = (k2 != ~0ull) ? __uint_as_float((uint32_t)(k2 >> 32)) : kInf;
+    idD2 = (k2 != ~0ull) ? (int)(uint32_t)k2 : -1;
+  }
+  if (n_raw >= p.N) return;
+  const bool separated = !(maxDepth >= 0.f);
+  const float value = separated ? sqrtf(minD2) : -maxDepth;
+  finalize_pose<V, MODE>(fp, p, P, n, th, value, separated ? idD2 : idDepth, separated);
+}
+
+// ------------------------------------------------------------------------------------------
+// Lane-split kernel for small batches: K = p.lanes lanes per pose, lane k takes obstacles
+// k, k+K, ...; (sd^i, i) arg-min by warp shuffle; lane 0 of the group finalises.
+template <int V, int MODE>
+__global__ void __launch_bounds__(128) psdf_lanes_kernel(const __grid_constant__ Footprint fp,
+                                                         const __grid_constant__ EvalParams p) {
+  const int K = p.lanes;
+  const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
+  const int n_raw = gtid / K, lane = gtid % K;
+  const int n = min(n_raw, p.N - 1);
+  const float x = __ldg(p.poses + 3 * n), y = __ldg(p.poses + 3 * n + 1), th = __ldg(p.poses + 3 * n + 2);
+  Posed<V> P;
+  pose_setup<V>(fp, x, y, th, P);
+  unsigned long long best = ~0ull;
+  ObstacleAcc<V> acc;
+  for (int slot = lane; slot < p.Mv; slot += K) {
+    const int eb = __ldg(p.row_begin + slot), ee = __ldg(p.row_begin + slot + 1);
+    acc.reset();
+    float d2 = kInf;
+    for (int k = eb; k < ee; ++k) {
+      const float4 e0 = __ldg(reinterpret_cast<const float4*>(p.edges + k));
+      edge_step<V>(fp, P, e0, __ldg(&p.edges[k].h), acc, d2);
+    }
+    const float depth = acc.depth();
+    const float sd = depth >= 0.f ? -depth : sqrtf(d2);            // eq.(23)
+    if ((MODE & kPerObs) && n_raw < p.N)
+      p.per_obs[(size_t)n * p.M_rows + __ldg(&p.edges[ee - 1].last)] = sd;
+    const unsigned long long key = ((unsigned long long)fkey(sd) << 32) | (unsigned)slot;
+    best = key < best ? key : best;
+  }
+  if ((MODE & kPerObs) && n_raw < p.N)
+    for (int r = lane; r < p.n_empty; r += K) p.per_obs[(size_t)n * p.M_rows + __ldg(p.empty_rows + r)] = kInf;
+  for (int o = K >> 1; o > 0; o >>= 1) {
+    const unsigned long long other = __shfl_xor_sync(0xffffffffu, best, o);
+    best = other < best ? other : best;
+  }
+  if (lane != 0 || n_raw >= p.N) return;
+  const bool any = best != ~0ull;
+  const float value = any ? fkey_inv((uint32_t)(best >> 32)) : kInf;
+  finalize_pose<V, MODE>(fp, p, P, n, th, value, any ? (int)(uint32_t)best : -1, value > 0.f);
+}
+
+// FP32 FMA-only micro-kernel for the measured roofline denominator (bench.py).
+__global__ void fp32_peak_kernel(float* out, int iters, float a, float b) {
+  float acc[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) acc[i] = threadIdx.x * 1e-3f + i;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) acc[i] = fmaf(acc[i], a, b);
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += acc[i];
+  if (s == 123.456f) out[0] = s;
+}
+
+}  // namespace psdf

@@ -1,0 +1,244 @@
+"""Thin ctypes binding over libpsdf.so (include/psdf.h), same names as the C ABI.
+
+Argument marshalling only: every step of the hot path runs in the CUDA kernels.
+PyTorch is used for device memory and streams.  There is NO CPU fallback: if the
+library is missing or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpsdf.so")
+
+PSDF_OK = 0
+PSDF_ERR_INVALID_ARG = -1
+PSDF_ERR_DEGENERATE = -2
+PSDF_ERR_CAPACITY = -3
+PSDF_ERR_CUDA = -4
+PSDF_ERR_ALLOC = -5
+PSDF_MEM_HOST = 0
+PSDF_MEM_DEVICE = 1
+
+EXPORTS = ["psdf_create_scene", "psdf_update_scene", "psdf_eval", "psdf_eval_host",
+           "psdf_mpc_coeffs_host", "psdf_destroy_scene", "psdf_scene_num_obstacles",
+           "psdf_scene_num_edges", "psdf_last_cuda_error", "psdf_kernel_launches",
+           "psdf_status_string", "psdf_version", "psdf_measure_fp32_peak"]
+
+_lib = None
+
+
+class PsdfError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = int(status)
+        msg = lib().psdf_status_string(int(status)).decode()
+        extra = f" (cudaError {lib().psdf_last_cuda_error()})" if status == PSDF_ERR_CUDA else ""
+        super().__init__(f"{where}: {msg}{extra}")
+
+
+def lib():
+    """Loads libpsdf.so (built in-tree by paper_2607_04310_b200/build.py); fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2607_04310_b200.build` "
+                          "(there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, fp_, u8p = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p
+    i = ctypes.c_int
+    L.psdf_create_scene.restype = i
+    L.psdf_create_scene.argtypes = [fp_, i, fp_, fp_, u8p, i, i, i, i, vp, ctypes.POINTER(vp)]
+    L.psdf_update_scene.restype = i
+    L.psdf_update_scene.argtypes = [vp, fp_, fp_, u8p, i, vp]
+    L.psdf_eval.restype = i
+    L.psdf_eval.argtypes = [vp, fp_, i, fp_, fp_, fp_, vp]
+    L.psdf_eval_host.restype = i
+    L.psdf_eval_host.argtypes = [vp, fp_, i, fp_, fp_, fp_]
+    L.psdf_mpc_coeffs_host.restype = i
+    L.psdf_mpc_coeffs_host.argtypes = [vp, fp_, i, ctypes.c_float, ctypes.c_float, ctypes.c_float, fp_]
+    L.psdf_destroy_scene.restype = None
+    L.psdf_destroy_scene.argtypes = [vp]
+    L.psdf_scene_num_obstacles.restype = i
+    L.psdf_scene_num_obstacles.argtypes = [vp]
+    L.psdf_scene_num_edges.restype = i
+    L.psdf_scene_num_edges.argtypes = [vp]
+    L.psdf_last_cuda_error.restype = i
+    L.psdf_kernel_launches.restype = ctypes.c_longlong
+    L.psdf_status_string.restype = ctypes.c_char_p
+    L.psdf_status_string.argtypes = [i]
+    L.psdf_version.restype = ctypes.c_char_p
+    L.psdf_measure_fp32_peak.restype = i
+    L.psdf_measure_fp32_peak.argtypes = [i, vp, ctypes.POINTER(ctypes.c_double)]
+    _lib = L
+    return L
+
+
+def _check(status, where):
+    if status != PSDF_OK:
+        raise PsdfError(status, where)
+
+
+def _host(a, dtype):
+    a = np.ascontiguousarray(a, dtype=dtype)
+    return a, a.ctypes.data
+
+
+def _is_torch(x):
+    return type(x).__module__.startswith("torch")
+
+
+def _dev_ptr(t, dtype_name, shape_last=None):
+    import torch
+    assert t.is_cuda and t.is_contiguous(), "device tensors must be contiguous CUDA tensors"
+    assert t.dtype == getattr(torch, dtype_name), f"expected {dtype_name}, got {t.dtype}"
+    return t.data_ptr()
+
+
+def _stream_ptr(stream=None):
+    """cudaStream_t of `stream` (a torch.cuda.Stream), else torch's current stream; the
+    legacy default stream (NULL) when torch has no CUDA device to ask."""
+    if stream is not None:
+        return ctypes.c_void_p(stream.cuda_stream)
+    try:
+        import torch
+        if torch.cuda.is_available():
+            return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    except ImportError:
+        pass
+    return ctypes.c_void_p(0)
+
+
+def psdf_kernel_launches() -> int:
+    return int(lib().psdf_kernel_launches())
+
+
+def psdf_version() -> str:
+    return lib().psdf_version().decode()
+
+
+def psdf_measure_fp32_peak(iters: int = 4096, stream=None) -> float:
+    out = ctypes.c_double(0.0)
+    _check(lib().psdf_measure_fp32_peak(int(iters), _stream_ptr(stream), ctypes.byref(out)),
+           "psdf_measure_fp32_peak")
+    return out.value
+
+
+class Scene:
+    """Owns a psdf_scene*.  Methods mirror the C entry points."""
+
+    def __init__(self, footprint, A, B, S, max_poses, stream=None):
+        fp, fp_ptr = _host(footprint, np.float32)
+        self.V = int(fp.shape[0])
+        if _is_torch(A):
+            M, E = int(S.shape[0]), int(S.shape[1])
+            pa, pb = _dev_ptr(A, "float32"), _dev_ptr(B, "float32")
+            ps = _dev_ptr(S, "uint8")
+            where = PSDF_MEM_DEVICE
+            keep = (A, B, S)
+        else:
+            A_, pa = _host(A, np.float32)
+            B_, pb = _host(B, np.float32)
+            S_, ps = _host(S, np.uint8)
+            M, E = int(S_.shape[0]), int(S_.shape[1])
+            assert A_.shape == (M, E, 2) and B_.shape == (M, E, 2)
+            where = PSDF_MEM_HOST
+            keep = (A_, B_, S_)
+        self.M, self.E, self.max_poses = M, E, int(max_poses)
+        h = ctypes.c_void_p()
+        _check(lib().psdf_create_scene(fp_ptr, self.V, pa, pb, ps, M, E, where, int(max_poses),
+                                       _stream_ptr(stream), ctypes.byref(h)), "psdf_create_scene")
+        del keep
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().psdf_destroy_scene(self._h)
+            self._h = None
+
+    __del__ = close
+
+    @property
+    def num_obstacles(self):
+        return int(lib().psdf_scene_num_obstacles(self._h))
+
+    @property
+    def num_edges(self):
+        return int(lib().psdf_scene_num_edges(self._h))
+
+    def update(self, A, B, S, stream=None):
+        """psdf_update_scene: same (M,E), values only."""
+        if _is_torch(A):
+            args = (_dev_ptr(A, "float32"), _dev_ptr(B, "float32"), _dev_ptr(S, "uint8"), PSDF_MEM_DEVICE)
+        else:
+            A_, pa = _host(A, np.float32)
+            B_, pb = _host(B, np.float32)
+            S_, ps = _host(S, np.uint8)
+            assert S_.shape == (self.M, self.E)
+            args = (pa, pb, ps, PSDF_MEM_HOST)
+        _check(lib().psdf_update_scene(self._h, *args, _stream_ptr(stream)), "psdf_update_scene")
+
+    def eval(self, poses, value=None, grad=True, per_obstacle=False, stream=None):
+        """psdf_eval on device tensors (async on the stream).  `grad` / `per_obstacle` may
+        be False (not wanted), True (allocate) or a preallocated tensor."""
+        import torch
+        N = int(poses.shape[0])
+        pp = _dev_ptr(poses, "float32")
+        if value is None:
+            value = torch.empty(N, dtype=torch.float32, device=poses.device)
+        if grad is True:
+            grad = torch.empty((N, 3), dtype=torch.float32, device=poses.device)
+        if per_obstacle is True:
+            per_obstacle = torch.empty((N, self.M), dtype=torch.float32, device=poses.device)
+        pg = _dev_ptr(grad, "float32") if grad is not False and grad is not None else None
+        po = _dev_ptr(per_obstacle, "float32") if per_obstacle is not False and per_obstacle is not None else None
+        _check(lib().psdf_eval(self._h, pp, N, _dev_ptr(value, "float32"), pg, po, _stream_ptr(stream)),
+               "psdf_eval")
+        return value, (grad if pg else None), (per_obstacle if po else None)
+
+    def eval_host(self, poses, grad=True, per_obstacle=False):
+        """psdf_eval_host on numpy arrays (CUDA-graph replay, returns after sync)."""
+        poses, pp = _host(poses, np.float32)
+        N = int(poses.shape[0])
+        value = np.empty(N, np.float32)
+        g = np.empty((N, 3), np.float32) if grad else None
+        po = np.empty((N, self.M), np.float32) if per_obstacle else None
+        _check(lib().psdf_eval_host(self._h, pp, N, value.ctypes.data,
+                                    g.ctypes.data if g is not None else None,
+                                    po.ctypes.data if po is not None else None), "psdf_eval_host")
+        return value, g, po
+
+    def mpc_coeffs_host(self, poses, d_min, rho_p, rho_theta):
+        poses, pp = _host(poses, np.float32)
+        N = int(poses.shape[0])
+        coeff = np.empty((N, 4), np.float32)
+        _check(lib().psdf_mpc_coeffs_host(self._h, pp, N, float(d_min), float(rho_p), float(rho_theta),
+                                          coeff.ctypes.data), "psdf_mpc_coeffs_host")
+        return coeff
+
+
+def psdf_create_scene(footprint, A, B, S, max_poses, stream=None) -> Scene:
+    return Scene(footprint, A, B, S, max_poses, stream)
+
+
+def psdf_eval(scene: Scene, poses, **kw):
+    return scene.eval(poses, **kw)
+
+
+def psdf_eval_host(scene: Scene, poses, **kw):
+    return scene.eval_host(poses, **kw)
+
+
+def psdf_update_scene(scene: Scene, A, B, S, stream=None):
+    return scene.update(A, B, S, stream)
+
+
+def psdf_mpc_coeffs_host(scene: Scene, poses, d_min, rho_p, rho_theta):
+    return scene.mpc_coeffs_host(poses, d_min, rho_p, rho_theta)
+
+
+def psdf_destroy_scene(scene: Scene):
+    scene.close()

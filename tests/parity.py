@@ -1,0 +1,38 @@
+"""Shared GPU-vs-oracle comparison (the bar of BASELINE.json.north_star):
+|d value| <= 1e-5 m everywhere; gradient relative error <= 1e-3 where the oracle's
+arg-min margin exceeds 1e-4 m and |phi| > 1e-3 m (reading G9)."""
+import numpy as np
+
+VALUE_TOL = 1e-5
+GRAD_REL_TOL = 1e-3
+MARGIN_MIN = 1e-4
+PHI_MIN = 1e-3
+
+
+def compare(ref, value, grad=None, per_obstacle=None, what=""):
+    value = np.asarray(value, np.float64)
+    fin = np.isfinite(ref.value)
+    assert np.array_equal(np.isinf(value), ~fin), what
+    dv = np.abs(value[fin] - ref.value[fin])
+    stats = {"max_dvalue": float(dv.max()) if dv.size else 0.0}
+    assert stats["max_dvalue"] <= VALUE_TOL, (what, stats, int(np.argmax(dv)))
+    if grad is not None:
+        grad = np.asarray(grad, np.float64)
+        ok = fin & (ref.margin > MARGIN_MIN) & (np.abs(ref.value) > PHI_MIN)
+        den = np.linalg.norm(ref.grad[ok], axis=1)
+        rel = np.linalg.norm(grad[ok] - ref.grad[ok], axis=1) / den
+        stats["grad_compared"] = float(ok.mean()) if ok.size else 0.0
+        stats["max_grad_rel"] = float(rel.max()) if rel.size else 0.0
+        if rel.size:
+            k = int(np.argmax(rel))
+            assert stats["max_grad_rel"] <= GRAD_REL_TOL, (what, stats, np.nonzero(ok)[0][k],
+                                                          grad[ok][k], ref.grad[ok][k])
+        assert np.isfinite(grad[fin]).all()
+    if per_obstacle is not None:
+        po = np.asarray(per_obstacle, np.float64)
+        pf = np.isfinite(ref.per_obstacle)
+        assert np.array_equal(np.isposinf(po), ~pf), what
+        dpo = np.abs(po[pf] - ref.per_obstacle[pf])
+        stats["max_dper_obstacle"] = float(dpo.max()) if dpo.size else 0.0
+        assert stats["max_dper_obstacle"] <= VALUE_TOL, (what, stats)
+    return stats

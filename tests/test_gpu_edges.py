@@ -1,0 +1,158 @@
+"""Edge cases of the C ABI on the GPU: empty / ragged inputs, masks, footprint sizes,
+orientation, updates, capacity, NaN poses, MPC coefficients."""
+import math
+
+import numpy as np
+import pytest
+
+from tests.parity import compare
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    from oracle import psdf_oracle as O
+    from paper_2607_04310_b200 import psdf, workloads as W
+    assert torch.cuda.is_available()
+    return torch, O, psdf, W
+
+
+def _run(torch, scene, poses, **kw):
+    v, g, po = scene.eval(torch.from_numpy(np.ascontiguousarray(poses, np.float32)).cuda(), **kw)
+    torch.cuda.synchronize()
+    return v.cpu().numpy(), None if g is None else g.cpu().numpy(), None if po is None else po.cpu().numpy()
+
+
+@pytest.mark.parametrize("V", [3, 5, 6, 7, 8, 9, 11, 13, 16])
+def test_footprint_vertex_counts(env, V):
+    """Rectangle, triangle, pentagon ... by changing only V0; V without a
+    compiled instance is padded with collinear midpoints."""
+    torch, O, psdf, W = env
+    rng = np.random.default_rng(100 + V)
+    fp = W.convex_kgon(rng, V, 0.6).astype(np.float32)
+    w = W.make_config(2)
+    poses = np.stack([rng.uniform(0, 20, 600), rng.uniform(0, 20, 600), rng.uniform(-7, 7, 600)], 1).astype(np.float32)
+    ref = O.evaluate(fp, w.A, w.B, w.S, poses, per_obstacle=True)
+    scene = psdf.Scene(fp, w.A, w.B, w.S, max_poses=600)
+    v, g, po = _run(torch, scene, poses, grad=True, per_obstacle=True)
+    print(V, compare(ref, v, g, po, what=f"V={V}"))
+    scene.close()
+
+
+def test_empty_and_degenerate_inputs(env):
+    torch, O, psdf, W = env
+    w = W.make_config(2)
+    scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=64)
+    # N = 0 is a no-op
+    v, g, _ = scene.eval(torch.empty((0, 3), dtype=torch.float32, device="cuda"))
+    assert v.numel() == 0 and g.numel() == 0
+    # N = 1
+    v, g, po = _run(torch, scene, w.poses[:1], grad=True, per_obstacle=True)
+    compare(O.evaluate(w.footprint, w.A, w.B, w.S, w.poses[:1], per_obstacle=True), v, g, po)
+    # capacity
+    with pytest.raises(psdf.PsdfError) as e:
+        scene.eval(torch.zeros((65, 3), dtype=torch.float32, device="cuda"))
+    assert e.value.status == psdf.PSDF_ERR_CAPACITY
+    # non-finite pose: NaN outputs, neighbours unaffected
+    poses = w.poses[:8].copy()
+    poses[3, 0] = np.nan
+    poses[5, 2] = np.inf
+    v, g, _ = _run(torch, scene, poses, grad=True)
+    assert np.isnan(v[[3, 5]]).all() and np.isnan(g[[3, 5]]).all()
+    keep = [0, 1, 2, 4, 6, 7]
+    compare(O.evaluate(w.footprint, w.A, w.B, w.S, poses[keep]), v[keep], g[keep])
+    # no valid obstacle at all: +inf, zero gradient, +inf per obstacle
+    scene.update(w.A, w.B, np.zeros_like(w.S))
+    v, g, po = _run(torch, scene, w.poses[:10], grad=True, per_obstacle=True)
+    assert np.isposinf(v).all() and (g == 0).all() and np.isposinf(po).all()
+    assert scene.num_obstacles == 0 and scene.num_edges == 0
+    # degenerate update is rejected and leaves the scene in force
+    S_bad = w.S.copy()
+    S_bad[0, np.nonzero(S_bad[0])[0][0]] = 0
+    with pytest.raises(psdf.PsdfError) as e:
+        scene.update(w.A, w.B, S_bad)
+    assert e.value.status == psdf.PSDF_ERR_DEGENERATE
+    v, _, _ = _run(torch, scene, w.poses[:10], grad=False)
+    assert np.isposinf(v).all()
+    scene.close()
+
+
+def test_masks_padding_orientation_update(env):
+    torch, O, psdf, W = env
+    w = W.make_config(2)
+    rng = np.random.default_rng(8)
+    ref = O.evaluate(w.footprint, w.A, w.B, w.S, w.poses, per_obstacle=True)
+    scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=w.N)
+    base = _run(torch, scene, w.poses, grad=True, per_obstacle=True)
+    # garbage in padded slots, extra masked rows and wider E are inert (bit-identical)
+    A, B = w.A.copy(), w.B.copy()
+    pad = w.S == 0
+    A[pad] = rng.uniform(-1e3, 1e3, (pad.sum(), 2)).astype(np.float32)
+    B[pad] = rng.uniform(-1e3, 1e3, (pad.sum(), 2)).astype(np.float32)
+    scene.update(A, B, w.S)
+    again = _run(torch, scene, w.poses, grad=True, per_obstacle=True)
+    for a, b in zip(base, again):
+        assert np.array_equal(a, b)
+    A2 = np.concatenate([np.concatenate([w.A, rng.uniform(0, 20, (w.M, 3, 2)).astype(np.float32)], 1),
+                         rng.uniform(0, 20, (5, w.E + 3, 2)).astype(np.float32)])
+    B2 = np.concatenate([np.concatenate([w.B, rng.uniform(0, 20, (w.M, 3, 2)).astype(np.float32)], 1),
+                         rng.uniform(0, 20, (5, w.E + 3, 2)).astype(np.float32)])
+    S2 = np.concatenate([np.concatenate([w.S, np.zeros((w.M, 3), np.uint8)], 1),
+                         np.zeros((5, w.E + 3), np.uint8)])
+    s2 = psdf.Scene(w.footprint, A2, B2, S2, max_poses=w.N)
+    v, g, po = _run(torch, s2, w.poses, grad=True, per_obstacle=True)
+    assert np.array_equal(v, base[0]) and np.array_equal(g, base[1])
+    assert np.array_equal(po[:, :w.M], base[2]) and np.isposinf(po[:, w.M:]).all()
+    s2.close()
+    # clockwise obstacle rows give the same values (reading G8)
+    A3, B3 = w.A.copy(), w.B.copy()
+    for i in range(0, w.M, 2):
+        sl = np.nonzero(w.S[i])[0]
+        A3[i, sl], B3[i, sl] = w.B[i, sl][::-1].copy(), w.A[i, sl][::-1].copy()
+    s3 = psdf.Scene(w.footprint, A3, B3, w.S, max_poses=w.N)
+    v, g, po = _run(torch, s3, w.poses, grad=True, per_obstacle=True)
+    compare(ref, v, g, po, what="clockwise rows")
+    s3.close()
+    # device-resident scene tensors
+    s4 = psdf.Scene(w.footprint, torch.from_numpy(w.A).cuda(), torch.from_numpy(w.B).cuda(),
+                    torch.from_numpy(w.S).cuda(), max_poses=w.N)
+    v, g, po = _run(torch, s4, w.poses, grad=True, per_obstacle=True)
+    for a, b in zip(base, (v, g, po)):
+        assert np.array_equal(a, b)
+    s4.close()
+    scene.close()
+
+
+def test_mpc_coefficients(env):
+    """[h_s - gamma_s ; J_g,s] of eqs.(26)-(28), N=15 stages, d_min=0.01
+    (PAPER.md:301)."""
+    torch, O, psdf, W = env
+    w = W.table1_case(100, 15)
+    ref = O.evaluate(w.footprint, w.A, w.B, w.S, w.poses)
+    scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=64)
+    d_min, v_max, w_max, dt = 0.01, 1.0, 1.0, 0.1
+    rho_p, rho_t = v_max * dt, w_max * dt
+    c = scene.mpc_coeffs_host(w.poses, d_min, rho_p, rho_t)
+    rmax = np.hypot(w.footprint[:, 0].astype(np.float64), w.footprint[:, 1]).max()
+    gamma = 0.5 * (rmax + ref.value) * rho_t ** 2 + rho_p * rho_t
+    assert np.abs(c[:, 0] - (ref.value - d_min - gamma)).max() < 2e-5
+    ok = (ref.margin > 1e-4) & (np.abs(ref.value) > 1e-3)
+    assert np.abs(c[ok, 1:] + ref.grad[ok]).max() < 1e-3
+    v, g, _ = scene.eval_host(w.poses)
+    assert np.array_equal(c[:, 1:], -g)
+    scene.close()
+
+
+def test_table1_shapes(env):
+    """Paper Table I grid M in {1,10,100} x B in {1,15,100}."""
+    torch, O, psdf, W = env
+    for M in (1, 10, 100):
+        for Bsz in (1, 15, 100):
+            w = W.table1_case(M, Bsz)
+            ref = O.evaluate(w.footprint, w.A, w.B, w.S, w.poses)
+            scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=Bsz)
+            v, g, _ = scene.eval_host(w.poses)
+            compare(ref, v, g, what=w.name)
+            scene.close()

@@ -1,0 +1,104 @@
+"""Parity tests proper: CUDA path (through the C ABI) vs the oracle, element by element,
+on the five BASELINE configs.  Need a B200: `pytest -m gpu`."""
+import numpy as np
+import pytest
+
+from tests.parity import compare
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    from oracle import psdf_oracle as O
+    from paper_2607_04310_b200 import psdf
+    assert torch.cuda.is_available()
+    return torch, O, psdf
+
+
+def _gpu_eval(torch, psdf, w, grad=True, per_obstacle=False, poses=None):
+    poses = w.poses if poses is None else poses
+    scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=max(len(poses), 1))
+    p = torch.from_numpy(np.ascontiguousarray(poses)).cuda()
+    v, g, po = scene.eval(p, grad=grad, per_obstacle=per_obstacle)
+    torch.cuda.synchronize()
+    out = (v.cpu().numpy(), None if g is None else g.cpu().numpy(), None if po is None else po.cpu().numpy())
+    return scene, out
+
+
+def _oracle(O, w, poses=None, per_obstacle=False):
+    return O.evaluate(w.footprint, w.A, w.B, w.S, w.poses if poses is None else poses,
+                      per_obstacle=per_obstacle)
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_small_configs_device_and_host_paths(env, workloads_cache, cfg):
+    torch, O, psdf = env
+    w = workloads_cache(cfg)
+    ref = _oracle(O, w, per_obstacle=True)
+    scene, (v, g, po) = _gpu_eval(torch, psdf, w, grad=True, per_obstacle=True)
+    st = compare(ref, v, g, po, what=w.name)
+    print(w.name, st)
+    assert st["grad_compared"] > 0.5
+    # host (CUDA graph) path, twice (capture, then replay), all output combinations
+    for _ in range(2):
+        v2, g2, po2 = scene.eval_host(w.poses, grad=True, per_obstacle=True)
+        assert np.array_equal(v2, v) and np.array_equal(g2, g) and np.array_equal(po2, po)
+    v3, g3, po3 = scene.eval_host(w.poses, grad=False)
+    assert g3 is None and po3 is None
+    compare(ref, v3, what=w.name + " value-only host")
+    # value-only device path gives the same value
+    v4, _, _ = scene.eval(torch.from_numpy(w.poses).cuda(), grad=False)
+    compare(ref, v4.cpu().numpy(), what=w.name + " value-only")
+    scene.close()
+
+
+@pytest.mark.parametrize("cfg,n", [(3, 5003), (4, 3001), (5, 2501)])
+def test_scan_kernel_subsampled(env, workloads_cache, cfg, n):
+    """Sizes the oracle finishes in seconds, several pose tiles, ragged tail, chunked
+    obstacle ranges with the cross-chunk arg-min."""
+    torch, O, psdf = env
+    w = workloads_cache(cfg).subsample(n)
+    ref = _oracle(O, w)
+    scene, (v, g, _) = _gpu_eval(torch, psdf, w, grad=True)
+    st = compare(ref, v, g, what=w.name)
+    print(w.name, st, "penetrating frac", float((ref.value < 0).mean()))
+    assert st["grad_compared"] > 0.5
+    p = torch.from_numpy(w.poses).cuda()
+    v0, _, _ = scene.eval(p, grad=False)                 # value-only variant
+    compare(ref, v0.cpu().numpy(), what=w.name + " value-only")
+    v1, g1, _ = scene.eval(p, grad=True)                 # workspace left clean: same answer again
+    assert np.array_equal(v1.cpu().numpy(), v) and np.array_equal(g1.cpu().numpy(), g)
+    scene.close()
+
+
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_size_sampled(env, workloads_cache, cfg):
+    """BASELINE full sizes in the launch configuration bench.py times; the oracle checks
+    a random sample of the outputs one by one."""
+    torch, O, psdf = env
+    w = workloads_cache(cfg)
+    scene, (v, g, _) = _gpu_eval(torch, psdf, w, grad=True)
+    rng = np.random.default_rng(99 + cfg)
+    idx = np.sort(rng.choice(w.N, size={3: 4000, 4: 1500, 5: 1200}[cfg], replace=False))
+    ref = _oracle(O, w, poses=w.poses[idx])
+    st = compare(ref, v[idx], g[idx], what=w.name + " full")
+    print(w.name, "full", st)
+    # property that holds at any size: |grad_p| = 1 wherever finite and away from contact
+    gn = np.hypot(g[:, 0], g[:, 1])
+    far = np.abs(v) > 1e-3
+    assert np.abs(gn[far] - 1.0).max() < 1e-4
+    v0, _, _ = scene.eval(torch.from_numpy(w.poses).cuda(), grad=False)
+    assert np.array_equal(v0.cpu().numpy(), v)
+    scene.close()
+
+
+def test_per_obstacle_large_batch(env, workloads_cache):
+    torch, O, psdf = env
+    w = workloads_cache(3).subsample(3000)
+    ref = _oracle(O, w, per_obstacle=True)
+    scene, (v, g, po) = _gpu_eval(torch, psdf, w, grad=True, per_obstacle=True)
+    print(compare(ref, v, g, po, what="per-obstacle scan path"))
+    assert np.array_equal(po.min(axis=1), v)
+    scene.close()
