@@ -1,0 +1,280 @@
+#!/usr/bin/env python
+"""bench.py — PSDF value+grad throughput on the BASELINE workload (contract in the task brief).
+
+A "step" is one pass of the whole hot path (H1-H8: pose setup, both pools, SAT, min over
+obstacles, witness gradient) over one batch of synthetic poses, i.e. ONE psdf_eval call.
+Default workload: config 5 (throughput stress, the largest single-GPU config, the one
+BASELINE.json's ">= 60 % of the FP32 roofline" is quoted on).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 3|4|5] [--impl reference]
+
+Prints ONE JSON line on rank 0.  `--impl reference` times the CPU oracle as it stands on
+the host cores on a bounded sample of the same workload (no GPU work).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "psdf_value_grad_pose_obstacle_pairs_per_s"
+UNIT = "pairs/s"
+FP32_LANES_PER_SM = 128            # B200 SM: 4 SMSPs x 32 FP32 lanes (guide: blackwell_cuda_programming.md)
+
+
+def flops_per_launch(w) -> float:
+    """Algorithmic FLOPs, fixed before tuning:
+    F(V,e) = 32 V e + 6 e + 4 V + 6 per (pose, obstacle with e valid edges)."""
+    e = w.valid_edges().astype(np.float64)
+    e = e[e > 0]
+    V = w.V
+    return float(w.N) * float((32.0 * V * e + 6.0 * e + 4.0 * V + 6.0).sum())
+
+
+def algorithmic_bytes(w) -> float:
+    return w.N * (12 + 16) + int(w.valid_edges().sum()) * 32.0
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.t.join(timeout=2)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if f[3 + k].lower() == "active":
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def load_workload(idx: int, rank: int):
+    from paper_2607_04310_b200 import workloads as W
+    w = W.make_config(idx)
+    if rank > 0:                       # weak scaling: same scene, a different pose batch per rank
+        w.poses = w.poses.copy()
+        w.poses[:, 2] += np.float32(0.37 * rank)
+    return w
+
+
+def measured_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except (OSError, ValueError):
+        return {}
+
+
+def ncu_traffic(workload_name: str):
+    """Per-launch DRAM bytes of the dominant kernel from the committed ncu --set full
+    capture (profiles/traffic.json), or None."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(workload_name)
+    except (OSError, ValueError):
+        return None
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle, as it stands, on the host cores; each step is a bounded
+    sample (`--ref-poses` poses of the workload, value+grad)."""
+    from oracle import psdf_oracle as O
+    n = min(args.ref_poses, w.N)
+    sub = w.subsample(n)
+    for _ in range(min(args.warmup, 1)):
+        O.evaluate(sub.footprint, sub.A, sub.B, sub.S, sub.poses[: max(n // 8, 1)])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        O.evaluate(sub.footprint, sub.A, sub.B, sub.S, sub.poses)
+    dt = (time.perf_counter() - t0) / args.steps
+    val = sub.n_pairs() / dt
+    cores = O.max_threads()
+    sample = f"{n} of {w.N} poses (stride subsample) x {w.M} obstacles per step, value+grad, float64"
+    return {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "N": n, "M": w.M, "E": w.E, "V": w.V, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--workload", type=int, default=5, choices=[3, 4, 5])
+    ap.add_argument("--impl", default="psdf", choices=["psdf", "reference"])
+    ap.add_argument("--ref-poses", type=int, default=1024)
+    ap.add_argument("--cpu-poses", type=int, default=2048)
+    ap.add_argument("--value-only", action="store_true", help="extra run without gradients is always reported; "
+                    "this flag makes it the headline")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        if rank == 0:
+            print(json.dumps(run_reference(args, load_workload(args.workload, 0))), flush=True)
+        return 0
+
+    import torch
+    import torch.distributed as dist
+    from paper_2607_04310_b200 import psdf
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = load_workload(args.workload, rank)
+    scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=w.N)
+    poses = torch.from_numpy(w.poses).cuda()
+    value = torch.empty(w.N, dtype=torch.float32, device="cuda")
+    grad = torch.empty((w.N, 3), dtype=torch.float32, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def timed(n_steps, with_grad):
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_steps)]
+        for a, b in evs:
+            flush.zero_()                                    # L2 flush between timed iterations
+            a.record(stream)
+            scene.eval(poses, value=value, grad=grad if with_grad else False, stream=stream)
+            b.record(stream)
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in evs]
+
+    timed(max(args.warmup, 3), True)
+    fp32_meas = psdf.psdf_measure_fp32_peak(8192) if rank == 0 else None
+    timed(3, True)
+    sampler = ClockSampler(local_rank)
+    n_launch0 = psdf.psdf_kernel_launches()
+    barrier()
+    sampler.start()
+    t_wall0 = time.perf_counter()
+    times = timed(args.steps, not args.value_only)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop()
+    launches = psdf.psdf_kernel_launches() - n_launch0
+    t_dev = float(np.sum(times)) * 1e-3
+    other = timed(max(args.steps // 4, 5), args.value_only)     # the other variant, for the record
+
+    # end to end through the public host API: pinned staging + H2D + kernel + D2H inside
+    for _ in range(3):
+        scene.eval_host(w.poses, grad=True)
+    barrier()
+    k_e2e = max(args.steps // 4, 5)
+    t0 = time.perf_counter()
+    for _ in range(k_e2e):
+        scene.eval_host(w.poses, grad=True)
+    t_e2e = (time.perf_counter() - t0) / k_e2e
+
+    tt = torch.tensor([t_dev, t_e2e, t_wall], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_dev, t_e2e, t_wall = [float(x) for x in tt.cpu()]
+
+    if rank == 0:
+        pairs = w.n_pairs()
+        F = flops_per_launch(w)
+        t_kernel = float(np.mean(times)) * 1e-3              # average launch duration, CUDA events
+        peaks = measured_peaks()
+        sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+        sms = torch.cuda.get_device_properties(0).multi_processor_count
+        peak_nominal = sms * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+        achieved = F / t_kernel / 1e12
+        hbm = float(peaks.get("hbm_gbs", 6650.0))
+        out = {
+            "metric": METRIC, "value": pairs * world * args.steps / t_dev, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_dev / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{w.name} (BASELINE.json configs[4]), "
+                                   f"{'value-only' if args.value_only else 'value+grad'}",
+                       "N_per_gpu": w.N, "M": w.M, "E": w.E, "V": w.V, "pairs_per_gpu": pairs,
+                       "valid_edges": int(w.valid_edges().sum()), "l2_flush": "256 MiB memset between timed launches",
+                       "parallelism": f"replicated scene, pose-sharded x{world}", "seed": 43100 + args.workload},
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
+                         "frac": achieved / peak_nominal, "traffic": ncu_traffic(w.name),
+                         "peak_source": f"derived: {sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x {sm_max:.0f} MHz "
+                                        "(clocks.max.sm, MEASURED_PEAKS.json); no FP32 figure in MEASURED_PEAKS.json",
+                         "flops_per_launch": F, "flop_formula": "32*V*e+6*e+4*V+6 per (pose, obstacle), valid edges only",
+                         "kernel_ms": t_kernel * 1e3, "kernel_ms_min": float(np.min(times)),
+                         "peak_measured_ffma": fp32_meas, "frac_of_measured_ffma": achieved / fp32_meas if fp32_meas else None,
+                         "hbm_bytes_algorithmic": algorithmic_bytes(w),
+                         "hbm_gbs_achieved": algorithmic_bytes(w) / t_kernel / 1e9, "hbm_gbs_peak_measured": hbm},
+            "other_variant": {"what": "value+grad" if args.value_only else "value-only",
+                              "ms_per_step": float(np.mean(other)), "value": pairs / (float(np.mean(other)) * 1e-3)},
+            "e2e": {"value": pairs * world / t_e2e, "unit": UNIT, "ms_per_step": t_e2e * 1e3,
+                    "h2d_bytes_per_step": w.N * 12, "d2h_bytes_per_step": w.N * 16,
+                    "api": "psdf_eval_host (host buffers -> pinned staging -> CUDA graph {H2D, kernel, D2H} -> host)"},
+            "gpu_launches": int(launches), "wall_s_timed_region": t_wall, "clocks": clocks,
+            "paper_context": {"psdf_rtx4090_M100_B100_ms": 2.207, "implied_pairs_per_s": 4.5e6,
+                              "source": "PAPER.md:419 Table I (other hardware, context only)"},
+        }
+        if world == 1:
+            from oracle import psdf_oracle as O          # cpu_baseline leg: the oracle as it stands
+            sub = w.subsample(min(args.cpu_poses, w.N))
+            t0 = time.perf_counter()
+            O.evaluate(sub.footprint, sub.A, sub.B, sub.S, sub.poses)
+            dt = time.perf_counter() - t0
+            out["cpu_baseline"] = {"value": sub.n_pairs() / dt, "unit": UNIT, "cores": O.max_threads(),
+                                   "kind": "oracle", "seconds": dt,
+                                   "sample": f"{sub.N} of {w.N} poses (stride subsample) x {w.M} obstacles, "
+                                             "value+grad, float64, OpenMP"}
+        print(json.dumps(out), flush=True)
+    scene.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -193,11 +193,13 @@ class Scene:
             grad = torch.empty((N, 3), dtype=torch.float32, device=poses.device)
         if per_obstacle is True:
             per_obstacle = torch.empty((N, self.M), dtype=torch.float32, device=poses.device)
-        pg = _dev_ptr(grad, "float32") if grad is not False and grad is not None else None
-        po = _dev_ptr(per_obstacle, "float32") if per_obstacle is not False and per_obstacle is not None else None
+        want_g = grad is not False and grad is not None
+        want_po = per_obstacle is not False and per_obstacle is not None
+        pg = _dev_ptr(grad, "float32") if want_g else None
+        po = _dev_ptr(per_obstacle, "float32") if want_po else None
         _check(lib().psdf_eval(self._h, pp, N, _dev_ptr(value, "float32"), pg, po, _stream_ptr(stream)),
                "psdf_eval")
-        return value, (grad if pg else None), (per_obstacle if po else None)
+        return value, (grad if want_g else None), (per_obstacle if want_po else None)
 
     def eval_host(self, poses, grad=True, per_obstacle=False):
         """psdf_eval_host on numpy arrays (CUDA-graph replay, returns after sync)."""
