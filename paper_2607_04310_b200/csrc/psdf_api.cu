@@ -41,8 +41,10 @@ struct psdf_scene {
   int n_edges = 0, Mv = 0, n_empty = 0;
   int edge_cap = 0;
   int sm_count = 148;
-  std::vector<int> h_row_begin;       // host copy for chunk planning
+  std::vector<int> h_pair_begin;      // host copy for chunk planning
+  int n_pairs = 0;
   EdgeRec* d_edges = nullptr;
+  PairRec* d_pairs = nullptr;
   int* d_row_begin = nullptr;
   int* d_empty = nullptr;
   unsigned long long* d_ws_depth = nullptr;
@@ -110,6 +112,7 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
   if (N == 0) return PSDF_OK;
   EvalParams p{};
   p.edges = sc->d_edges;
+  p.pairs = sc->d_pairs;
   p.row_begin = sc->d_row_begin;
   p.empty_rows = sc->d_empty;
   p.poses = poses;
@@ -142,23 +145,30 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
     bd = 64;
     grid = dim3((unsigned)(((long long)N * K + bd - 1) / bd));
   } else {
-    bd = (N >= sc->sm_count * 128 * 6) ? 128 : 64;
-    const int tiles = (N + bd - 1) / bd;
+    // One thread per pose leaves only N/32 warps; the loop is issue/operand-bound and wants
+    // >= ~64 resident warps per SM to hide FMA/ALU latency (measured, profiles/r01_sweep.md),
+    // so the obstacle range is cut into C chunks (C CTAs per pose tile, combined by atomics).
+    bd = N >= 32768 ? 128 : 64;
     int C = 1;
-    const int want = sc->sm_count * 6;               // CTAs we would like in flight
-    if (tiles < want) C = (want + tiles - 1) / tiles;
-    const int maxC = sc->Mv / 8 > 0 ? sc->Mv / 8 : 1;
+    const double warps_per_sm = (double)N / 32.0 / sc->sm_count;
+    if (warps_per_sm < 80.0) C = (int)std::ceil(80.0 / warps_per_sm);
+    const int maxC = sc->Mv / 16 > 0 ? sc->Mv / 16 : 1;
+    if (const char* e = std::getenv("PSDF_BD")) bd = std::atoi(e);           // tuning overrides
+    if (const char* e = std::getenv("PSDF_CHUNKS")) C = std::atoi(e);
+    if (bd != 32 && bd != 64 && bd != 128 && bd != 256) bd = 64;
+    if (C < 1) C = 1;
     if (C > maxC) C = maxC;
     if (C > kMaxChunks) C = kMaxChunks;
+    const int tiles = (N + bd - 1) / bd;
     // chunk boundaries on obstacle boundaries, balanced by edge count
     p.chunk_begin[0] = 0;
     int o = 0;
     for (int c = 1; c < C; ++c) {
-      const long long target = (long long)sc->n_edges * c / C;
-      while (o < sc->Mv && sc->h_row_begin[o] < target) ++o;
-      p.chunk_begin[c] = sc->h_row_begin[o];
+      const long long target = (long long)sc->n_pairs * c / C;
+      while (o < sc->Mv && sc->h_pair_begin[o] < target) ++o;
+      p.chunk_begin[c] = sc->h_pair_begin[o];
     }
-    p.chunk_begin[C] = sc->n_edges;
+    p.chunk_begin[C] = sc->n_pairs;
     p.n_chunks = C;
     grid = dim3((unsigned)tiles, (unsigned)C);
   }
@@ -188,9 +198,12 @@ psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const u
   sc->n_edges = (int)ps.edges.size();
   sc->Mv = (int)ps.row_begin.size() - 1;
   sc->n_empty = (int)ps.empty_rows.size();
-  sc->h_row_begin = ps.row_begin;
-  if (sc->n_edges)
+  sc->h_pair_begin = ps.pair_begin;
+  sc->n_pairs = (int)ps.pairs.size();
+  if (sc->n_edges) {
     CU_TRY(cudaMemcpyAsync(sc->d_edges, ps.edges.data(), sizeof(EdgeRec) * sc->n_edges, cudaMemcpyHostToDevice, st));
+    CU_TRY(cudaMemcpyAsync(sc->d_pairs, ps.pairs.data(), sizeof(PairRec) * sc->n_pairs, cudaMemcpyHostToDevice, st));
+  }
   CU_TRY(cudaMemcpyAsync(sc->d_row_begin, ps.row_begin.data(), sizeof(int) * (sc->Mv + 1), cudaMemcpyHostToDevice, st));
   if (sc->n_empty)
     CU_TRY(cudaMemcpyAsync(sc->d_empty, ps.empty_rows.data(), sizeof(int) * sc->n_empty, cudaMemcpyHostToDevice, st));
@@ -208,7 +221,7 @@ void psdf_destroy_scene(psdf_scene* sc) {
   for (auto& g : sc->graphs)
     if (g.exec) cudaGraphExecDestroy(g.exec);
   if (sc->gstream) cudaStreamDestroy(sc->gstream);
-  cudaFree(sc->d_edges); cudaFree(sc->d_row_begin); cudaFree(sc->d_empty);
+  cudaFree(sc->d_edges); cudaFree(sc->d_pairs); cudaFree(sc->d_row_begin); cudaFree(sc->d_empty);
   cudaFree(sc->d_ws_depth); cudaFree(sc->d_ws_d2); cudaFree(sc->d_ws_count);
   cudaFree(sc->d_in); cudaFree(sc->d_out); cudaFree(sc->d_per);
   if (sc->h_in) cudaFreeHost(sc->h_in);
@@ -240,6 +253,7 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
     CU_TRY(cudaGetDevice(&dev));
     CU_TRY(cudaDeviceGetAttribute(&sc->sm_count, cudaDevAttrMultiProcessorCount, dev));
     CU_TRY(cudaMalloc(&sc->d_edges, sizeof(EdgeRec) * (size_t)sc->edge_cap));
+    CU_TRY(cudaMalloc(&sc->d_pairs, sizeof(PairRec) * (size_t)(sc->edge_cap / 2 + M)));
     CU_TRY(cudaMalloc(&sc->d_row_begin, sizeof(int) * (size_t)(M + 1)));
     CU_TRY(cudaMalloc(&sc->d_empty, sizeof(int) * (size_t)M));
     CU_TRY(cudaMalloc(&sc->d_ws_depth, sizeof(unsigned long long) * (size_t)max_poses));

@@ -71,6 +71,9 @@ __device__ __forceinline__ void pose_setup(const Footprint& fp, float x, float y
   }
 }
 
+__device__ __forceinline__ float fmax3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }
+__device__ __forceinline__ float fmin3(float a, float b, float c) { return fminf(fminf(a, b), c); }
+
 // Scan accumulators for the obstacle currently being traversed.
 template <int V>
 struct ObstacleAcc {
@@ -84,7 +87,8 @@ struct ObstacleAcc {
   __device__ __forceinline__ float depth() const {
     float d = gO;
 #pragma unroll
-    for (int l = 0; l < V; ++l) d = fminf(d, gR[l]);
+    for (int l = 0; l + 1 < V; l += 2) d = fmin3(d, gR[l], gR[l + 1]);
+    if (V & 1) d = fminf(d, gR[V - 1]);
     return d;
   }
 };
@@ -117,6 +121,67 @@ __device__ __forceinline__ void edge_step(const Footprint& fp, const Posed<V>& P
     m = fminf(fminf(m, d1), d2);
   }
   acc.gO = fminf(acc.gO, gj);
+  minD2 = m;
+}
+
+// Two packed edges of the same obstacle, 48 bytes (three float4): the tile-scan kernel's
+// record.  Obstacles with an odd edge count repeat their last edge (a duplicate changes no
+// min/max).  q2 = (h0, h1, last, slot): `last` = obstacle row if this pair ends the
+// obstacle, else -1 (int bits); slot = packed obstacle index (int bits).
+struct __align__(16) PairRec {
+  float4 q0, q1, q2;
+};
+
+
+// Hot inner step for a pair of edges (H2-H5): 2 x V x (pool 1 + pool 2 + both SAT axes).
+// Min/max reductions are arranged as 3-input FMNMX3 trees.
+template <int V>
+__device__ __forceinline__ void pair_step(const Footprint& fp, const Posed<V>& P, const float4 q0,
+                                          const float4 q1, const float h0, const float h1,
+                                          ObstacleAcc<V>& acc, float& minD2) {
+  const float ax0 = q0.x - P.px, ay0 = q0.y - P.py, ax1 = q1.x - P.px, ay1 = q1.y - P.py;
+  const float tx0 = q0.z, ty0 = q0.w, tx1 = q1.z, ty1 = q1.w;
+  const float cn0 = fmaf(ay0, tx0, -ax0 * ty0), cn1 = fmaf(ay1, tx1, -ax1 * ty1);
+  const float ct0 = fmaf(ax0, tx0, fmaf(ay0, ty0, h0)), ct1 = fmaf(ax1, tx1, fmaf(ay1, ty1, h1));
+  float s0[V], s1[V];
+  float m = minD2;
+#pragma unroll
+  for (int l = 0; l < V; ++l) {
+    const float rx = P.rx[l], ry = P.ry[l], Tx = P.Tx[l], Ty = P.Ty[l];
+    // pool 1 + obstacle axes
+    s0[l] = fmaf(ry, tx0, fmaf(-rx, ty0, -cn0));
+    s1[l] = fmaf(ry, tx1, fmaf(-rx, ty1, -cn1));
+    const float u0 = fmaf(rx, tx0, fmaf(ry, ty0, -ct0));
+    const float u1 = fmaf(rx, tx1, fmaf(ry, ty1, -ct1));
+    const float e0 = fmaxf(fabsf(u0), h0) - h0;
+    const float e1 = fmaxf(fabsf(u1), h1) - h1;
+    const float d0 = fmaf(e0, e0, s0[l] * s0[l]);
+    const float d1 = fmaf(e1, e1, s1[l] * s1[l]);
+    // pool 2 + robot axis l
+    const float p0 = fmaf(ay0, Tx, fmaf(-ax0, Ty, -fp.cN[l]));
+    const float p1 = fmaf(ay1, Tx, fmaf(-ax1, Ty, -fp.cN[l]));
+    const float w0 = fmaf(ax0, Tx, fmaf(ay0, Ty, -fp.cT[l]));
+    const float w1 = fmaf(ax1, Tx, fmaf(ay1, Ty, -fp.cT[l]));
+    const float f0 = fmaxf(fabsf(w0), fp.h[l]) - fp.h[l];
+    const float f1 = fmaxf(fabsf(w1), fp.h[l]) - fp.h[l];
+    const float g0 = fmaf(f0, f0, p0 * p0);
+    const float g1 = fmaf(f1, f1, p1 * p1);
+    acc.gR[l] = fmax3(acc.gR[l], p0, p1);
+    m = fmin3(m, d0, g0);
+    m = fmin3(m, d1, g1);
+  }
+  // G_j = max_l sigma for both edges, then min into gO
+  float gj0 = s0[0], gj1 = s1[0];
+#pragma unroll
+  for (int l = 1; l + 1 < V; l += 2) {
+    gj0 = fmax3(gj0, s0[l], s0[l + 1]);
+    gj1 = fmax3(gj1, s1[l], s1[l + 1]);
+  }
+  if ((V & 1) == 0) {
+    gj0 = fmaxf(gj0, s0[V - 1]);
+    gj1 = fmaxf(gj1, s1[V - 1]);
+  }
+  acc.gO = fmin3(acc.gO, gj0, gj1);
   minD2 = m;
 }
 

@@ -7,13 +7,14 @@
 
 namespace psdf {
 
-constexpr int kTileEdges = 128;    // records per shared-memory tile (4 KB), double buffered
+constexpr int kTilePairs = 96;     // pair records per shared-memory tile (4.5 KB), double buffered
 constexpr int kMaxChunks = 64;
 
 enum Mode : int { kGrad = 1, kPerObs = 2, kCoeff = 4 };
 
 struct EvalParams {
   const EdgeRec* edges;        // [n_edges] packed valid edges, grouped by obstacle
+  const PairRec* pairs;        // [n_pairs] the same edges two per record (tile-scan kernel)
   const int* row_begin;        // [Mv+1] packed obstacle -> first edge
   const int* empty_rows;       // [n_empty] obstacle rows with no valid edge
   const float* poses;          // [N,3]
@@ -28,7 +29,7 @@ struct EvalParams {
   int n_chunks;
   int lanes;                   // lane-split kernel: lanes per pose (power of two <= 32)
   float d_min, rho_p, rho_theta;
-  int chunk_begin[kMaxChunks + 1];   // edge offsets of the obstacle chunks
+  int chunk_begin[kMaxChunks + 1];   // pair-record offsets of the obstacle chunks
 };
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
@@ -72,7 +73,7 @@ __device__ __forceinline__ void finalize_pose(const Footprint& fp, const EvalPar
 template <int V, int MODE>
 __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ Footprint fp,
                                                         const __grid_constant__ EvalParams p) {
-  __shared__ float4 tile[2][kTileEdges * 2];
+  __shared__ float4 tile[2][kTilePairs * 3];
   __shared__ int s_is_last;
   const int tid = threadIdx.x, bd = blockDim.x;
   const int n_raw = blockIdx.x * bd + tid;
@@ -82,13 +83,13 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
   pose_setup<V>(fp, x, y, th, P);
 
   const int cb = p.chunk_begin[blockIdx.y], ce = p.chunk_begin[blockIdx.y + 1];
-  const int n_tiles = (ce - cb + kTileEdges - 1) / kTileEdges;
-  const float4* gsrc = reinterpret_cast<const float4*>(p.edges);
+  const int n_tiles = (ce - cb + kTilePairs - 1) / kTilePairs;
+  const float4* gsrc = reinterpret_cast<const float4*>(p.pairs);
 
   auto issue = [&](int t) {
-    const int e0 = cb + t * kTileEdges;
-    const int cnt = min(kTileEdges, ce - e0) * 2;  // float4 count
-    for (int i = tid; i < cnt; i += bd) cp_async16(&tile[t & 1][i], gsrc + 2 * (size_t)e0 + i);
+    const int e0 = cb + t * kTilePairs;
+    const int cnt = min(kTilePairs, ce - e0) * 3;  // float4 count
+    for (int i = tid; i < cnt; i += bd) cp_async16(&tile[t & 1][i], gsrc + 3 * (size_t)e0 + i);
     cp_async_commit();
   };
 
@@ -107,15 +108,16 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
     }
     __syncthreads();
     const float4* buf = tile[t & 1];
-    const int cnt = min(kTileEdges, ce - (cb + t * kTileEdges));
+    const int cnt = min(kTilePairs, ce - (cb + t * kTilePairs));
 #pragma unroll 1
     for (int k = 0; k < cnt; ++k) {
-      const float4 e0 = buf[2 * k];
-      const float4 e1 = buf[2 * k + 1];
-      edge_step<V>(fp, P, e0, e1.x, acc, minD2);
-      const int last = __float_as_int(e1.y);
+      const float4 q0 = buf[3 * k];
+      const float4 q1 = buf[3 * k + 1];
+      const float4 q2 = buf[3 * k + 2];
+      pair_step<V>(fp, P, q0, q1, q2.x, q2.y, acc, minD2);
+      const int last = __float_as_int(q2.z);
       if (last >= 0) {                             // uniform: end of an obstacle (H6, H7)
-        const int slot = __float_as_int(e1.z);
+        const int slot = __float_as_int(q2.w);
         const float depth = acc.depth();
         if (MODE & kPerObs) {
           if (n_raw < p.N)

@@ -14,6 +14,8 @@ namespace psdf {
 struct PackedScene {
   std::vector<EdgeRec> edges;     // grouped by obstacle
   std::vector<int> row_begin;     // [Mv+1]
+  std::vector<PairRec> pairs;     // tile-scan records: two edges each, grouped by obstacle
+  std::vector<int> pair_begin;    // [Mv+1]
   std::vector<int> empty_rows;
 };
 
@@ -68,6 +70,27 @@ inline int pack_scene(const float* A, const float* B, const uint8_t* S, int M, i
       out.edges.push_back(r);
     }
     out.row_begin.push_back((int)out.edges.size());
+  }
+  // pair records for the tile-scan kernel
+  out.pairs.clear();
+  out.pair_begin.assign(1, 0);
+  const int Mv = (int)out.row_begin.size() - 1;
+  for (int s = 0; s < Mv; ++s) {
+    const int b = out.row_begin[s], e = out.row_begin[s + 1];
+    for (int k = b; k < e; k += 2) {
+      const EdgeRec& r0 = out.edges[k];
+      const EdgeRec& r1 = out.edges[k + 1 < e ? k + 1 : k];      // odd count: repeat the last edge
+      PairRec pr;
+      pr.q0 = make_float4(r0.ax, r0.ay, r0.tx, r0.ty);
+      pr.q1 = make_float4(r1.ax, r1.ay, r1.tx, r1.ty);
+      const int last = (k + 2 >= e) ? out.edges[e - 1].last : -1;
+      float lf, sf;
+      std::memcpy(&lf, &last, 4);
+      std::memcpy(&sf, &s, 4);
+      pr.q2 = make_float4(r0.h, r1.h, lf, sf);
+      out.pairs.push_back(pr);
+    }
+    out.pair_begin.push_back((int)out.pairs.size());
   }
   return 0;
 }

@@ -34,5 +34,8 @@ def compare(ref, value, grad=None, per_obstacle=None, what=""):
         assert np.array_equal(np.isposinf(po), ~pf), what
         dpo = np.abs(po[pf] - ref.per_obstacle[pf])
         stats["max_dper_obstacle"] = float(dpo.max()) if dpo.size else 0.0
-        assert stats["max_dper_obstacle"] <= VALUE_TOL, (what, stats)
+        # far obstacles: fp32 cannot hold 1e-5 m at tens of metres (ulp(32 m) = 3.8e-6), so the
+        # per-obstacle bar is 1e-5 m + 4 ulp_fp32(|sd|); phi itself stays at 1e-5.
+        tol = VALUE_TOL + 4.0 * np.abs(ref.per_obstacle[pf]) * 2.0 ** -23
+        assert (dpo <= tol).all(), (what, stats)
     return stats
