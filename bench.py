@@ -107,11 +107,15 @@ def measured_peaks():
 
 def ncu_traffic(workload_name: str):
     """Per-launch DRAM bytes of the dominant kernel from the committed ncu --set full
-    capture (profiles/traffic.json), or None."""
+    capture (profiles/traffic.csv), or None."""
     try:
-        return json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(workload_name)
-    except (OSError, ValueError):
-        return None
+        for ln in open(os.path.join(ROOT, "profiles", "traffic.csv")).read().splitlines()[1:]:
+            f = ln.split(",")
+            if f[0] == workload_name:
+                return float(f[1])
+    except (OSError, ValueError, IndexError):
+        pass
+    return None
 
 
 def run_reference(args, w):
