@@ -90,11 +90,8 @@ cudaError_t launch_mode(const psdf_scene* sc, const EvalParams& p, int mode, boo
 cudaError_t launch_v(const psdf_scene* sc, const EvalParams& p, int mode, bool lanes, dim3 grid, int bd,
                      cudaStream_t st) {
   switch (sc->Vp) {
-    case 3: return launch_mode<3>(sc, p, mode, lanes, grid, bd, st);
     case 4: return launch_mode<4>(sc, p, mode, lanes, grid, bd, st);
-    case 5: return launch_mode<5>(sc, p, mode, lanes, grid, bd, st);
     case 6: return launch_mode<6>(sc, p, mode, lanes, grid, bd, st);
-    case 7: return launch_mode<7>(sc, p, mode, lanes, grid, bd, st);
     case 8: return launch_mode<8>(sc, p, mode, lanes, grid, bd, st);
     case 10: return launch_mode<10>(sc, p, mode, lanes, grid, bd, st);
     case 12: return launch_mode<12>(sc, p, mode, lanes, grid, bd, st);

@@ -39,12 +39,13 @@ struct __align__(16) EdgeRec {
 
 // Footprint constants (pose independent), passed by value as a kernel parameter so that
 // the unrolled loops read them as constant-bank operands.
-struct Footprint {
+struct __align__(16) Footprint {
   float vx[kMaxV], vy[kMaxV];   // vertices v_l (robot-local)
   float tx[kMaxV], ty[kMaxV];   // unit edge tangents t~_l of E_l = [v_l, v_{l+1}]
   float h[kMaxV];               // half lengths
   float cN[kMaxV];              // v_l . n~_l      (n~_l = rot90(t~_l), inward)
   float cT[kMaxV];              // v_l . t~_l + h_l
+  float ncN[kMaxV], ncT[kMaxV], nh[kMaxV];   // negated copies (f32x2 constant operands)
   float rmax;                   // max_l |v_l|  (Prop.1)
 };
 
@@ -133,55 +134,82 @@ struct __align__(16) PairRec {
 };
 
 
-// Hot inner step for a pair of edges (H2-H5): 2 x V x (pool 1 + pool 2 + both SAT axes).
-// Min/max reductions are arranged as 3-input FMNMX3 trees.
+// ---- packed (FFMA2) formulation used by the tile-scan kernel -------------------------------
+// Robot vertices/edges are held two per 64-bit register pair so that the eight dot products,
+// the squares and the excess subtraction of two (l, l+1) candidates issue as one f32x2
+// instruction each (fma.rn.f32x2 -> FFMA2; the per-edge scalars enter as broadcast operands).
+// V must be even (odd footprints are padded with a collinear midpoint at pack time).
 template <int V>
-__device__ __forceinline__ void pair_step(const Footprint& fp, const Posed<V>& P, const float4 q0,
-                                          const float4 q1, const float h0, const float h1,
-                                          ObstacleAcc<V>& acc, float& minD2) {
-  const float ax0 = q0.x - P.px, ay0 = q0.y - P.py, ax1 = q1.x - P.px, ay1 = q1.y - P.py;
-  const float tx0 = q0.z, ty0 = q0.w, tx1 = q1.z, ty1 = q1.w;
-  const float cn0 = fmaf(ay0, tx0, -ax0 * ty0), cn1 = fmaf(ay1, tx1, -ax1 * ty1);
-  const float ct0 = fmaf(ax0, tx0, fmaf(ay0, ty0, h0)), ct1 = fmaf(ax1, tx1, fmaf(ay1, ty1, h1));
-  float s0[V], s1[V];
+struct Posed2 {
+  float px, py;
+  float2 rx[V / 2], ry[V / 2], Tx[V / 2], Ty[V / 2];
+};
+
+template <int V>
+__device__ __forceinline__ void pose_setup2(const Footprint& fp, float x, float y, float th, Posed2<V>& P) {
+  float s, c;
+  sincosf(th, &s, &c);
+  P.px = x;
+  P.py = y;
+#pragma unroll
+  for (int l = 0; l < V / 2; ++l) {
+    P.rx[l] = make_float2(c * fp.vx[2 * l] - s * fp.vy[2 * l], c * fp.vx[2 * l + 1] - s * fp.vy[2 * l + 1]);
+    P.ry[l] = make_float2(s * fp.vx[2 * l] + c * fp.vy[2 * l], s * fp.vx[2 * l + 1] + c * fp.vy[2 * l + 1]);
+    P.Tx[l] = make_float2(c * fp.tx[2 * l] - s * fp.ty[2 * l], c * fp.tx[2 * l + 1] - s * fp.ty[2 * l + 1]);
+    P.Ty[l] = make_float2(s * fp.tx[2 * l] + c * fp.ty[2 * l], s * fp.tx[2 * l + 1] + c * fp.ty[2 * l + 1]);
+  }
+}
+
+template <int V>
+__device__ __forceinline__ void unpack_pose(const Posed2<V>& P2, Posed<V>& P) {
+  P.px = P2.px;
+  P.py = P2.py;
+#pragma unroll
+  for (int l = 0; l < V / 2; ++l) {
+    P.rx[2 * l] = P2.rx[l].x; P.rx[2 * l + 1] = P2.rx[l].y;
+    P.ry[2 * l] = P2.ry[l].x; P.ry[2 * l + 1] = P2.ry[l].y;
+    P.Tx[2 * l] = P2.Tx[l].x; P.Tx[2 * l + 1] = P2.Tx[l].y;
+    P.Ty[2 * l] = P2.Ty[l].x; P.Ty[2 * l + 1] = P2.Ty[l].y;
+  }
+}
+
+__device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
+
+// Hot inner step (H2-H5) for one edge against all V robot vertices/edges, two at a time.
+template <int V>
+__device__ __forceinline__ void edge_step2(const Footprint& fp, const Posed2<V>& P, const float4 q,
+                                           const float h, ObstacleAcc<V>& acc, float& minD2) {
+  const float sax = q.x - P.px, say = q.y - P.py;                 // H2: a_j = A_j - p
+  const float sncn = fmaf(sax, q.w, -say * q.z);                  // -(a_j . n_j)
+  const float snct = -fmaf(sax, q.z, fmaf(say, q.w, h));          // -(a_j . t_j + h_j)
+  const float2 ax = bc2(sax), ay = bc2(say), nax = bc2(-sax);
+  const float2 tx = bc2(q.z), ty = bc2(q.w), nty = bc2(-q.w);
+  const float2 ncn = bc2(sncn), nct = bc2(snct), nh = bc2(-h);
+  float gj = -kInf;
   float m = minD2;
 #pragma unroll
-  for (int l = 0; l < V; ++l) {
-    const float rx = P.rx[l], ry = P.ry[l], Tx = P.Tx[l], Ty = P.Ty[l];
-    // pool 1 + obstacle axes
-    s0[l] = fmaf(ry, tx0, fmaf(-rx, ty0, -cn0));
-    s1[l] = fmaf(ry, tx1, fmaf(-rx, ty1, -cn1));
-    const float u0 = fmaf(rx, tx0, fmaf(ry, ty0, -ct0));
-    const float u1 = fmaf(rx, tx1, fmaf(ry, ty1, -ct1));
-    const float e0 = fmaxf(fabsf(u0), h0) - h0;
-    const float e1 = fmaxf(fabsf(u1), h1) - h1;
-    const float d0 = fmaf(e0, e0, s0[l] * s0[l]);
-    const float d1 = fmaf(e1, e1, s1[l] * s1[l]);
-    // pool 2 + robot axis l
-    const float p0 = fmaf(ay0, Tx, fmaf(-ax0, Ty, -fp.cN[l]));
-    const float p1 = fmaf(ay1, Tx, fmaf(-ax1, Ty, -fp.cN[l]));
-    const float w0 = fmaf(ax0, Tx, fmaf(ay0, Ty, -fp.cT[l]));
-    const float w1 = fmaf(ax1, Tx, fmaf(ay1, Ty, -fp.cT[l]));
-    const float f0 = fmaxf(fabsf(w0), fp.h[l]) - fp.h[l];
-    const float f1 = fmaxf(fabsf(w1), fp.h[l]) - fp.h[l];
-    const float g0 = fmaf(f0, f0, p0 * p0);
-    const float g1 = fmaf(f1, f1, p1 * p1);
-    acc.gR[l] = fmax3(acc.gR[l], p0, p1);
-    m = fmin3(m, d0, g0);
-    m = fmin3(m, d1, g1);
+  for (int l = 0; l < V / 2; ++l) {
+    // pool 1 + obstacle axis j
+    const float2 s = __ffma2_rn(P.ry[l], tx, __ffma2_rn(P.rx[l], nty, ncn));
+    const float2 u = __ffma2_rn(P.rx[l], tx, __ffma2_rn(P.ry[l], ty, nct));
+    const float2 e = __fadd2_rn(make_float2(fmaxf(fabsf(u.x), h), fmaxf(fabsf(u.y), h)), nh);
+    const float2 d = __ffma2_rn(e, e, __fmul2_rn(s, s));
+    gj = fmax3(gj, s.x, s.y);
+    // pool 2 + robot axes l, l+1
+    const float2 ncN = *reinterpret_cast<const float2*>(&fp.ncN[2 * l]);
+    const float2 ncT = *reinterpret_cast<const float2*>(&fp.ncT[2 * l]);
+    const float2 hR = *reinterpret_cast<const float2*>(&fp.h[2 * l]);
+    const float2 nhR = *reinterpret_cast<const float2*>(&fp.nh[2 * l]);
+    const float2 pp = __ffma2_rn(ay, P.Tx[l], __ffma2_rn(nax, P.Ty[l], ncN));
+    const float2 w = __ffma2_rn(ax, P.Tx[l], __ffma2_rn(ay, P.Ty[l], ncT));
+    const float2 f = __fadd2_rn(make_float2(fmaxf(fabsf(w.x), hR.x), fmaxf(fabsf(w.y), hR.y)), nhR);
+    const float2 g = __ffma2_rn(f, f, __fmul2_rn(pp, pp));
+    acc.gR[2 * l] = fmaxf(acc.gR[2 * l], pp.x);
+    acc.gR[2 * l + 1] = fmaxf(acc.gR[2 * l + 1], pp.y);
+    m = fmin3(m, d.x, d.y);
+    m = fmin3(m, g.x, g.y);
   }
-  // G_j = max_l sigma for both edges, then min into gO
-  float gj0 = s0[0], gj1 = s1[0];
-#pragma unroll
-  for (int l = 1; l + 1 < V; l += 2) {
-    gj0 = fmax3(gj0, s0[l], s0[l + 1]);
-    gj1 = fmax3(gj1, s1[l], s1[l + 1]);
-  }
-  if ((V & 1) == 0) {
-    gj0 = fmaxf(gj0, s0[V - 1]);
-    gj1 = fmaxf(gj1, s1[V - 1]);
-  }
-  acc.gO = fmin3(acc.gO, gj0, gj1);
+  acc.gO = fminf(acc.gO, gj);
   minD2 = m;
 }
 

@@ -79,8 +79,8 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
   const int n_raw = blockIdx.x * bd + tid;
   const int n = min(n_raw, p.N - 1);               // tail threads recompute the last pose
   const float x = __ldg(p.poses + 3 * n), y = __ldg(p.poses + 3 * n + 1), th = __ldg(p.poses + 3 * n + 2);
-  Posed<V> P;
-  pose_setup<V>(fp, x, y, th, P);
+  Posed2<V> P;
+  pose_setup2<V>(fp, x, y, th, P);
 
   const int cb = p.chunk_begin[blockIdx.y], ce = p.chunk_begin[blockIdx.y + 1];
   const int n_tiles = (ce - cb + kTilePairs - 1) / kTilePairs;
@@ -114,7 +114,8 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
       const float4 q0 = buf[3 * k];
       const float4 q1 = buf[3 * k + 1];
       const float4 q2 = buf[3 * k + 2];
-      pair_step<V>(fp, P, q0, q1, q2.x, q2.y, acc, minD2);
+      edge_step2<V>(fp, P, q0, q2.x, acc, minD2);
+      edge_step2<V>(fp, P, q1, q2.y, acc, minD2);
       const int last = __float_as_int(q2.z);
       if (last >= 0) {                             // uniform: end of an obstacle (H6, H7)
         const int slot = __float_as_int(q2.w);
@@ -168,7 +169,9 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
   if (n_raw >= p.N) return;
   const bool separated = !(maxDepth >= 0.f);
   const float value = separated ? sqrtf(minD2) : -maxDepth;
-  finalize_pose<V, MODE>(fp, p, P, n, th, value, separated ? idD2 : idDepth, separated);
+  Posed<V> Ps;
+  unpack_pose<V>(P, Ps);
+  finalize_pose<V, MODE>(fp, p, Ps, n, th, value, separated ? idD2 : idDepth, separated);
 }
 
 // ------------------------------------------------------------------------------------------

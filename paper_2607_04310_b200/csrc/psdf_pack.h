@@ -95,10 +95,10 @@ inline int pack_scene(const float* A, const float* B, const uint8_t* S, int M, i
   return 0;
 }
 
-// Supported compile-time vertex counts; other V are padded with collinear midpoints
+// Supported compile-time vertex counts (even: the scan kernel packs vertices in pairs); other V are padded with collinear midpoints
 // (splitting an edge changes neither the polygon nor any min/max of eqs.(14)-(22)).
 inline int padded_vertex_count(int V) {
-  static const int sizes[] = {3, 4, 5, 6, 7, 8, 10, 12, 16};
+  static const int sizes[] = {4, 6, 8, 10, 12, 16};
   for (int s : sizes)
     if (V <= s) return s;
   return -1;
@@ -142,6 +142,7 @@ inline int pack_footprint(const float* fpv, int V, Footprint& fp, int& Vp) {
     fp.h[l] = (float)(0.5 * L);
     fp.cN[l] = (float)(x[l] * (-ty) + y[l] * tx);
     fp.cT[l] = (float)(x[l] * tx + y[l] * ty + 0.5 * L);
+    fp.ncN[l] = -fp.cN[l]; fp.ncT[l] = -fp.cT[l]; fp.nh[l] = -fp.h[l];
   }
   for (int l = 0; l < V; ++l) rmax = std::fmax(rmax, std::hypot((double)fpv[2 * l], (double)fpv[2 * l + 1]));
   fp.rmax = (float)rmax;
