@@ -118,14 +118,94 @@ def ncu_traffic(workload_name: str):
     return None
 
 
+def _pct(xs_us):
+    a = np.sort(np.asarray(xs_us))
+    return {"p50_us": float(a[len(a) // 2]), "p95_us": float(a[int(len(a) * 0.95)]),
+            "p99_us": float(a[int(len(a) * 0.99)]), "min_us": float(a[0]), "n": int(len(a))}
+
+
+def mpc_latency(torch, psdf, replays=2000):
+    """p50/p95/p99 end-to-end latency of the MPC-sized configs (BASELINE.json configs[0], [1]):
+    psdf_eval_host = host poses -> pinned staging -> CUDA-graph {H2D, kernel, D2H} -> host results,
+    timed on the host clock around the C-ABI call; kernel-only by CUDA events around psdf_eval.
+    Also the paper's Table-I shape sweep (context, other hardware)."""
+    from paper_2607_04310_b200 import workloads as W
+    out = {}
+
+    def host_lat(scene, w, n_rep, grad=True, per_obs=False, coeffs=False):
+        value = np.empty(w.N, np.float32)
+        g = np.empty((w.N, 3), np.float32) if grad else None
+        po = np.empty((w.N, w.M), np.float32) if per_obs else None
+        call = (lambda: scene.mpc_coeffs_host(w.poses, 0.3, 0.05, 0.05)) if coeffs else \
+               (lambda: scene.eval_host_into(w.poses, value, g, po))
+        for _ in range(50):
+            call()
+        ts = []
+        for _ in range(n_rep):
+            t0 = time.perf_counter_ns()
+            call()
+            ts.append((time.perf_counter_ns() - t0) * 1e-3)
+        return _pct(ts)
+
+    def kernel_lat(scene, w, n_rep=300, per_obs=False):
+        poses = torch.from_numpy(w.poses).cuda()
+        value = torch.empty(w.N, dtype=torch.float32, device="cuda")
+        grad = torch.empty((w.N, 3), dtype=torch.float32, device="cuda")
+        po = torch.empty((w.N, w.M), dtype=torch.float32, device="cuda") if per_obs else False
+        st = torch.cuda.current_stream()
+        for _ in range(20):
+            scene.eval(poses, value=value, grad=grad, per_obstacle=po, stream=st)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_rep)]
+        for a, b in evs:
+            a.record(st)
+            scene.eval(poses, value=value, grad=grad, per_obstacle=po, stream=st)
+            b.record(st)
+        torch.cuda.synchronize()
+        return _pct([a.elapsed_time(b) * 1e3 for a, b in evs])
+
+    for idx in (1, 2):
+        w = W.make_config(idx)
+        scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=w.N)
+        e = {"N": w.N, "M": w.M, "pairs": w.n_pairs(),
+             "eval_host_value_grad": host_lat(scene, w, replays),
+             "kernel_only_value_grad": kernel_lat(scene, w)}
+        if idx == 1:
+            e["mpc_coeffs_host"] = host_lat(scene, w, replays, coeffs=True)
+        else:
+            e["eval_host_value_grad_per_obstacle"] = host_lat(scene, w, replays, per_obs=True)
+        out[w.name] = e
+        scene.close()
+    t1 = {}
+    for M in (1, 10, 100):
+        for B in (1, 15, 100):
+            w = W.table1_case(M, B)
+            scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=w.N)
+            t1[f"M{M}_B{B}"] = host_lat(scene, w, 500)["p50_us"]
+            scene.close()
+    out["table1_shapes_eval_host_p50_us"] = t1
+    out["table1_paper_rtx4090_ms"] = {"M1_B1": 1.981, "M1_B15": 2.154, "M1_B100": 2.212, "M10_B1": 2.152,
+                                      "M10_B15": 2.213, "M10_B100": 2.250, "M100_B1": 2.221, "M100_B15": 2.222,
+                                      "M100_B100": 2.207,
+                                      "note": "PAPER.md:417-419 Table I, PSDF rows (PyTorch graph incl. backward, "
+                                              "RTX 4090): context only, other hardware"}
+    out["clock"] = "host perf_counter_ns around the Python binding's C-ABI call (ctypes overhead included)"
+    return out
+
+
 def run_reference(args, w):
     """--impl reference: the oracle, as it stands, on the host cores; each step is a bounded
     sample (`--ref-poses` poses of the workload, value+grad)."""
     from oracle import psdf_oracle as O
-    n = min(args.ref_poses, w.N)
+    # bounded sample: calibrate on 64 poses, then size the per-step sample so that the whole
+    # --steps/--warmup run takes about --ref-seconds on this box's cores
+    cal = w.subsample(min(64, w.N))
+    t0 = time.perf_counter()
+    O.evaluate(cal.footprint, cal.A, cal.B, cal.S, cal.poses)
+    rate = cal.N / max(time.perf_counter() - t0, 1e-6)                       # poses/s
+    n = int(min(args.ref_poses, w.N, max(32, rate * args.ref_seconds / (args.steps + min(args.warmup, 1)))))
     sub = w.subsample(n)
     for _ in range(min(args.warmup, 1)):
-        O.evaluate(sub.footprint, sub.A, sub.B, sub.S, sub.poses[: max(n // 8, 1)])
+        O.evaluate(sub.footprint, sub.A, sub.B, sub.S, sub.poses)
     t0 = time.perf_counter()
     for _ in range(args.steps):
         O.evaluate(sub.footprint, sub.A, sub.B, sub.S, sub.poses)
@@ -136,7 +216,7 @@ def run_reference(args, w):
     return {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "N": n, "M": w.M, "E": w.E, "V": w.V, "sample": sample},
+            "config": {"workload": f"{w.name} (BASELINE.json configs[{args.workload - 1}]), value+grad", "N": n, "M": w.M, "E": w.E, "V": w.V, "sample": sample},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -149,8 +229,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--workload", type=int, default=5, choices=[3, 4, 5])
     ap.add_argument("--impl", default="psdf", choices=["psdf", "reference"])
-    ap.add_argument("--ref-poses", type=int, default=1024)
+    ap.add_argument("--ref-poses", type=int, default=4096)
+    ap.add_argument("--ref-seconds", type=float, default=90.0, help="--impl reference: target total run time")
     ap.add_argument("--cpu-poses", type=int, default=2048)
+    ap.add_argument("--no-latency", action="store_true", help="skip the MPC-sized latency section")
     ap.add_argument("--value-only", action="store_true", help="extra run without gradients is always reported; "
                     "this flag makes it the headline")
     args = ap.parse_args()
@@ -165,7 +247,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2607_04310_b200 import psdf
+    from paper_2607_04310_b200 import psdf, sharding
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
     torch.cuda.set_device(local_rank)
@@ -221,10 +303,7 @@ def main():
         scene.eval_host(w.poses, grad=True)
     t_e2e = (time.perf_counter() - t0) / k_e2e
 
-    tt = torch.tensor([t_dev, t_e2e, t_wall], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_dev, t_e2e, t_wall = [float(x) for x in tt.cpu()]
+    t_dev, t_e2e, t_wall = sharding.max_over_ranks([t_dev, t_e2e, t_wall])      # max over ranks
 
     if rank == 0:
         pairs = w.n_pairs()
@@ -240,7 +319,7 @@ def main():
             "metric": METRIC, "value": pairs * world * args.steps / t_dev, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_dev / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"{w.name} (BASELINE.json configs[4]), "
+            "config": {"workload": f"{w.name} (BASELINE.json configs[{args.workload - 1}]), "
                                    f"{'value-only' if args.value_only else 'value+grad'}",
                        "N_per_gpu": w.N, "M": w.M, "E": w.E, "V": w.V, "pairs_per_gpu": pairs,
                        "valid_edges": int(w.valid_edges().sum()), "l2_flush": "256 MiB memset between timed launches",
@@ -273,6 +352,8 @@ def main():
                                    "kind": "oracle", "seconds": dt,
                                    "sample": f"{sub.N} of {w.N} poses (stride subsample) x {w.M} obstacles, "
                                              "value+grad, float64, OpenMP"}
+            if not args.no_latency:
+                out["mpc_latency"] = mpc_latency(torch, psdf)
         print(json.dumps(out), flush=True)
     scene.close()
     if world > 1:

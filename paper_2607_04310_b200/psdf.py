@@ -213,6 +213,17 @@ class Scene:
                                     po.ctypes.data if po is not None else None), "psdf_eval_host")
         return value, g, po
 
+    def eval_host_into(self, poses, value, grad=None, per_obstacle=None):
+        """psdf_eval_host into caller-owned contiguous float32 numpy arrays (no allocation in
+        the binding: the call an MPC loop makes every control cycle)."""
+        N = int(poses.shape[0])
+        for a in (poses, value, grad, per_obstacle):
+            assert a is None or (a.dtype == np.float32 and a.flags.c_contiguous)
+        _check(lib().psdf_eval_host(self._h, poses.ctypes.data, N, value.ctypes.data,
+                                    grad.ctypes.data if grad is not None else None,
+                                    per_obstacle.ctypes.data if per_obstacle is not None else None),
+               "psdf_eval_host")
+
     def mpc_coeffs_host(self, poses, d_min, rho_p, rho_theta):
         poses, pp = _host(poses, np.float32)
         N = int(poses.shape[0])
