@@ -126,8 +126,8 @@ __device__ __forceinline__ void edge_step(const Footprint& fp, const Posed<V>& P
 }
 
 // Two packed edges of the same obstacle, 48 bytes (three float4): the tile-scan kernel's
-// record.  Obstacles with an odd edge count repeat their last edge (a duplicate changes no
-// min/max).  q2 = (h0, h1, last, slot): `last` = obstacle row if this pair ends the
+// record.  q2 = (h0, h1, last, slot): h1 < 0 marks a record whose second half is unused
+// (obstacle with an odd edge count; skipped by a uniform branch); `last` = obstacle row if this pair ends the
 // obstacle, else -1 (int bits); slot = packed obstacle index (int bits).
 struct __align__(16) PairRec {
   float4 q0, q1, q2;

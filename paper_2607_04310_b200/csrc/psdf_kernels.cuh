@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
       const float4 q1 = buf[3 * k + 1];
       const float4 q2 = buf[3 * k + 2];
       edge_step2<V>(fp, P, q0, q2.x, acc, minD2);
-      edge_step2<V>(fp, P, q1, q2.y, acc, minD2);
+      if (q2.y >= 0.f) edge_step2<V>(fp, P, q1, q2.y, acc, minD2);   // uniform: odd edge count
       const int last = __float_as_int(q2.z);
       if (last >= 0) {                             // uniform: end of an obstacle (H6, H7)
         const int slot = __float_as_int(q2.w);

@@ -19,77 +19,124 @@ struct PackedScene {
   std::vector<int> empty_rows;
 };
 
-// returns 0 ok, -2 degenerate
-inline int pack_scene(const float* A, const float* B, const uint8_t* S, int M, int E, PackedScene& out) {
-  out.edges.clear();
-  out.row_begin.assign(1, 0);
-  out.empty_rows.clear();
-  std::vector<int> idx;
-  for (int i = 0; i < M; ++i) {
-    idx.clear();
-    for (int j = 0; j < E; ++j)
-      if (S[(size_t)i * E + j]) idx.push_back(j);
-    const int e = (int)idx.size();
-    if (e == 0) { out.empty_rows.push_back(i); continue; }
-    if (e < 3) return -2;
-    const float* Ai = A + (size_t)i * E * 2;
-    const float* Bi = B + (size_t)i * E * 2;
-    double area2 = 0.0;
-    for (int k = 0; k < e; ++k) {
-      const int j = idx[k], jn = idx[(k + 1) % e];
-      if (std::memcmp(Bi + 2 * j, Ai + 2 * jn, 2 * sizeof(float)) != 0) return -2;   // not closed
-      area2 += (double)Ai[2 * j] * Ai[2 * jn + 1] - (double)Ai[2 * jn] * Ai[2 * j + 1];
+// Double-precision helpers that round identically on host and device: nvcc contracts a*b+c
+// into FMA in device code, the host compiler does not, so the device side uses the
+// never-contracted intrinsics.  This makes the device pack kernel (psdf_pack_kernels.cuh)
+// bit-identical to the host packer.
+#ifdef __CUDA_ARCH__
+#define PSDF_HD __host__ __device__ __forceinline__
+__device__ __forceinline__ double pk_mul(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ double pk_add(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ double pk_sub(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ double pk_div(double a, double b) { return __ddiv_rn(a, b); }
+__device__ __forceinline__ double pk_sqrt(double a) { return __dsqrt_rn(a); }
+#else
+#ifdef __CUDACC__
+#define PSDF_HD __host__ __device__ inline
+#else
+#define PSDF_HD inline
+#endif
+inline double pk_mul(double a, double b) { return a * b; }
+inline double pk_add(double a, double b) { return a + b; }
+inline double pk_sub(double a, double b) { return a - b; }
+inline double pk_div(double a, double b) { return a / b; }
+inline double pk_sqrt(double a) { return std::sqrt(a); }
+#endif
+
+PSDF_HD bool pk_same_point(const float* p, const float* q) {      // bitwise, like memcmp
+  const uint32_t* a = reinterpret_cast<const uint32_t*>(p);
+  const uint32_t* b = reinterpret_cast<const uint32_t*>(q);
+  return a[0] == b[0] && a[1] == b[1];
+}
+PSDF_HD bool pk_finite(double x) { return x - x == 0.0; }
+
+// One obstacle row of (A,B,S): validates Assumption 1 (closed, convex, non-degenerate) and,
+// if `out` is non-null, writes its `*e_out` EdgeRec records (CCW-normalised) to out[0..e).
+// returns 0 ok (e may be 0: absent obstacle), -2 degenerate.
+PSDF_HD int pack_row(const float* Ai, const float* Bi, const uint8_t* Si, int E, int row, int slot,
+                     EdgeRec* out, int* e_out) {
+  int e = 0, first = -1;
+  for (int j = 0; j < E; ++j)
+    if (Si[j]) { if (first < 0) first = j; ++e; }
+  *e_out = e;
+  if (e == 0) return 0;
+  if (e < 3) return -2;
+  auto next_valid = [&](int j) {
+    for (int q = j + 1; q < E; ++q) if (Si[q]) return q;
+    return first;
+  };
+  double area2 = 0.0;
+  for (int k = 0, j = first; k < e; ++k) {
+    const int jn = next_valid(j);
+    if (!pk_same_point(Bi + 2 * j, Ai + 2 * jn)) return -2;                              // not closed
+    area2 = pk_add(area2, pk_sub(pk_mul((double)Ai[2 * j], (double)Ai[2 * jn + 1]),
+                                 pk_mul((double)Ai[2 * jn], (double)Ai[2 * j + 1])));
+    j = jn;
+  }
+  if (!(area2 > 0.0 || area2 < 0.0) || !pk_finite(area2)) return -2;
+  const bool ccw = area2 > 0.0;
+  double ptx = 0, pty = 0;
+  for (int k = 0, j = first; k <= e; ++k) {   // one extra turn closes the convexity check
+    // CCW-normalised edge: for a clockwise row the edge is traversed backwards (origin B_j).
+    const double ox = ccw ? Ai[2 * j] : Bi[2 * j], oy = ccw ? Ai[2 * j + 1] : Bi[2 * j + 1];
+    const double qx = ccw ? Bi[2 * j] : Ai[2 * j], qy = ccw ? Bi[2 * j + 1] : Ai[2 * j + 1];
+    const double dx = pk_sub(qx, ox), dy = pk_sub(qy, oy);
+    const double L2 = pk_add(pk_mul(dx, dx), pk_mul(dy, dy));
+    if (!(L2 >= 1e-12) || !pk_finite(L2)) return -2;
+    const double L = pk_sqrt(L2), tx = pk_div(dx, L), ty = pk_div(dy, L);
+    if (k > 0) {
+      // consecutive tangents must turn left (CCW order) or right (CW order, walked backwards)
+      const double cr = ccw ? pk_sub(pk_mul(ptx, ty), pk_mul(pty, tx)) : pk_sub(pk_mul(tx, pty), pk_mul(ty, ptx));
+      if (cr < -1e-6) return -2;                                                         // not convex
     }
-    if (!(std::fabs(area2) > 0.0) || !std::isfinite(area2)) return -2;
-    const bool ccw = area2 > 0.0;
-    const int slot = (int)out.row_begin.size() - 1;
-    double ptx = 0, pty = 0;
-    for (int k = 0; k <= e; ++k) {     // one extra turn closes the convexity check
-      const int j = idx[k % e];
-      // CCW-normalised edge: for a clockwise row the edge is traversed backwards (origin B_j).
-      const double ox = ccw ? Ai[2 * j] : Bi[2 * j], oy = ccw ? Ai[2 * j + 1] : Bi[2 * j + 1];
-      const double qx = ccw ? Bi[2 * j] : Ai[2 * j], qy = ccw ? Bi[2 * j + 1] : Ai[2 * j + 1];
-      const double dx = qx - ox, dy = qy - oy;
-      const double L2 = dx * dx + dy * dy;
-      if (!(L2 >= 1e-12) || !std::isfinite(L2)) return -2;
-      const double L = std::sqrt(L2), tx = dx / L, ty = dy / L;
-      if (k > 0) {
-        // consecutive tangents must turn left (CCW order) or right (CW order, walked backwards)
-        const double cr = ccw ? (ptx * ty - pty * tx) : (tx * pty - ty * ptx);
-        if (cr < -1e-6) return -2;                                                    // not convex
-      }
-      ptx = tx; pty = ty;
-      if (k == e) break;
+    ptx = tx; pty = ty;
+    if (k == e) break;
+    if (out) {
       EdgeRec r;
       r.ax = (float)ox; r.ay = (float)oy;
       r.tx = (float)tx; r.ty = (float)ty;
-      r.h = (float)(0.5 * L);
-      r.last = (k == e - 1) ? i : -1;
+      r.h = (float)pk_mul(0.5, L);
+      r.last = (k == e - 1) ? row : -1;
       r.slot = slot;
       r.pad = 0.f;
-      out.edges.push_back(r);
+      out[k] = r;
     }
-    out.row_begin.push_back((int)out.edges.size());
+    j = next_valid(j);
   }
-  // pair records for the tile-scan kernel
+  return 0;
+}
+
+// Pair record k2 (edges 2*k2, 2*k2+1) of an obstacle with e edge records `er`.
+PSDF_HD PairRec make_pair_rec(const EdgeRec* er, int e, int k2, int slot) {
+  const int k = 2 * k2;
+  const EdgeRec r0 = er[k];
+  const EdgeRec r1 = er[k + 1 < e ? k + 1 : k];                    // odd count: second half unused
+  PairRec pr;
+  pr.q0 = make_float4(r0.ax, r0.ay, r0.tx, r0.ty);
+  pr.q1 = make_float4(r1.ax, r1.ay, r1.tx, r1.ty);
+  const int last = (k + 2 >= e) ? er[e - 1].last : -1;
+  pr.q2 = make_float4(r0.h, k + 1 < e ? r1.h : -1.f, __builtin_bit_cast(float, last),
+                      __builtin_bit_cast(float, slot));            // h1 < 0: no second edge
+  return pr;
+}
+
+// Host packer.  returns 0 ok, -2 degenerate
+inline int pack_scene(const float* A, const float* B, const uint8_t* S, int M, int E, PackedScene& out) {
+  out.edges.clear();
   out.pairs.clear();
+  out.row_begin.assign(1, 0);
   out.pair_begin.assign(1, 0);
-  const int Mv = (int)out.row_begin.size() - 1;
-  for (int s = 0; s < Mv; ++s) {
-    const int b = out.row_begin[s], e = out.row_begin[s + 1];
-    for (int k = b; k < e; k += 2) {
-      const EdgeRec& r0 = out.edges[k];
-      const EdgeRec& r1 = out.edges[k + 1 < e ? k + 1 : k];      // odd count: repeat the last edge
-      PairRec pr;
-      pr.q0 = make_float4(r0.ax, r0.ay, r0.tx, r0.ty);
-      pr.q1 = make_float4(r1.ax, r1.ay, r1.tx, r1.ty);
-      const int last = (k + 2 >= e) ? out.edges[e - 1].last : -1;
-      float lf, sf;
-      std::memcpy(&lf, &last, 4);
-      std::memcpy(&sf, &s, 4);
-      pr.q2 = make_float4(r0.h, r1.h, lf, sf);
-      out.pairs.push_back(pr);
-    }
+  out.empty_rows.clear();
+  std::vector<EdgeRec> tmp((size_t)E);
+  for (int i = 0; i < M; ++i) {
+    int e = 0;
+    const int slot = (int)out.row_begin.size() - 1;
+    if (pack_row(A + (size_t)i * E * 2, B + (size_t)i * E * 2, S + (size_t)i * E, E, i, slot, tmp.data(), &e) != 0)
+      return -2;
+    if (e == 0) { out.empty_rows.push_back(i); continue; }
+    out.edges.insert(out.edges.end(), tmp.begin(), tmp.begin() + e);
+    for (int k2 = 0; k2 < (e + 1) / 2; ++k2) out.pairs.push_back(make_pair_rec(tmp.data(), e, k2, slot));
+    out.row_begin.push_back((int)out.edges.size());
     out.pair_begin.push_back((int)out.pairs.size());
   }
   return 0;
