@@ -7,6 +7,7 @@
 #include "../../include/psdf.h"
 #include "psdf_kernels.cuh"
 #include "psdf_pack.h"
+#include "psdf_pack_kernels.cuh"
 
 using namespace psdf;
 
@@ -50,6 +51,11 @@ struct psdf_scene {
   unsigned long long* d_ws_depth = nullptr;
   unsigned long long* d_ws_d2 = nullptr;
   unsigned int* d_ws_count = nullptr;
+  // device packer scratch (psdf_pack_kernels.cuh)
+  int* d_cnt = nullptr;               // [M] valid edges per row
+  int4* d_offs = nullptr;             // [M] scanned offsets
+  int* d_pair_begin = nullptr;        // [M+1]
+  PackTotals* d_totals = nullptr;
   // host (graph) path
   cudaStream_t gstream = nullptr;
   float* h_in = nullptr;              // pinned [max_poses,3]
@@ -177,19 +183,38 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
   return PSDF_OK;
 }
 
+// Device-resident (A,B,S): pack on the GPU (count+validate -> scan -> write); only the
+// totals and the per-obstacle pair offsets (for the host launch plan) come back.
+psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const uint8_t* S, cudaStream_t st) {
+  const int M = sc->M, E = sc->E;
+  const int bd = 128, gd = (M + bd - 1) / bd;
+  CU_TRY(cudaMemsetAsync(sc->d_totals, 0, sizeof(PackTotals), st));
+  pack_count_kernel<<<gd, bd, 0, st>>>(A, B, S, M, E, sc->d_cnt, sc->d_totals);
+  pack_scan_kernel<<<1, 1024, 0, st>>>(sc->d_cnt, M, sc->d_offs, sc->d_totals);
+  g_launches.fetch_add(2);
+  PackTotals t{};
+  CU_TRY(cudaMemcpyAsync(&t, sc->d_totals, sizeof(t), cudaMemcpyDeviceToHost, st));
+  CU_TRY(cudaStreamSynchronize(st));
+  CU_TRY(cudaGetLastError());
+  if (t.status != 0) return PSDF_ERR_DEGENERATE;          // nothing live has been touched yet
+  pack_write_kernel<<<gd, bd, 0, st>>>(A, B, S, M, E, sc->d_cnt, sc->d_offs, sc->d_totals, sc->d_edges, sc->d_pairs,
+                                       sc->d_row_begin, sc->d_pair_begin, sc->d_empty);
+  g_launches.fetch_add(1);
+  sc->h_pair_begin.resize((size_t)t.Mv + 1);
+  CU_TRY(cudaMemcpyAsync(sc->h_pair_begin.data(), sc->d_pair_begin, sizeof(int) * ((size_t)t.Mv + 1),
+                         cudaMemcpyDeviceToHost, st));
+  CU_TRY(cudaStreamSynchronize(st));
+  CU_TRY(cudaGetLastError());
+  sc->n_edges = t.n_edges;
+  sc->Mv = t.Mv;
+  sc->n_empty = t.n_empty;
+  sc->n_pairs = t.n_pairs;
+  return PSDF_OK;
+}
+
 psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const uint8_t* S, psdf_mem where,
                          cudaStream_t st) {
-  const size_t nAB = (size_t)sc->M * sc->E * 2, nS = (size_t)sc->M * sc->E;
-  std::vector<float> hA, hB;
-  std::vector<uint8_t> hS;
-  if (where == PSDF_MEM_DEVICE) {
-    hA.resize(nAB); hB.resize(nAB); hS.resize(nS);
-    CU_TRY(cudaMemcpyAsync(hA.data(), A, nAB * sizeof(float), cudaMemcpyDeviceToHost, st));
-    CU_TRY(cudaMemcpyAsync(hB.data(), B, nAB * sizeof(float), cudaMemcpyDeviceToHost, st));
-    CU_TRY(cudaMemcpyAsync(hS.data(), S, nS, cudaMemcpyDeviceToHost, st));
-    CU_TRY(cudaStreamSynchronize(st));
-    A = hA.data(); B = hB.data(); S = hS.data();
-  }
+  if (where == PSDF_MEM_DEVICE) return pack_on_device(sc, A, B, S, st);
   PackedScene ps;
   if (pack_scene(A, B, S, sc->M, sc->E, ps) != 0) return PSDF_ERR_DEGENERATE;
   sc->n_edges = (int)ps.edges.size();
@@ -220,6 +245,7 @@ void psdf_destroy_scene(psdf_scene* sc) {
   if (sc->gstream) cudaStreamDestroy(sc->gstream);
   cudaFree(sc->d_edges); cudaFree(sc->d_pairs); cudaFree(sc->d_row_begin); cudaFree(sc->d_empty);
   cudaFree(sc->d_ws_depth); cudaFree(sc->d_ws_d2); cudaFree(sc->d_ws_count);
+  cudaFree(sc->d_cnt); cudaFree(sc->d_offs); cudaFree(sc->d_pair_begin); cudaFree(sc->d_totals);
   cudaFree(sc->d_in); cudaFree(sc->d_out); cudaFree(sc->d_per);
   if (sc->h_in) cudaFreeHost(sc->h_in);
   if (sc->h_out) cudaFreeHost(sc->h_out);
@@ -253,6 +279,10 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
     CU_TRY(cudaMalloc(&sc->d_pairs, sizeof(PairRec) * (size_t)(sc->edge_cap / 2 + M)));
     CU_TRY(cudaMalloc(&sc->d_row_begin, sizeof(int) * (size_t)(M + 1)));
     CU_TRY(cudaMalloc(&sc->d_empty, sizeof(int) * (size_t)M));
+    CU_TRY(cudaMalloc(&sc->d_cnt, sizeof(int) * (size_t)M));
+    CU_TRY(cudaMalloc(&sc->d_offs, sizeof(int4) * (size_t)M));
+    CU_TRY(cudaMalloc(&sc->d_pair_begin, sizeof(int) * (size_t)(M + 1)));
+    CU_TRY(cudaMalloc(&sc->d_totals, sizeof(PackTotals)));
     CU_TRY(cudaMalloc(&sc->d_ws_depth, sizeof(unsigned long long) * (size_t)max_poses));
     CU_TRY(cudaMalloc(&sc->d_ws_d2, sizeof(unsigned long long) * (size_t)max_poses));
     const size_t n_cnt = (size_t)(max_poses + 63) / 64 + 1;

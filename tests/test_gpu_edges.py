@@ -156,3 +156,68 @@ def test_table1_shapes(env):
             v, g, _ = scene.eval_host(w.poses)
             compare(ref, v, g, what=w.name)
             scene.close()
+
+
+def test_device_encode_edges(env):
+    """On-device EncodeEdges (Alg.1 l.1-4): device-resident (A,B,S) are
+    packed by the pack kernels; results must be bit-identical to the host packer, and a
+    rejected device update must leave the old scene in force."""
+    torch, O, psdf, W = env
+    rng = np.random.default_rng(77)
+    for cfg, n in ((4, 700), (5, 600)):
+        w = W.make_config(cfg).subsample(n)
+        A, B, S = w.A.copy(), w.B.copy(), w.S.copy()
+        for i in range(0, w.M, 3):                      # every third row clockwise
+            sl = np.nonzero(S[i])[0]
+            A[i, sl], B[i, sl] = w.B[i, sl][::-1].copy(), w.A[i, sl][::-1].copy()
+        S[5::17] = 0                                    # some absent obstacles
+        host = psdf.Scene(w.footprint, A, B, S, max_poses=n)
+        dev = psdf.Scene(w.footprint, torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(),
+                         torch.from_numpy(S).cuda(), max_poses=n)
+        assert (dev.num_obstacles, dev.num_edges) == (host.num_obstacles, host.num_edges)
+        a = _run(torch, host, w.poses, grad=True, per_obstacle=True)
+        b = _run(torch, dev, w.poses, grad=True, per_obstacle=True)
+        for x, y in zip(a, b):
+            assert np.array_equal(x, y)
+        compare(O.evaluate(w.footprint, A, B, S, w.poses[:200], per_obstacle=True), b[0][:200], b[1][:200], b[2][:200])
+        # device update with new values (perception update, PAPER.md:139) == fresh host scene
+        shift = rng.uniform(-0.5, 0.5, (w.M, 1, 2)).astype(np.float32)
+        A2 = (A + shift).astype(np.float32)
+        B2 = A2.copy()
+        for i in range(w.M):                            # re-close the rows after the shift
+            sl = np.nonzero(S[i])[0]
+            if sl.size:
+                B2[i, sl] = A2[i, np.roll(sl, -1)]         # B_j == A_next for either orientation
+        try:
+            host2 = psdf.Scene(w.footprint, A2, B2, S, max_poses=n)
+        except psdf.PsdfError:
+            host2 = None                                # fp32 rounding of the shift made an edge degenerate
+        if host2 is not None:
+            dev.update(torch.from_numpy(A2).cuda(), torch.from_numpy(B2).cuda(), torch.from_numpy(S).cuda())
+            for x, y in zip(_run(torch, host2, w.poses, grad=True), _run(torch, dev, w.poses, grad=True)):
+                assert x is None or np.array_equal(x, y)
+            host2.close()
+            dev.update(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), torch.from_numpy(S).cuda())
+        # degenerate device updates are rejected, old scene stays
+        bad = []
+        S1 = S.copy(); r = int(np.nonzero(S.sum(1) > 3)[0][0]); S1[r, np.nonzero(S1[r])[0][1]] = 0
+        bad.append((A, B, S1))                          # open row
+        S2 = S.copy(); r2 = int(np.nonzero(S.sum(1) >= 3)[0][1]); S2[r2] = 0; S2[r2, :2] = 1
+        bad.append((A, B, S2))                          # fewer than 3 edges
+        A3, B3 = A.copy(), B.copy(); sl = np.nonzero(S[r])[0]
+        A3[r, sl[1]] = B3[r, sl[0]] = A[r, sl[0]]
+        bad.append((A3, B3, S))                         # zero-length edge
+        A4, B4 = A.copy(), B.copy()
+        c = A[r, sl].mean(0)
+        A4[r, sl[1]] = B4[r, sl[0]] = (c - 0.3 * (A[r, sl[1]] - c)).astype(np.float32)   # past the diagonal
+        bad.append((A4, B4, S))                         # dented (non-convex) polygon
+        for Ab, Bb, Sb in bad:
+            with pytest.raises(psdf.PsdfError) as e:
+                dev.update(torch.from_numpy(Ab).cuda(), torch.from_numpy(Bb).cuda(), torch.from_numpy(Sb).cuda())
+            assert e.value.status == psdf.PSDF_ERR_DEGENERATE
+            with pytest.raises(psdf.PsdfError):
+                host.update(Ab, Bb, Sb)                 # the host packer agrees
+            for x, y in zip(a, _run(torch, dev, w.poses, grad=True, per_obstacle=True)):
+                assert np.array_equal(x, y)
+        host.close()
+        dev.close()
