@@ -91,6 +91,14 @@ psdf_status psdf_eval_host(psdf_scene* scene, const float* poses, int N, float* 
 psdf_status psdf_mpc_coeffs_host(psdf_scene* scene, const float* poses, int N, float d_min,
                                  float rho_p, float rho_theta, float* coeff);
 
+/* Exact broad-phase culling (beyond the paper; valid because phi is a minimum over obstacles,
+ * eq.(6)).  When enabled, large batches (N > 2048) evaluated without
+ * per_obstacle output go through a grid sort of the poses and a warp-per-32-poses kernel that
+ * skips every obstacle whose bounding-circle lower bound |p - c_i| - R_i - r_max exceeds the
+ * running value; surviving pairs use the same arithmetic as the dense path, so value and grad
+ * are bit-identical to the dense result.  Default: disabled (dense, branch-free evaluation). */
+psdf_status psdf_set_culling(psdf_scene* scene, int enable);
+
 void psdf_destroy_scene(psdf_scene* scene);
 
 /* Introspection (no CUDA work). */

@@ -6,6 +6,7 @@
 
 #include "../../include/psdf.h"
 #include "psdf_kernels.cuh"
+#include "psdf_cull_kernels.cuh"
 #include "psdf_pack.h"
 #include "psdf_pack_kernels.cuh"
 
@@ -56,6 +57,12 @@ struct psdf_scene {
   int4* d_offs = nullptr;             // [M] scanned offsets
   int* d_pair_begin = nullptr;        // [M+1]
   PackTotals* d_totals = nullptr;
+  // culled path (psdf_cull_kernels.cuh)
+  int culling = 0;                    // psdf_set_culling
+  float4* d_bounds = nullptr;         // [M]
+  int* d_perm = nullptr;              // [max_poses]
+  int* d_cell = nullptr;              // [kSortGridMax^2 + 1]
+  unsigned int* d_bbox = nullptr;     // [4]
   // host (graph) path
   cudaStream_t gstream = nullptr;
   float* h_in = nullptr;              // pinned [max_poses,3]
@@ -91,6 +98,56 @@ cudaError_t launch_mode(const psdf_scene* sc, const EvalParams& p, int mode, boo
     case kCoeff: return launch_one<V, kCoeff>(sc, p, lanes, grid, bd, st);
     default: return cudaErrorInvalidValue;
   }
+}
+
+template <int V>
+cudaError_t launch_cull_mode(const psdf_scene* sc, const EvalParams& p, int mode, dim3 grid, cudaStream_t st) {
+  switch (mode) {
+    case 0: psdf_cull_kernel<V, 0><<<grid, 64, 0, st>>>(sc->fp, p); break;
+    case kGrad: psdf_cull_kernel<V, kGrad><<<grid, 64, 0, st>>>(sc->fp, p); break;
+    case kCoeff: psdf_cull_kernel<V, kCoeff><<<grid, 64, 0, st>>>(sc->fp, p); break;
+    default: return cudaErrorInvalidValue;
+  }
+  g_launches.fetch_add(1);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_cull_v(const psdf_scene* sc, const EvalParams& p, int mode, dim3 grid, cudaStream_t st) {
+  switch (sc->Vp) {
+    case 4: return launch_cull_mode<4>(sc, p, mode, grid, st);
+    case 6: return launch_cull_mode<6>(sc, p, mode, grid, st);
+    case 8: return launch_cull_mode<8>(sc, p, mode, grid, st);
+    case 10: return launch_cull_mode<10>(sc, p, mode, grid, st);
+    case 12: return launch_cull_mode<12>(sc, p, mode, grid, st);
+    case 16: return launch_cull_mode<16>(sc, p, mode, grid, st);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+// Culled path: grid-sort the poses (4 small kernels), then one warp per 32 sorted poses.
+cudaError_t enqueue_culled(const psdf_scene* sc, EvalParams& p, int mode, cudaStream_t st) {
+  SortParams s{};
+  s.poses = p.poses;
+  s.N = p.N;
+  int G = (int)std::floor(std::sqrt((double)p.N / 32.0));
+  s.G = G < 1 ? 1 : (G > kSortGridMax ? kSortGridMax : G);
+  s.bbox = sc->d_bbox;
+  s.cell = sc->d_cell;
+  s.perm = sc->d_perm;
+  cudaError_t e;
+  if ((e = cudaMemsetAsync(sc->d_bbox, 0xff, 4 * sizeof(unsigned int), st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(sc->d_cell, 0, sizeof(int) * (size_t)(s.G * s.G + 1), st)) != cudaSuccess) return e;
+  const int bd = 256, gd = (p.N + bd - 1) / bd;
+  pose_bbox_kernel<<<gd < 4 * sc->sm_count ? gd : 4 * sc->sm_count, bd, 0, st>>>(s);
+  pose_hist_kernel<<<gd, bd, 0, st>>>(s);
+  pose_scan_kernel<<<1, 1024, 0, st>>>(s);
+  pose_scatter_kernel<<<gd, bd, 0, st>>>(s);
+  g_launches.fetch_add(4);
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  p.perm = sc->d_perm;
+  p.bounds = sc->d_bounds;
+  p.n_chunks = 1;
+  return launch_cull_v(sc, p, mode, dim3((unsigned)((p.N + 63) / 64)), st);
 }
 
 cudaError_t launch_v(const psdf_scene* sc, const EvalParams& p, int mode, bool lanes, dim3 grid, int bd,
@@ -140,6 +197,14 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
   const bool lanes = N <= 2048 || pairs <= (1 << 16);
   dim3 grid;
   int bd;
+  if (sc->culling && !lanes && !per_obs && sc->Mv >= 64) {
+    cudaError_t e = enqueue_culled(sc, p, mode, st);
+    if (e != cudaSuccess) {
+      g_last_cuda_error.store((int)e);
+      return PSDF_ERR_CUDA;
+    }
+    return PSDF_OK;
+  }
   if (lanes) {
     int K = 1;
     while (K < 32 && K < sc->Mv && (long long)N * K < 148LL * 4 * 128) K <<= 1;
@@ -198,7 +263,7 @@ psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const
   CU_TRY(cudaGetLastError());
   if (t.status != 0) return PSDF_ERR_DEGENERATE;          // nothing live has been touched yet
   pack_write_kernel<<<gd, bd, 0, st>>>(A, B, S, M, E, sc->d_cnt, sc->d_offs, sc->d_totals, sc->d_edges, sc->d_pairs,
-                                       sc->d_row_begin, sc->d_pair_begin, sc->d_empty);
+                                       sc->d_row_begin, sc->d_pair_begin, sc->d_empty, sc->d_bounds);
   g_launches.fetch_add(1);
   sc->h_pair_begin.resize((size_t)t.Mv + 1);
   CU_TRY(cudaMemcpyAsync(sc->h_pair_begin.data(), sc->d_pair_begin, sizeof(int) * ((size_t)t.Mv + 1),
@@ -226,6 +291,8 @@ psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const u
     CU_TRY(cudaMemcpyAsync(sc->d_edges, ps.edges.data(), sizeof(EdgeRec) * sc->n_edges, cudaMemcpyHostToDevice, st));
     CU_TRY(cudaMemcpyAsync(sc->d_pairs, ps.pairs.data(), sizeof(PairRec) * sc->n_pairs, cudaMemcpyHostToDevice, st));
   }
+  if (sc->Mv)
+    CU_TRY(cudaMemcpyAsync(sc->d_bounds, ps.bounds.data(), sizeof(float4) * sc->Mv, cudaMemcpyHostToDevice, st));
   CU_TRY(cudaMemcpyAsync(sc->d_row_begin, ps.row_begin.data(), sizeof(int) * (sc->Mv + 1), cudaMemcpyHostToDevice, st));
   if (sc->n_empty)
     CU_TRY(cudaMemcpyAsync(sc->d_empty, ps.empty_rows.data(), sizeof(int) * sc->n_empty, cudaMemcpyHostToDevice, st));
@@ -245,6 +312,7 @@ void psdf_destroy_scene(psdf_scene* sc) {
   if (sc->gstream) cudaStreamDestroy(sc->gstream);
   cudaFree(sc->d_edges); cudaFree(sc->d_pairs); cudaFree(sc->d_row_begin); cudaFree(sc->d_empty);
   cudaFree(sc->d_ws_depth); cudaFree(sc->d_ws_d2); cudaFree(sc->d_ws_count);
+  cudaFree(sc->d_bounds); cudaFree(sc->d_perm); cudaFree(sc->d_cell); cudaFree(sc->d_bbox);
   cudaFree(sc->d_cnt); cudaFree(sc->d_offs); cudaFree(sc->d_pair_begin); cudaFree(sc->d_totals);
   cudaFree(sc->d_in); cudaFree(sc->d_out); cudaFree(sc->d_per);
   if (sc->h_in) cudaFreeHost(sc->h_in);
@@ -283,6 +351,10 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
     CU_TRY(cudaMalloc(&sc->d_offs, sizeof(int4) * (size_t)M));
     CU_TRY(cudaMalloc(&sc->d_pair_begin, sizeof(int) * (size_t)(M + 1)));
     CU_TRY(cudaMalloc(&sc->d_totals, sizeof(PackTotals)));
+    CU_TRY(cudaMalloc(&sc->d_bounds, sizeof(float4) * (size_t)M));
+    CU_TRY(cudaMalloc(&sc->d_perm, sizeof(int) * (size_t)max_poses));
+    CU_TRY(cudaMalloc(&sc->d_cell, sizeof(int) * (size_t)(kSortGridMax * kSortGridMax + 1)));
+    CU_TRY(cudaMalloc(&sc->d_bbox, sizeof(unsigned int) * 4));
     CU_TRY(cudaMalloc(&sc->d_ws_depth, sizeof(unsigned long long) * (size_t)max_poses));
     CU_TRY(cudaMalloc(&sc->d_ws_d2, sizeof(unsigned long long) * (size_t)max_poses));
     const size_t n_cnt = (size_t)(max_poses + 63) / 64 + 1;
@@ -421,6 +493,17 @@ psdf_status psdf_mpc_coeffs_host(psdf_scene* sc, const float* poses, int N, floa
   s = run_graph(sc, N, kCoeff, d_min, rho_p, rho_theta);
   if (s != PSDF_OK) return s;
   std::memcpy(coeff, sc->h_out, sizeof(float) * 4 * (size_t)N);
+  return PSDF_OK;
+}
+
+psdf_status psdf_set_culling(psdf_scene* sc, int enable) {
+  if (!sc) return PSDF_ERR_INVALID_ARG;
+  if (sc->gstream) CU_TRY(cudaStreamSynchronize(sc->gstream));
+  sc->culling = enable ? 1 : 0;
+  for (auto& g : sc->graphs) {           // launch plans are baked into the captured graphs
+    if (g.exec) cudaGraphExecDestroy(g.exec);
+    g = GraphEntry();
+  }
   return PSDF_OK;
 }
 

@@ -1,0 +1,178 @@
+// Exact broad-phase culling (beyond the paper).  phi is a minimum
+// over obstacles (eq.(6)), so an obstacle whose lower bound
+//     sd^i >= |p - c_i| - R_i - r_max          (bounding circles of obstacle and footprint)
+// exceeds an upper bound of phi already in hand cannot be the arg-min and cannot change the
+// value: skipping it is exact.  The culled path evaluates every surviving (pose, obstacle)
+// pair with the same arithmetic as the dense tile-scan kernel (edge_step2), so its outputs
+// are bit-identical to the dense path.
+//
+//   * poses are bucketed into a uniform grid (counting sort: bbox -> histogram -> scan ->
+//     scatter) so that the 32 poses of a warp are spatially close;
+//   * one warp owns 32 sorted poses and walks the obstacle bounds 32 at a time: lane j tests
+//     obstacle j against the warp's pose box and its largest running upper bound (one test per
+//     obstacle per WARP), the ballot gives the survivors, each survivor is re-tested per lane
+//     and evaluated only if some lane still needs it; records are read straight from L2/L1
+//     with warp-uniform 128-bit loads (no shared memory, no block barriers);
+//   * the running upper bound is the exact value over the obstacles evaluated so far.
+#pragma once
+#include "psdf_kernels.cuh"
+
+namespace psdf {
+
+constexpr int kSortGridMax = 64;      // pose grid is G x G cells, G <= 64
+
+__device__ __forceinline__ float warp_min_f(float v) { return fkey_inv(__reduce_min_sync(0xffffffffu, fkey(v))); }
+__device__ __forceinline__ float warp_max_f(float v) { return fkey_inv(__reduce_max_sync(0xffffffffu, fkey(v))); }
+
+struct SortParams {
+  const float* poses;
+  int N, G;
+  unsigned int* bbox;      // [4] ordered keys: min x, min y, ~max x, ~max y  (all atomicMin; clean = 0xff..)
+  int* cell;               // [G*G + 1] histogram -> offsets -> cursors
+  int* perm;               // [N] sorted position -> pose index
+};
+
+__device__ __forceinline__ bool pose_finite(float x, float y) { return isfinite(x) && isfinite(y); }
+
+__global__ void pose_bbox_kernel(const SortParams s) {
+  float x0 = kInf, y0 = kInf, x1 = -kInf, y1 = -kInf;
+  for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < s.N; n += gridDim.x * blockDim.x) {
+    const float x = __ldg(s.poses + 3 * n), y = __ldg(s.poses + 3 * n + 1);
+    if (pose_finite(x, y)) { x0 = fminf(x0, x); y0 = fminf(y0, y); x1 = fmaxf(x1, x); y1 = fmaxf(y1, y); }
+  }
+  x0 = warp_min_f(x0); y0 = warp_min_f(y0); x1 = warp_max_f(x1); y1 = warp_max_f(y1);
+  if ((threadIdx.x & 31) == 0) {
+    atomicMin(s.bbox + 0, fkey(x0)); atomicMin(s.bbox + 1, fkey(y0));
+    atomicMin(s.bbox + 2, ~fkey(x1)); atomicMin(s.bbox + 3, ~fkey(y1));
+  }
+}
+
+__device__ __forceinline__ int pose_cell(const SortParams& s, int n) {
+  const float x = __ldg(s.poses + 3 * n), y = __ldg(s.poses + 3 * n + 1);
+  if (!pose_finite(x, y)) return 0;
+  const float x0 = fkey_inv(s.bbox[0]), y0 = fkey_inv(s.bbox[1]);
+  const float x1 = fkey_inv(~s.bbox[2]), y1 = fkey_inv(~s.bbox[3]);
+  const float sx = (float)s.G / fmaxf(x1 - x0, 1e-6f), sy = (float)s.G / fmaxf(y1 - y0, 1e-6f);
+  const int gx = min(max((int)((x - x0) * sx), 0), s.G - 1);
+  int gy = min(max((int)((y - y0) * sy), 0), s.G - 1);
+  if (gx & 1) gy = s.G - 1 - gy;                          // snake order: neighbours stay neighbours
+  return gx * s.G + gy;
+}
+
+__global__ void pose_hist_kernel(const SortParams s) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n < s.N) atomicAdd(s.cell + pose_cell(s, n), 1);
+}
+
+// one CTA of 1024 threads: exclusive scan of the (<= 4096) cell counts, in place
+__global__ void __launch_bounds__(1024) pose_scan_kernel(const SortParams s) {
+  __shared__ int wsum[32];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int cells = s.G * s.G;
+  int v[4], sum = 0;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { const int c = 4 * tid + k; v[k] = c < cells ? s.cell[c] : 0; sum += v[k]; }
+  int inc = sum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+  if (lane == 31) wsum[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    const int w = wsum[lane];
+    int winc = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += t; }
+    wsum[lane] = winc - w;
+  }
+  __syncthreads();
+  int run = wsum[wid] + inc - sum;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { const int c = 4 * tid + k; if (c < cells) s.cell[c] = run; run += v[k]; }
+}
+
+__global__ void pose_scatter_kernel(const SortParams s) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n < s.N) s.perm[atomicAdd(s.cell + pose_cell(s, n), 1)] = n;
+}
+
+// Per-obstacle bound, one float4 per packed obstacle: bounding circle (cx, cy, R) of its
+// vertices and the index of its first pair record (int bits).
+//
+// Culled evaluation: one warp = 32 sorted poses; MODE in {0, kGrad, kCoeff}.
+template <int V, int MODE>
+__global__ void __launch_bounds__(64) psdf_cull_kernel(const __grid_constant__ Footprint fp,
+                                                       const __grid_constant__ EvalParams p) {
+  const int lane = threadIdx.x & 31;
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  const int n = __ldg(p.perm + min(k, p.N - 1));           // tail lanes recompute the last pose
+  const float x = __ldg(p.poses + 3 * n), y = __ldg(p.poses + 3 * n + 1), th = __ldg(p.poses + 3 * n + 2);
+  const bool finite = isfinite(x) && isfinite(y) && isfinite(th);
+  Posed2<V> P;
+  pose_setup2<V>(fp, x, y, th, P);
+  // pose box of the warp (non-finite poses take no part; they are finalised to NaN)
+  const float xmin = warp_min_f(finite ? x : kInf), xmax = warp_max_f(finite ? x : -kInf);
+  const float ymin = warp_min_f(finite ? y : kInf), ymax = warp_max_f(finite ? y : -kInf);
+  const float rpad = fp.rmax * 1.0001f + 1e-4f;            // footprint radius + safety for fp32 rounding
+
+  ObstacleAcc<V> acc;
+  float minD2 = kInf, prevD2 = kInf, maxDepth = -kInf;
+  float ub = finite ? kInf : -kInf;                        // running upper bound of phi for this lane
+  int idD2 = -1, idDepth = -1;
+  const float4* __restrict__ bounds = p.bounds;
+  const float4* __restrict__ recs = reinterpret_cast<const float4*>(p.pairs);
+
+  for (int base = 0; base < p.Mv; base += 32) {
+    const int i = base + lane;
+    const float4 b = i < p.Mv ? __ldg(bounds + i) : make_float4(0.f, 0.f, 0.f, 0.f);
+    const float ubmax = warp_max_f(ub);
+    // distance from the obstacle centre to the warp's pose box
+    const float ddx = fmaxf(fmaxf(xmin - b.x, b.x - xmax), 0.f), ddy = fmaxf(fmaxf(ymin - b.y, b.y - ymax), 0.f);
+    const float thr = (ubmax + b.z) * 1.0001f + rpad;
+    const bool skip = (i >= p.Mv) || (thr < 0.f) || (fmaf(ddx, ddx, ddy * ddy) > thr * thr);
+    unsigned mask = __ballot_sync(0xffffffffu, !skip);
+    while (mask) {
+      const int j = __ffs(mask) - 1;
+      mask &= mask - 1;
+      const float cx = __shfl_sync(0xffffffffu, b.x, j), cy = __shfl_sync(0xffffffffu, b.y, j);
+      const float R = __shfl_sync(0xffffffffu, b.z, j);
+      int rec = __shfl_sync(0xffffffffu, __float_as_int(b.w), j);
+      // exact per-lane test against this lane's own bound
+      const float dx = cx - x, dy = cy - y;
+      const float t = (ub + R) * 1.0001f + rpad;
+      const bool need = !((t < 0.f) || (fmaf(dx, dx, dy * dy) > t * t));
+      if (!__any_sync(0xffffffffu, need)) continue;
+      acc.reset();
+      const float4* src = recs + 3 * (size_t)rec;
+      float4 q0 = __ldg(src), q1 = __ldg(src + 1), q2 = __ldg(src + 2);
+      int last, slot;
+      while (true) {
+        last = __float_as_int(q2.z);
+        slot = __float_as_int(q2.w);
+        const float4 c0 = q0, c1 = q1;
+        const float h0 = q2.x, h1 = q2.y;
+        if (last < 0) {                                    // prefetch the next record of this obstacle
+          src += 3;
+          q0 = __ldg(src); q1 = __ldg(src + 1); q2 = __ldg(src + 2);
+        }
+        edge_step2<V>(fp, P, c0, h0, acc, minD2);
+        if (h1 >= 0.f) edge_step2<V>(fp, P, c1, h1, acc, minD2);
+        if (last >= 0) break;
+      }
+      const float depth = acc.depth();
+      if (MODE & (kGrad | kCoeff)) {
+        if (minD2 < prevD2) { prevD2 = minD2; idD2 = slot; }
+      }
+      if (depth > maxDepth) { maxDepth = depth; idDepth = slot; }
+      if (finite) ub = maxDepth >= 0.f ? -maxDepth : sqrtf(minD2);
+    }
+  }
+  if (!(MODE & (kGrad | kCoeff))) idD2 = minD2 < kInf ? 0 : -1;
+  if (k >= p.N) return;
+  const bool separated = !(maxDepth >= 0.f);
+  const float value = separated ? sqrtf(minD2) : -maxDepth;
+  Posed<V> Ps;
+  unpack_pose<V>(P, Ps);
+  finalize_pose<V, MODE>(fp, p, Ps, n, th, value, separated ? idD2 : idDepth, separated);
+}
+
+}  // namespace psdf

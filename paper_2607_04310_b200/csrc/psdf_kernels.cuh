@@ -17,6 +17,8 @@ struct EvalParams {
   const PairRec* pairs;        // [n_pairs] the same edges two per record (tile-scan kernel)
   const int* row_begin;        // [Mv+1] packed obstacle -> first edge
   const int* empty_rows;       // [n_empty] obstacle rows with no valid edge
+  const float4* bounds;        // [Mv] per-obstacle bounding circle + first pair record (culled path)
+  const int* perm;             // [N] grid-sorted position -> pose index (culled path)
   const float* poses;          // [N,3]
   float* value;                // [N]
   float* grad;                 // [N,3] or null

@@ -17,6 +17,7 @@ struct PackedScene {
   std::vector<PairRec> pairs;     // tile-scan records: two edges each, grouped by obstacle
   std::vector<int> pair_begin;    // [Mv+1]
   std::vector<int> empty_rows;
+  std::vector<float4> bounds;     // [Mv] bounding circle + first pair record per obstacle
 };
 
 // Double-precision helpers that round identically on host and device: nvcc contracts a*b+c
@@ -120,6 +121,26 @@ PSDF_HD PairRec make_pair_rec(const EdgeRec* er, int e, int k2, int slot) {
   return pr;
 }
 
+// Bounding circle of an obstacle's vertices (culled path, psdf_cull_kernels.cuh): centre of the
+// vertex bounding box, radius rounded up; .w = index of the obstacle's first pair record.
+PSDF_HD float4 obstacle_bound(const EdgeRec* er, int e, int pair_begin) {
+  double x0 = er[0].ax, x1 = er[0].ax, y0 = er[0].ay, y1 = er[0].ay;
+  for (int k = 1; k < e; ++k) {
+    const double x = er[k].ax, y = er[k].ay;
+    x0 = x < x0 ? x : x0; x1 = x > x1 ? x : x1;
+    y0 = y < y0 ? y : y0; y1 = y > y1 ? y : y1;
+  }
+  const float cx = (float)pk_mul(0.5, pk_add(x0, x1)), cy = (float)pk_mul(0.5, pk_add(y0, y1));
+  double r2 = 0.0;
+  for (int k = 0; k < e; ++k) {
+    const double dx = pk_sub((double)er[k].ax, (double)cx), dy = pk_sub((double)er[k].ay, (double)cy);
+    const double d2 = pk_add(pk_mul(dx, dx), pk_mul(dy, dy));
+    r2 = d2 > r2 ? d2 : r2;
+  }
+  const float R = (float)pk_add(pk_mul(pk_sqrt(r2), 1.000001), 1e-6);     // rounded up
+  return make_float4(cx, cy, R, __builtin_bit_cast(float, pair_begin));
+}
+
 // Host packer.  returns 0 ok, -2 degenerate
 inline int pack_scene(const float* A, const float* B, const uint8_t* S, int M, int E, PackedScene& out) {
   out.edges.clear();
@@ -127,6 +148,7 @@ inline int pack_scene(const float* A, const float* B, const uint8_t* S, int M, i
   out.row_begin.assign(1, 0);
   out.pair_begin.assign(1, 0);
   out.empty_rows.clear();
+  out.bounds.clear();
   std::vector<EdgeRec> tmp((size_t)E);
   for (int i = 0; i < M; ++i) {
     int e = 0;
@@ -135,6 +157,7 @@ inline int pack_scene(const float* A, const float* B, const uint8_t* S, int M, i
       return -2;
     if (e == 0) { out.empty_rows.push_back(i); continue; }
     out.edges.insert(out.edges.end(), tmp.begin(), tmp.begin() + e);
+    out.bounds.push_back(obstacle_bound(tmp.data(), e, (int)out.pairs.size()));
     for (int k2 = 0; k2 < (e + 1) / 2; ++k2) out.pairs.push_back(make_pair_rec(tmp.data(), e, k2, slot));
     out.row_begin.push_back((int)out.edges.size());
     out.pair_begin.push_back((int)out.pairs.size());

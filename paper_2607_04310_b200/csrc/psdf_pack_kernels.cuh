@@ -89,7 +89,7 @@ __global__ void pack_write_kernel(const float* __restrict__ A, const float* __re
                                   const int4* __restrict__ offs, const PackTotals* __restrict__ totals,
                                   EdgeRec* __restrict__ edges, PairRec* __restrict__ pairs,
                                   int* __restrict__ row_begin, int* __restrict__ pair_begin,
-                                  int* __restrict__ empty_rows) {
+                                  int* __restrict__ empty_rows, float4* __restrict__ bounds) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i == 0) {
     row_begin[totals->Mv] = totals->n_edges;
@@ -102,6 +102,7 @@ __global__ void pack_write_kernel(const float* __restrict__ A, const float* __re
   EdgeRec* er = edges + o.y;
   pack_row(A + (size_t)i * E * 2, B + (size_t)i * E * 2, S + (size_t)i * E, E, i, o.x, er, &e);
   for (int k2 = 0; k2 < (e + 1) >> 1; ++k2) pairs[o.z + k2] = make_pair_rec(er, e, k2, o.x);
+  bounds[o.x] = obstacle_bound(er, e, o.z);
   row_begin[o.x] = o.y;
   pair_begin[o.x] = o.z;
 }

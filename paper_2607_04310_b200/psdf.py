@@ -24,7 +24,7 @@ PSDF_MEM_HOST = 0
 PSDF_MEM_DEVICE = 1
 
 EXPORTS = ["psdf_create_scene", "psdf_update_scene", "psdf_eval", "psdf_eval_host",
-           "psdf_mpc_coeffs_host", "psdf_destroy_scene", "psdf_scene_num_obstacles",
+           "psdf_mpc_coeffs_host", "psdf_set_culling", "psdf_destroy_scene", "psdf_scene_num_obstacles",
            "psdf_scene_num_edges", "psdf_last_cuda_error", "psdf_kernel_launches",
            "psdf_status_string", "psdf_version", "psdf_measure_fp32_peak"]
 
@@ -60,6 +60,8 @@ def lib():
     L.psdf_eval_host.argtypes = [vp, fp_, i, fp_, fp_, fp_]
     L.psdf_mpc_coeffs_host.restype = i
     L.psdf_mpc_coeffs_host.argtypes = [vp, fp_, i, ctypes.c_float, ctypes.c_float, ctypes.c_float, fp_]
+    L.psdf_set_culling.restype = i
+    L.psdf_set_culling.argtypes = [vp, i]
     L.psdf_destroy_scene.restype = None
     L.psdf_destroy_scene.argtypes = [vp]
     L.psdf_scene_num_obstacles.restype = i
@@ -169,6 +171,10 @@ class Scene:
     def num_edges(self):
         return int(lib().psdf_scene_num_edges(self._h))
 
+    def set_culling(self, enable: bool):
+        """psdf_set_culling: exact broad-phase culling for large batches (default off)."""
+        _check(lib().psdf_set_culling(self._h, int(bool(enable))), "psdf_set_culling")
+
     def update(self, A, B, S, stream=None):
         """psdf_update_scene: same (M,E), values only."""
         if _is_torch(A):
@@ -251,6 +257,10 @@ def psdf_update_scene(scene: Scene, A, B, S, stream=None):
 
 def psdf_mpc_coeffs_host(scene: Scene, poses, d_min, rho_p, rho_theta):
     return scene.mpc_coeffs_host(poses, d_min, rho_p, rho_theta)
+
+
+def psdf_set_culling(scene: Scene, enable: bool):
+    return scene.set_culling(enable)
 
 
 def psdf_destroy_scene(scene: Scene):

@@ -102,3 +102,40 @@ def test_per_obstacle_large_batch(env, workloads_cache):
     print(compare(ref, v, g, po, what="per-obstacle scan path"))
     assert np.array_equal(po.min(axis=1), v)
     scene.close()
+
+
+@pytest.mark.parametrize("cfg,n", [(3, None), (4, None), (5, None), (5, 4099), (2, None)])
+def test_culled_path_bit_identical_to_dense(env, workloads_cache, cfg, n):
+    """psdf_set_culling (exact broad-phase culling, NEXT-3): same value and gradient bits as
+    the dense path at BASELINE full sizes and on a ragged size; unique results, so compared
+    exactly.  cfg 2 is below the culled path's size threshold: the switch must be inert."""
+    torch, O, psdf = env
+    w = workloads_cache(cfg)
+    if n is not None:
+        w = w.subsample(n)
+    scene, (v, g, _) = _gpu_eval(torch, psdf, w, grad=True)
+    p = torch.from_numpy(w.poses).cuda()
+    scene.set_culling(True)
+    for with_grad in (True, False):
+        v1, g1, _ = scene.eval(p, grad=with_grad)
+        torch.cuda.synchronize()
+        assert np.array_equal(v1.cpu().numpy(), v)
+        if with_grad:
+            assert np.array_equal(g1.cpu().numpy(), g)
+    # non-finite poses and a second call (workspace left clean)
+    q = w.poses.copy()
+    q[7, 0] = np.nan
+    q[w.N // 2, 2] = np.inf
+    v2, g2, _ = scene.eval(torch.from_numpy(q).cuda(), grad=True)
+    v2, g2 = v2.cpu().numpy(), g2.cpu().numpy()
+    bad = np.zeros(w.N, bool)
+    bad[[7, w.N // 2]] = True
+    assert np.isnan(v2[bad]).all() and np.array_equal(v2[~bad], v[~bad]) and np.array_equal(g2[~bad], g[~bad])
+    if cfg == 5 and n is not None:
+        # per-stage coefficients through the host path with culling on
+        c = scene.mpc_coeffs_host(w.poses, 0.01, 0.1, 0.1)
+        assert np.array_equal(c[:, 1:], -g)
+    scene.set_culling(False)
+    v3, _, _ = scene.eval(p, grad=False)
+    assert np.array_equal(v3.cpu().numpy(), v)
+    scene.close()
