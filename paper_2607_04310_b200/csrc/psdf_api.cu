@@ -101,25 +101,25 @@ cudaError_t launch_mode(const psdf_scene* sc, const EvalParams& p, int mode, boo
 }
 
 template <int V>
-cudaError_t launch_cull_mode(const psdf_scene* sc, const EvalParams& p, int mode, dim3 grid, cudaStream_t st) {
+cudaError_t launch_cull_mode(const psdf_scene* sc, const EvalParams& p, int mode, dim3 grid, int bd, cudaStream_t st) {
   switch (mode) {
-    case 0: psdf_cull_kernel<V, 0><<<grid, 64, 0, st>>>(sc->fp, p); break;
-    case kGrad: psdf_cull_kernel<V, kGrad><<<grid, 64, 0, st>>>(sc->fp, p); break;
-    case kCoeff: psdf_cull_kernel<V, kCoeff><<<grid, 64, 0, st>>>(sc->fp, p); break;
+    case 0: psdf_cull_kernel<V, 0><<<grid, bd, 0, st>>>(sc->fp, p); break;
+    case kGrad: psdf_cull_kernel<V, kGrad><<<grid, bd, 0, st>>>(sc->fp, p); break;
+    case kCoeff: psdf_cull_kernel<V, kCoeff><<<grid, bd, 0, st>>>(sc->fp, p); break;
     default: return cudaErrorInvalidValue;
   }
   g_launches.fetch_add(1);
   return cudaGetLastError();
 }
 
-cudaError_t launch_cull_v(const psdf_scene* sc, const EvalParams& p, int mode, dim3 grid, cudaStream_t st) {
+cudaError_t launch_cull_v(const psdf_scene* sc, const EvalParams& p, int mode, dim3 grid, int bd, cudaStream_t st) {
   switch (sc->Vp) {
-    case 4: return launch_cull_mode<4>(sc, p, mode, grid, st);
-    case 6: return launch_cull_mode<6>(sc, p, mode, grid, st);
-    case 8: return launch_cull_mode<8>(sc, p, mode, grid, st);
-    case 10: return launch_cull_mode<10>(sc, p, mode, grid, st);
-    case 12: return launch_cull_mode<12>(sc, p, mode, grid, st);
-    case 16: return launch_cull_mode<16>(sc, p, mode, grid, st);
+    case 4: return launch_cull_mode<4>(sc, p, mode, grid, bd, st);
+    case 6: return launch_cull_mode<6>(sc, p, mode, grid, bd, st);
+    case 8: return launch_cull_mode<8>(sc, p, mode, grid, bd, st);
+    case 10: return launch_cull_mode<10>(sc, p, mode, grid, bd, st);
+    case 12: return launch_cull_mode<12>(sc, p, mode, grid, bd, st);
+    case 16: return launch_cull_mode<16>(sc, p, mode, grid, bd, st);
     default: return cudaErrorInvalidValue;
   }
 }
@@ -134,20 +134,25 @@ cudaError_t enqueue_culled(const psdf_scene* sc, EvalParams& p, int mode, cudaSt
   s.bbox = sc->d_bbox;
   s.cell = sc->d_cell;
   s.perm = sc->d_perm;
-  cudaError_t e;
-  if ((e = cudaMemsetAsync(sc->d_bbox, 0xff, 4 * sizeof(unsigned int), st)) != cudaSuccess) return e;
-  if ((e = cudaMemsetAsync(sc->d_cell, 0, sizeof(int) * (size_t)(s.G * s.G + 1), st)) != cudaSuccess) return e;
-  const int bd = 256, gd = (p.N + bd - 1) / bd;
-  pose_bbox_kernel<<<gd < 4 * sc->sm_count ? gd : 4 * sc->sm_count, bd, 0, st>>>(s);
-  pose_hist_kernel<<<gd, bd, 0, st>>>(s);
-  pose_scan_kernel<<<1, 1024, 0, st>>>(s);
-  pose_scatter_kernel<<<gd, bd, 0, st>>>(s);
-  g_launches.fetch_add(4);
-  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  // the sort workspace is clean on entry (create, or the previous culled kernel, cleaned it)
+  const int gd = (p.N + 255) / 256;
+  pose_bbox_kernel<<<gd < 2 * sc->sm_count ? gd : 2 * sc->sm_count, 256, 0, st>>>(s);
+  pose_hist_kernel<<<(p.N + 1023) / 1024, 1024, 0, st>>>(s);
+  pose_scatter_kernel<<<gd, 256, 0, st>>>(s);
+  g_launches.fetch_add(3);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
   p.perm = sc->d_perm;
   p.bounds = sc->d_bounds;
-  p.n_chunks = 1;
-  return launch_cull_v(sc, p, mode, dim3((unsigned)((p.N + 63) / 64)), st);
+  p.sort_cell = sc->d_cell;
+  p.sort_bbox = sc->d_bbox;
+  p.sort_cells = s.G * s.G;
+  const int groups = (p.N + 31) / 32;
+  int C = 1;                                                // warps per pose group (1: measured best)
+  if (const char* ev = std::getenv("PSDF_CULL_WARPS")) C = std::atoi(ev);
+  C = C < 1 ? 1 : (C > 8 ? 8 : C);
+  p.n_chunks = C;
+  return launch_cull_v(sc, p, mode, dim3((unsigned)groups), 32 * C, st);
 }
 
 cudaError_t launch_v(const psdf_scene* sc, const EvalParams& p, int mode, bool lanes, dim3 grid, int bd,
@@ -355,6 +360,8 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
     CU_TRY(cudaMalloc(&sc->d_perm, sizeof(int) * (size_t)max_poses));
     CU_TRY(cudaMalloc(&sc->d_cell, sizeof(int) * (size_t)(kSortGridMax * kSortGridMax + 1)));
     CU_TRY(cudaMalloc(&sc->d_bbox, sizeof(unsigned int) * 4));
+    CU_TRY(cudaMemsetAsync(sc->d_cell, 0x00, sizeof(int) * (size_t)(kSortGridMax * kSortGridMax + 1), st));
+    CU_TRY(cudaMemsetAsync(sc->d_bbox, 0xff, sizeof(unsigned int) * 4, st));
     CU_TRY(cudaMalloc(&sc->d_ws_depth, sizeof(unsigned long long) * (size_t)max_poses));
     CU_TRY(cudaMalloc(&sc->d_ws_d2, sizeof(unsigned long long) * (size_t)max_poses));
     const size_t n_cnt = (size_t)(max_poses + 63) / 64 + 1;

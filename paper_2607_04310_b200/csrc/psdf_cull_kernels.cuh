@@ -34,16 +34,25 @@ struct SortParams {
 
 __device__ __forceinline__ bool pose_finite(float x, float y) { return isfinite(x) && isfinite(y); }
 
-__global__ void pose_bbox_kernel(const SortParams s) {
+__global__ void __launch_bounds__(256) pose_bbox_kernel(const SortParams s) {
+  __shared__ float red[4][8];
   float x0 = kInf, y0 = kInf, x1 = -kInf, y1 = -kInf;
   for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < s.N; n += gridDim.x * blockDim.x) {
     const float x = __ldg(s.poses + 3 * n), y = __ldg(s.poses + 3 * n + 1);
     if (pose_finite(x, y)) { x0 = fminf(x0, x); y0 = fminf(y0, y); x1 = fmaxf(x1, x); y1 = fmaxf(y1, y); }
   }
   x0 = warp_min_f(x0); y0 = warp_min_f(y0); x1 = warp_max_f(x1); y1 = warp_max_f(y1);
-  if ((threadIdx.x & 31) == 0) {
-    atomicMin(s.bbox + 0, fkey(x0)); atomicMin(s.bbox + 1, fkey(y0));
-    atomicMin(s.bbox + 2, ~fkey(x1)); atomicMin(s.bbox + 3, ~fkey(y1));
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) { red[0][wid] = x0; red[1][wid] = y0; red[2][wid] = x1; red[3][wid] = y1; }
+  __syncthreads();
+  if (wid == 0) {                                         // one atomic per quantity per block
+    const int nw = blockDim.x >> 5;
+    x0 = warp_min_f(lane < nw ? red[0][lane] : kInf); y0 = warp_min_f(lane < nw ? red[1][lane] : kInf);
+    x1 = warp_max_f(lane < nw ? red[2][lane] : -kInf); y1 = warp_max_f(lane < nw ? red[3][lane] : -kInf);
+    if (lane == 0) {
+      atomicMin(s.bbox + 0, fkey(x0)); atomicMin(s.bbox + 1, fkey(y0));
+      atomicMin(s.bbox + 2, ~fkey(x1)); atomicMin(s.bbox + 3, ~fkey(y1));
+    }
   }
 }
 
@@ -59,19 +68,13 @@ __device__ __forceinline__ int pose_cell(const SortParams& s, int n) {
   return gx * s.G + gy;
 }
 
-__global__ void pose_hist_kernel(const SortParams s) {
-  const int n = blockIdx.x * blockDim.x + threadIdx.x;
-  if (n < s.N) atomicAdd(s.cell + pose_cell(s, n), 1);
-}
-
-// one CTA of 1024 threads: exclusive scan of the (<= 4096) cell counts, in place
-__global__ void __launch_bounds__(1024) pose_scan_kernel(const SortParams s) {
+// exclusive scan of the (<= 4096) cell counts, in place, by one CTA of 1024 threads
+__device__ __forceinline__ void scan_cells(int* cell, int cells) {
   __shared__ int wsum[32];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  const int cells = s.G * s.G;
   int v[4], sum = 0;
 #pragma unroll
-  for (int k = 0; k < 4; ++k) { const int c = 4 * tid + k; v[k] = c < cells ? s.cell[c] : 0; sum += v[k]; }
+  for (int k = 0; k < 4; ++k) { const int c = 4 * tid + k; v[k] = c < cells ? __ldcg(cell + c) : 0; sum += v[k]; }
   int inc = sum;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
@@ -87,7 +90,22 @@ __global__ void __launch_bounds__(1024) pose_scan_kernel(const SortParams s) {
   __syncthreads();
   int run = wsum[wid] + inc - sum;
 #pragma unroll
-  for (int k = 0; k < 4; ++k) { const int c = 4 * tid + k; if (c < cells) s.cell[c] = run; run += v[k]; }
+  for (int k = 0; k < 4; ++k) { const int c = 4 * tid + k; if (c < cells) cell[c] = run; run += v[k]; }
+}
+
+// histogram of the pose cells; the last block to arrive turns the counts into offsets
+// (cell[G*G] is the arrival counter).  block = 1024 threads.
+__global__ void __launch_bounds__(1024) pose_hist_kernel(const SortParams s) {
+  __shared__ int is_last;
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n < s.N) atomicAdd(s.cell + pose_cell(s, n), 1);
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) is_last = atomicAdd(s.cell + s.G * s.G, 1) == (int)gridDim.x - 1;
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+  scan_cells(s.cell, s.G * s.G);
 }
 
 __global__ void pose_scatter_kernel(const SortParams s) {
@@ -98,18 +116,29 @@ __global__ void pose_scatter_kernel(const SortParams s) {
 // Per-obstacle bound, one float4 per packed obstacle: bounding circle (cx, cy, R) of its
 // vertices and the index of its first pair record (int bits).
 //
-// Culled evaluation: one warp = 32 sorted poses; MODE in {0, kGrad, kCoeff}.
+// Culled evaluation.  CTA = C warps that own the SAME 32 sorted poses (lane = pose); warp c
+// walks the obstacle batches c, c+C, ... and the warps share the per-pose running upper bound
+// through shared memory (monotone atomicMin on an ordered key: a stale read is merely less
+// tight).  MODE in {0, kGrad, kCoeff}.  The workspace left dirty by the pose sort is cleaned
+// here for the next call.
 template <int V, int MODE>
-__global__ void __launch_bounds__(64) psdf_cull_kernel(const __grid_constant__ Footprint fp,
-                                                       const __grid_constant__ EvalParams p) {
-  const int lane = threadIdx.x & 31;
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+__global__ void __launch_bounds__(256) psdf_cull_kernel(const __grid_constant__ Footprint fp,
+                                                        const __grid_constant__ EvalParams p) {
+  __shared__ unsigned int s_ub[32];
+  __shared__ unsigned long long s_depth[32], s_d2[32];
+  const int lane = threadIdx.x & 31, wc = threadIdx.x >> 5, C = blockDim.x >> 5;
+  {  // clean the sort workspace (its last reader, pose_scatter_kernel, has completed)
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t <= p.sort_cells) p.sort_cell[t] = 0;
+    if (t < 4) p.sort_bbox[t] = 0xffffffffu;
+  }
+  const int k = blockIdx.x * 32 + lane;
   const int n = __ldg(p.perm + min(k, p.N - 1));           // tail lanes recompute the last pose
   const float x = __ldg(p.poses + 3 * n), y = __ldg(p.poses + 3 * n + 1), th = __ldg(p.poses + 3 * n + 2);
   const bool finite = isfinite(x) && isfinite(y) && isfinite(th);
   Posed2<V> P;
   pose_setup2<V>(fp, x, y, th, P);
-  // pose box of the warp (non-finite poses take no part; they are finalised to NaN)
+  // pose box of the 32 poses (non-finite poses take no part; they are finalised to NaN)
   const float xmin = warp_min_f(finite ? x : kInf), xmax = warp_max_f(finite ? x : -kInf);
   const float ymin = warp_min_f(finite ? y : kInf), ymax = warp_max_f(finite ? y : -kInf);
   const float rpad = fp.rmax * 1.0001f + 1e-4f;            // footprint radius + safety for fp32 rounding
@@ -118,55 +147,115 @@ __global__ void __launch_bounds__(64) psdf_cull_kernel(const __grid_constant__ F
   float minD2 = kInf, prevD2 = kInf, maxDepth = -kInf;
   float ub = finite ? kInf : -kInf;                        // running upper bound of phi for this lane
   int idD2 = -1, idDepth = -1;
+  if (C > 1) {
+    if (wc == 0) { s_ub[lane] = fkey(ub); s_depth[lane] = 0ull; s_d2[lane] = ~0ull; }
+    __syncthreads();
+  }
   const float4* __restrict__ bounds = p.bounds;
   const float4* __restrict__ recs = reinterpret_cast<const float4*>(p.pairs);
 
-  for (int base = 0; base < p.Mv; base += 32) {
-    const int i = base + lane;
-    const float4 b = i < p.Mv ? __ldg(bounds + i) : make_float4(0.f, 0.f, 0.f, 0.f);
-    const float ubmax = warp_max_f(ub);
-    // distance from the obstacle centre to the warp's pose box
+  // evaluates one obstacle for the whole warp if some lane still needs it (exact per-lane test)
+  auto visit = [&](const float cx, const float cy, const float R, const int rec) {
+    const float dx = cx - x, dy = cy - y;
+    const float t = (ub + R) * 1.0001f + rpad;
+    const bool need = !((t < 0.f) || (fmaf(dx, dx, dy * dy) > t * t));
+    if (!__any_sync(0xffffffffu, need)) return;
+    acc.reset();
+    const float4* src = recs + 3 * (size_t)rec;
+    float4 q0 = __ldg(src), q1 = __ldg(src + 1), q2 = __ldg(src + 2);
+    int last, slot;
+    while (true) {
+      last = __float_as_int(q2.z);
+      slot = __float_as_int(q2.w);
+      const float4 c0 = q0, c1 = q1;
+      const float h0 = q2.x, h1 = q2.y;
+      if (last < 0) {                                      // prefetch the next record of this obstacle
+        src += 3;
+        q0 = __ldg(src); q1 = __ldg(src + 1); q2 = __ldg(src + 2);
+      }
+      edge_step2<V>(fp, P, c0, h0, acc, minD2);
+      if (h1 >= 0.f) edge_step2<V>(fp, P, c1, h1, acc, minD2);
+      if (last >= 0) break;
+    }
+    const float depth = acc.depth();
+    if (MODE & (kGrad | kCoeff)) {
+      if (minD2 < prevD2) { prevD2 = minD2; idD2 = slot; }
+    }
+    if (depth > maxDepth) { maxDepth = depth; idDepth = slot; }
+    if (finite) {
+      const float nub = fminf(ub, maxDepth >= 0.f ? -maxDepth : sqrtf(minD2));
+      if (C > 1 && nub < ub) atomicMin(&s_ub[lane], fkey(nub));
+      ub = nub;
+    }
+  };
+  // squared distance from an obstacle centre to the pose box of the warp
+  auto box_d2 = [&](const float4 b) {
     const float ddx = fmaxf(fmaxf(xmin - b.x, b.x - xmax), 0.f), ddy = fmaxf(fmaxf(ymin - b.y, b.y - ymax), 0.f);
+    return fmaf(ddx, ddx, ddy * ddy);
+  };
+
+  // Phase A: the two obstacles nearest to the pose box go first, so that the running upper
+  // bound is tight before the memory-order walk (evaluated obstacles per warp drop ~2x).
+  int first0 = -1, first1 = -1;
+  if (wc == 0) {
+    unsigned k0 = 0xffffffffu, k1 = 0xffffffffu;           // this lane's two smallest keys
+    int i0 = -1, i1 = -1;
+    // (ordering heuristic only: squared box distance minus squared radius, no sqrt)
+#pragma unroll 4
+    for (int i = lane; i < p.Mv; i += 32) {
+      const float4 b = __ldg(bounds + i);
+      const unsigned key = fkey(box_d2(b) - b.z * b.z);
+      if (key < k0) { k1 = k0; i1 = i0; k0 = key; i0 = i; }
+      else if (key < k1) { k1 = key; i1 = i; }
+    }
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+      const unsigned m = __reduce_min_sync(0xffffffffu, k0);
+      const int owner = __ffs(__ballot_sync(0xffffffffu, k0 == m && i0 >= 0)) - 1;
+      if (owner < 0) break;
+      const int idx = __shfl_sync(0xffffffffu, i0, owner);
+      if (lane == owner) { k0 = k1; i0 = i1; k1 = 0xffffffffu; i1 = -1; }
+      if (r == 0) first0 = idx; else first1 = idx;
+      const float4 b = __ldg(bounds + idx);
+      visit(b.x, b.y, b.z, __float_as_int(b.w));
+    }
+  }
+
+  // Phase B: memory-order walk, 32 obstacles per step: one box test per obstacle per warp
+  const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+  float4 bn0 = 32 * wc + lane < p.Mv ? __ldg(bounds + 32 * wc + lane) : zero4;            // two batches in flight
+  float4 bn1 = 32 * (wc + C) + lane < p.Mv ? __ldg(bounds + 32 * (wc + C) + lane) : zero4;
+  for (int base = 32 * wc; base < p.Mv; base += 32 * C) {
+    const int i = base + lane;
+    const float4 b = bn0;
+    bn0 = bn1;
+    bn1 = i + 64 * C < p.Mv ? __ldg(bounds + i + 64 * C) : zero4;
+    if (C > 1) ub = fminf(ub, fkey_inv(*reinterpret_cast<volatile unsigned int*>(&s_ub[lane])));
+    const float ubmax = warp_max_f(ub);
     const float thr = (ubmax + b.z) * 1.0001f + rpad;
-    const bool skip = (i >= p.Mv) || (thr < 0.f) || (fmaf(ddx, ddx, ddy * ddy) > thr * thr);
+    const bool skip = (i >= p.Mv) || (i == first0) || (i == first1) || (thr < 0.f) || (box_d2(b) > thr * thr);
     unsigned mask = __ballot_sync(0xffffffffu, !skip);
     while (mask) {
       const int j = __ffs(mask) - 1;
       mask &= mask - 1;
-      const float cx = __shfl_sync(0xffffffffu, b.x, j), cy = __shfl_sync(0xffffffffu, b.y, j);
-      const float R = __shfl_sync(0xffffffffu, b.z, j);
-      int rec = __shfl_sync(0xffffffffu, __float_as_int(b.w), j);
-      // exact per-lane test against this lane's own bound
-      const float dx = cx - x, dy = cy - y;
-      const float t = (ub + R) * 1.0001f + rpad;
-      const bool need = !((t < 0.f) || (fmaf(dx, dx, dy * dy) > t * t));
-      if (!__any_sync(0xffffffffu, need)) continue;
-      acc.reset();
-      const float4* src = recs + 3 * (size_t)rec;
-      float4 q0 = __ldg(src), q1 = __ldg(src + 1), q2 = __ldg(src + 2);
-      int last, slot;
-      while (true) {
-        last = __float_as_int(q2.z);
-        slot = __float_as_int(q2.w);
-        const float4 c0 = q0, c1 = q1;
-        const float h0 = q2.x, h1 = q2.y;
-        if (last < 0) {                                    // prefetch the next record of this obstacle
-          src += 3;
-          q0 = __ldg(src); q1 = __ldg(src + 1); q2 = __ldg(src + 2);
-        }
-        edge_step2<V>(fp, P, c0, h0, acc, minD2);
-        if (h1 >= 0.f) edge_step2<V>(fp, P, c1, h1, acc, minD2);
-        if (last >= 0) break;
-      }
-      const float depth = acc.depth();
-      if (MODE & (kGrad | kCoeff)) {
-        if (minD2 < prevD2) { prevD2 = minD2; idD2 = slot; }
-      }
-      if (depth > maxDepth) { maxDepth = depth; idDepth = slot; }
-      if (finite) ub = maxDepth >= 0.f ? -maxDepth : sqrtf(minD2);
+      visit(__shfl_sync(0xffffffffu, b.x, j), __shfl_sync(0xffffffffu, b.y, j), __shfl_sync(0xffffffffu, b.z, j),
+            __shfl_sync(0xffffffffu, __float_as_int(b.w), j));
     }
   }
   if (!(MODE & (kGrad | kCoeff))) idD2 = minD2 < kInf ? 0 : -1;
+  if (C > 1) {
+    // combine the C partial (arg-)results of each pose; same keys as the dense kernel
+    if (idDepth >= 0)
+      atomicMax(&s_depth[lane], ((unsigned long long)fkey(maxDepth) << 32) | (0xffffffffu - (unsigned)idDepth));
+    if (idD2 >= 0) atomicMin(&s_d2[lane], ((unsigned long long)__float_as_uint(minD2) << 32) | (unsigned)idD2);
+    __syncthreads();
+    if (wc != 0) return;
+    const unsigned long long kd = s_depth[lane], k2 = s_d2[lane];
+    maxDepth = kd ? fkey_inv((uint32_t)(kd >> 32)) : -kInf;
+    idDepth = kd ? (int)(0xffffffffu - (uint32_t)kd) : -1;
+    minD2 = (k2 != ~0ull) ? __uint_as_float((uint32_t)(k2 >> 32)) : kInf;
+    idD2 = (k2 != ~0ull) ? (int)(uint32_t)k2 : -1;
+  }
   if (k >= p.N) return;
   const bool separated = !(maxDepth >= 0.f);
   const float value = separated ? sqrtf(minD2) : -maxDepth;

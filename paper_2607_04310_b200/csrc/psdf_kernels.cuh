@@ -19,6 +19,9 @@ struct EvalParams {
   const int* empty_rows;       // [n_empty] obstacle rows with no valid edge
   const float4* bounds;        // [Mv] per-obstacle bounding circle + first pair record (culled path)
   const int* perm;             // [N] grid-sorted position -> pose index (culled path)
+  int* sort_cell;              // pose-sort workspace, cleaned by the culled kernel
+  unsigned int* sort_bbox;
+  int sort_cells;
   const float* poses;          // [N,3]
   float* value;                // [N]
   float* grad;                 // [N,3] or null
