@@ -79,8 +79,10 @@ psdf_status psdf_eval(psdf_scene* scene, const float* poses, int N, float* value
                       float* per_obstacle, void* cuda_stream);
 
 /* MPC-sized path: same semantics with HOST buffers.  Copies the poses into the scene's
- * pinned staging buffer, replays a captured CUDA graph {H2D, kernel, D2H} on the scene's
- * own stream, synchronises, copies the results out.  grad / per_obstacle may be NULL. */
+ * pinned staging buffer, then either (N <= 512 and <= 64 obstacles) launches ONE kernel that
+ * reads the poses from and writes the results to the pinned, device-mapped staging buffers
+ * directly, or replays a captured CUDA graph {H2D, kernel, D2H}; both on the scene's own
+ * stream; synchronises, copies the results out.  grad / per_obstacle may be NULL. */
 psdf_status psdf_eval_host(psdf_scene* scene, const float* poses, int N, float* value, float* grad,
                            float* per_obstacle);
 

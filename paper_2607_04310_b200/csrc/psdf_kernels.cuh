@@ -27,6 +27,7 @@ struct EvalParams {
   float* grad;                 // [N,3] or null
   float* per_obs;              // [N,M_rows] or null
   float* coeff;                // [N,4] or null (kCoeff)
+  float* packed;               // zero-copy host path: poses are [N,4], results one float4 (value, grad) per pose
   unsigned long long* ws_depth;  // [max_poses] cross-chunk arg-max keys (clean = 0)
   unsigned long long* ws_d2;     // [max_poses] cross-chunk arg-min keys (clean = ~0)
   unsigned int* ws_count;        // [pose tiles] arrival counters (clean = 0)
@@ -60,8 +61,12 @@ __device__ __forceinline__ void finalize_pose(const Footprint& fp, const EvalPar
     witness_gradient<V>(fp, P, p.edges, __ldg(p.row_begin + slot), __ldg(p.row_begin + slot + 1),
                         separated, g);
   }
-  p.value[n] = value;
-  if (MODE & kGrad) {
+  if (p.packed) {                                   // zero-copy staging: one 16-byte store per pose
+    if (!(MODE & kCoeff)) reinterpret_cast<float4*>(p.packed)[n] = make_float4(value, g[0], g[1], g[2]);
+  } else {
+    p.value[n] = value;
+  }
+  if ((MODE & kGrad) && !p.packed) {
     p.grad[3 * n + 0] = g[0];
     p.grad[3 * n + 1] = g[1];
     p.grad[3 * n + 2] = g[2];
@@ -189,7 +194,15 @@ __global__ void __launch_bounds__(128) psdf_lanes_kernel(const __grid_constant__
   const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
   const int n_raw = gtid / K, lane = gtid % K;
   const int n = min(n_raw, p.N - 1);
-  const float x = __ldg(p.poses + 3 * n), y = __ldg(p.poses + 3 * n + 1), th = __ldg(p.poses + 3 * n + 2);
+  float x, y, th;
+  if (p.packed) {
+    // zero-copy staging (host-mapped [N,4] poses): one 16-byte read per pose (L1-cached
+    // within the launch, so the K lanes of a group share one PCIe read)
+    const float4 q = __ldg(reinterpret_cast<const float4*>(p.poses) + n);
+    x = q.x; y = q.y; th = q.z;
+  } else {
+    x = __ldg(p.poses + 3 * n); y = __ldg(p.poses + 3 * n + 1); th = __ldg(p.poses + 3 * n + 2);
+  }
   Posed<V> P;
   pose_setup<V>(fp, x, y, th, P);
   unsigned long long best = ~0ull;
