@@ -101,6 +101,11 @@ psdf_status psdf_mpc_coeffs_host(psdf_scene* scene, const float* poses, int N, f
  * are bit-identical to the dense result.  Default: disabled (dense, branch-free evaluation). */
 psdf_status psdf_set_culling(psdf_scene* scene, int enable);
 
+/* Culled-path statistics accumulated since the last call (then reset): out2[0] = number of
+ * (warp of 32 poses, obstacle) evaluations, out2[1] = number of (warp, obstacle edge) steps.
+ * Synchronises `cuda_stream`.  Used by bench.py for the evaluated-pair fraction and FLOPs. */
+psdf_status psdf_cull_stats(psdf_scene* scene, void* cuda_stream, unsigned long long* out2);
+
 void psdf_destroy_scene(psdf_scene* scene);
 
 /* Introspection (no CUDA work). */

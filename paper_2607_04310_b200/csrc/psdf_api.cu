@@ -63,6 +63,7 @@ struct psdf_scene {
   int* d_perm = nullptr;              // [max_poses]
   int* d_cell = nullptr;              // [kSortGridMax^2 + 1]
   unsigned int* d_bbox = nullptr;     // [4]
+  unsigned long long* d_stats = nullptr;   // [2] psdf_cull_stats
   // host (graph) path
   cudaStream_t gstream = nullptr;
   float* h_in = nullptr;              // pinned [max_poses,3]
@@ -148,6 +149,7 @@ cudaError_t enqueue_culled(const psdf_scene* sc, EvalParams& p, int mode, cudaSt
   p.sort_cell = sc->d_cell;
   p.sort_bbox = sc->d_bbox;
   p.sort_cells = s.G * s.G;
+  p.stats = sc->d_stats;
   const int groups = (p.N + 31) / 32;
   int C = 1;                                                // warps per pose group (1: measured best)
   if (const char* ev = std::getenv("PSDF_CULL_WARPS")) C = std::atoi(ev);
@@ -319,7 +321,7 @@ void psdf_destroy_scene(psdf_scene* sc) {
   if (sc->gstream) cudaStreamDestroy(sc->gstream);
   cudaFree(sc->d_edges); cudaFree(sc->d_pairs); cudaFree(sc->d_row_begin); cudaFree(sc->d_empty);
   cudaFree(sc->d_ws_depth); cudaFree(sc->d_ws_d2); cudaFree(sc->d_ws_count);
-  cudaFree(sc->d_bounds); cudaFree(sc->d_perm); cudaFree(sc->d_cell); cudaFree(sc->d_bbox);
+  cudaFree(sc->d_stats); cudaFree(sc->d_bounds); cudaFree(sc->d_perm); cudaFree(sc->d_cell); cudaFree(sc->d_bbox);
   cudaFree(sc->d_cnt); cudaFree(sc->d_offs); cudaFree(sc->d_pair_begin); cudaFree(sc->d_totals);
   cudaFree(sc->d_in); cudaFree(sc->d_out); cudaFree(sc->d_per);
   if (sc->h_in) cudaFreeHost(sc->h_in);
@@ -362,6 +364,8 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
     CU_TRY(cudaMalloc(&sc->d_perm, sizeof(int) * (size_t)max_poses));
     CU_TRY(cudaMalloc(&sc->d_cell, sizeof(int) * (size_t)(kSortGridMax * kSortGridMax + 1)));
     CU_TRY(cudaMalloc(&sc->d_bbox, sizeof(unsigned int) * 4));
+    CU_TRY(cudaMalloc(&sc->d_stats, sizeof(unsigned long long) * 2));
+    CU_TRY(cudaMemsetAsync(sc->d_stats, 0, sizeof(unsigned long long) * 2, st));
     CU_TRY(cudaMemsetAsync(sc->d_cell, 0x00, sizeof(int) * (size_t)(kSortGridMax * kSortGridMax + 1), st));
     CU_TRY(cudaMemsetAsync(sc->d_bbox, 0xff, sizeof(unsigned int) * 4, st));
     CU_TRY(cudaMalloc(&sc->d_ws_depth, sizeof(unsigned long long) * (size_t)max_poses));
@@ -557,6 +561,15 @@ psdf_status psdf_set_culling(psdf_scene* sc, int enable) {
     if (g.exec) cudaGraphExecDestroy(g.exec);
     g = GraphEntry();
   }
+  return PSDF_OK;
+}
+
+psdf_status psdf_cull_stats(psdf_scene* sc, void* cuda_stream, unsigned long long* out2) {
+  if (!sc || !out2) return PSDF_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CU_TRY(cudaMemcpyAsync(out2, sc->d_stats, sizeof(unsigned long long) * 2, cudaMemcpyDeviceToHost, st));
+  CU_TRY(cudaMemsetAsync(sc->d_stats, 0, sizeof(unsigned long long) * 2, st));
+  CU_TRY(cudaStreamSynchronize(st));
   return PSDF_OK;
 }
 

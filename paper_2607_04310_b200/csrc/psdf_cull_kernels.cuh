@@ -147,6 +147,7 @@ __global__ void __launch_bounds__(256) psdf_cull_kernel(const __grid_constant__ 
   float minD2 = kInf, prevD2 = kInf, maxDepth = -kInf;
   float ub = finite ? kInf : -kInf;                        // running upper bound of phi for this lane
   int idD2 = -1, idDepth = -1;
+  unsigned n_visit = 0, n_edge = 0;                        // statistics (psdf_cull_stats)
   if (C > 1) {
     if (wc == 0) { s_ub[lane] = fkey(ub); s_depth[lane] = 0ull; s_d2[lane] = ~0ull; }
     __syncthreads();
@@ -175,8 +176,10 @@ __global__ void __launch_bounds__(256) psdf_cull_kernel(const __grid_constant__ 
       }
       edge_step2<V>(fp, P, c0, h0, acc, minD2);
       if (h1 >= 0.f) edge_step2<V>(fp, P, c1, h1, acc, minD2);
+      n_edge += h1 >= 0.f ? 2u : 1u;
       if (last >= 0) break;
     }
+    ++n_visit;
     const float depth = acc.depth();
     if (MODE & (kGrad | kCoeff)) {
       if (minD2 < prevD2) { prevD2 = minD2; idD2 = slot; }
@@ -241,6 +244,10 @@ __global__ void __launch_bounds__(256) psdf_cull_kernel(const __grid_constant__ 
       visit(__shfl_sync(0xffffffffu, b.x, j), __shfl_sync(0xffffffffu, b.y, j), __shfl_sync(0xffffffffu, b.z, j),
             __shfl_sync(0xffffffffu, __float_as_int(b.w), j));
     }
+  }
+  if (p.stats && lane == 0) {
+    atomicAdd(p.stats, (unsigned long long)n_visit);
+    atomicAdd(p.stats + 1, (unsigned long long)n_edge);
   }
   if (!(MODE & (kGrad | kCoeff))) idD2 = minD2 < kInf ? 0 : -1;
   if (C > 1) {

@@ -22,6 +22,7 @@ struct EvalParams {
   int* sort_cell;              // pose-sort workspace, cleaned by the culled kernel
   unsigned int* sort_bbox;
   int sort_cells;
+  unsigned long long* stats;   // [2] culled path: (warp x obstacle) visits, (warp x edge) steps; or null
   const float* poses;          // [N,3]
   float* value;                // [N]
   float* grad;                 // [N,3] or null

@@ -24,7 +24,7 @@ PSDF_MEM_HOST = 0
 PSDF_MEM_DEVICE = 1
 
 EXPORTS = ["psdf_create_scene", "psdf_update_scene", "psdf_eval", "psdf_eval_host",
-           "psdf_mpc_coeffs_host", "psdf_set_culling", "psdf_destroy_scene", "psdf_scene_num_obstacles",
+           "psdf_mpc_coeffs_host", "psdf_set_culling", "psdf_cull_stats", "psdf_destroy_scene", "psdf_scene_num_obstacles",
            "psdf_scene_num_edges", "psdf_last_cuda_error", "psdf_kernel_launches",
            "psdf_status_string", "psdf_version", "psdf_measure_fp32_peak"]
 
@@ -62,6 +62,8 @@ def lib():
     L.psdf_mpc_coeffs_host.argtypes = [vp, fp_, i, ctypes.c_float, ctypes.c_float, ctypes.c_float, fp_]
     L.psdf_set_culling.restype = i
     L.psdf_set_culling.argtypes = [vp, i]
+    L.psdf_cull_stats.restype = i
+    L.psdf_cull_stats.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_ulonglong)]
     L.psdf_destroy_scene.restype = None
     L.psdf_destroy_scene.argtypes = [vp]
     L.psdf_scene_num_obstacles.restype = i
@@ -174,6 +176,12 @@ class Scene:
     def set_culling(self, enable: bool):
         """psdf_set_culling: exact broad-phase culling for large batches (default off)."""
         _check(lib().psdf_set_culling(self._h, int(bool(enable))), "psdf_set_culling")
+
+    def cull_stats(self, stream=None):
+        """psdf_cull_stats: (warp x obstacle visits, warp x edge steps) since the last call."""
+        out = (ctypes.c_ulonglong * 2)()
+        _check(lib().psdf_cull_stats(self._h, _stream_ptr(stream), out), "psdf_cull_stats")
+        return int(out[0]), int(out[1])
 
     def update(self, A, B, S, stream=None):
         """psdf_update_scene: same (M,E), values only."""
