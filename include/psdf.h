@@ -86,6 +86,18 @@ psdf_status psdf_eval(psdf_scene* scene, const float* poses, int N, float* value
 psdf_status psdf_eval_host(psdf_scene* scene, const float* poses, int N, float* value, float* grad,
                            float* per_obstacle);
 
+/* Time-varying environments ("batching {(x_{k+s}, E_{k+s})} instead"): the scene
+ * holds the rows of all stage-wise edge sets one after another (e.g. M = H * M_stage rows) and
+ * pose n is evaluated against the obstacle ROWS row_window[2n] <= i < row_window[2n+1] only
+ * (clamped to [0, M]; an empty window gives value=+INF, grad=0).  Same outputs and conventions as
+ * psdf_eval; row_window is a device [N,2] int32 array (host array for the _host variant, which
+ * copies, evaluates on the scene's stream and synchronises).  Meant for MPC-sized batches: one
+ * group of lanes per pose, any N <= max_poses. */
+psdf_status psdf_eval_windows(psdf_scene* scene, const float* poses, int N, const int* row_window, float* value,
+                              float* grad, void* cuda_stream);
+psdf_status psdf_eval_windows_host(psdf_scene* scene, const float* poses, int N, const int* row_window,
+                                   float* value, float* grad);
+
 /* MPC coefficient epilogue (Alg.1 l.7-11; eqs.(26)-(28)):
  * for each stage s writes coeff[s] = [ h_s - gamma_s ; J_g,s ] with h_s = phi_s - d_min,
  * J_g,s = -grad phi_s, gamma_s = 0.5 (r_max + phi_s) rho_theta^2 + rho_p rho_theta,

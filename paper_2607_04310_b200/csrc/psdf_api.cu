@@ -48,6 +48,9 @@ struct psdf_scene {
   EdgeRec* d_edges = nullptr;
   PairRec* d_pairs = nullptr;
   int* d_row_begin = nullptr;
+  int* d_row_slot = nullptr;          // [M+1]
+  int* h_win = nullptr;               // pinned [max_poses,2]  (psdf_eval_windows_host)
+  int* d_win = nullptr;
   int* d_empty = nullptr;
   unsigned long long* d_ws_depth = nullptr;
   unsigned long long* d_ws_d2 = nullptr;
@@ -176,12 +179,14 @@ cudaError_t launch_v(const psdf_scene* sc, const EvalParams& p, int mode, bool l
 // would not fill 148 SMs several times over.
 psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float* value, float* grad,
                          float* per_obs, float* coeff, float d_min, float rho_p, float rho_theta,
-                         cudaStream_t st, float* packed = nullptr) {
+                         cudaStream_t st, float* packed = nullptr, const int* window = nullptr) {
   if (N == 0) return PSDF_OK;
   EvalParams p{};
   p.edges = sc->d_edges;
   p.pairs = sc->d_pairs;
   p.row_begin = sc->d_row_begin;
+  p.row_slot = sc->d_row_slot;
+  p.window = window;
   p.empty_rows = sc->d_empty;
   p.poses = poses;
   p.value = value;
@@ -203,7 +208,7 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
   const int mode = coeff ? kCoeff : ((grad ? kGrad : 0) | (per_obs ? kPerObs : 0));
 
   const long long pairs = (long long)N * (sc->Mv > 0 ? sc->Mv : 1);
-  const bool lanes = N <= 2048 || pairs <= (1 << 16);
+  const bool lanes = N <= 2048 || pairs <= (1 << 16) || window != nullptr;
   dim3 grid;
   int bd;
   if (sc->culling && !lanes && !per_obs && sc->Mv >= 64) {
@@ -272,7 +277,7 @@ psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const
   CU_TRY(cudaGetLastError());
   if (t.status != 0) return PSDF_ERR_DEGENERATE;          // nothing live has been touched yet
   pack_write_kernel<<<gd, bd, 0, st>>>(A, B, S, M, E, sc->d_cnt, sc->d_offs, sc->d_totals, sc->d_edges, sc->d_pairs,
-                                       sc->d_row_begin, sc->d_pair_begin, sc->d_empty, sc->d_bounds);
+                                       sc->d_row_begin, sc->d_pair_begin, sc->d_empty, sc->d_bounds, sc->d_row_slot);
   g_launches.fetch_add(1);
   sc->h_pair_begin.resize((size_t)t.Mv + 1);
   CU_TRY(cudaMemcpyAsync(sc->h_pair_begin.data(), sc->d_pair_begin, sizeof(int) * ((size_t)t.Mv + 1),
@@ -300,6 +305,7 @@ psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const u
     CU_TRY(cudaMemcpyAsync(sc->d_edges, ps.edges.data(), sizeof(EdgeRec) * sc->n_edges, cudaMemcpyHostToDevice, st));
     CU_TRY(cudaMemcpyAsync(sc->d_pairs, ps.pairs.data(), sizeof(PairRec) * sc->n_pairs, cudaMemcpyHostToDevice, st));
   }
+  CU_TRY(cudaMemcpyAsync(sc->d_row_slot, ps.row_slot.data(), sizeof(int) * (size_t)(sc->M + 1), cudaMemcpyHostToDevice, st));
   if (sc->Mv)
     CU_TRY(cudaMemcpyAsync(sc->d_bounds, ps.bounds.data(), sizeof(float4) * sc->Mv, cudaMemcpyHostToDevice, st));
   CU_TRY(cudaMemcpyAsync(sc->d_row_begin, ps.row_begin.data(), sizeof(int) * (sc->Mv + 1), cudaMemcpyHostToDevice, st));
@@ -320,6 +326,8 @@ void psdf_destroy_scene(psdf_scene* sc) {
     if (g.exec) cudaGraphExecDestroy(g.exec);
   if (sc->gstream) cudaStreamDestroy(sc->gstream);
   cudaFree(sc->d_edges); cudaFree(sc->d_pairs); cudaFree(sc->d_row_begin); cudaFree(sc->d_empty);
+  cudaFree(sc->d_row_slot); cudaFree(sc->d_win);
+  if (sc->h_win) cudaFreeHost(sc->h_win);
   cudaFree(sc->d_ws_depth); cudaFree(sc->d_ws_d2); cudaFree(sc->d_ws_count);
   cudaFree(sc->d_stats); cudaFree(sc->d_bounds); cudaFree(sc->d_perm); cudaFree(sc->d_cell); cudaFree(sc->d_bbox);
   cudaFree(sc->d_cnt); cudaFree(sc->d_offs); cudaFree(sc->d_pair_begin); cudaFree(sc->d_totals);
@@ -355,6 +363,7 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
     CU_TRY(cudaMalloc(&sc->d_edges, sizeof(EdgeRec) * (size_t)sc->edge_cap));
     CU_TRY(cudaMalloc(&sc->d_pairs, sizeof(PairRec) * (size_t)(sc->edge_cap / 2 + M)));
     CU_TRY(cudaMalloc(&sc->d_row_begin, sizeof(int) * (size_t)(M + 1)));
+    CU_TRY(cudaMalloc(&sc->d_row_slot, sizeof(int) * (size_t)(M + 1)));
     CU_TRY(cudaMalloc(&sc->d_empty, sizeof(int) * (size_t)M));
     CU_TRY(cudaMalloc(&sc->d_cnt, sizeof(int) * (size_t)M));
     CU_TRY(cudaMalloc(&sc->d_offs, sizeof(int4) * (size_t)M));
@@ -536,6 +545,40 @@ psdf_status psdf_eval_host(psdf_scene* sc, const float* poses, int N, float* val
     if (grad) std::memcpy(grad, sc->h_out + N, sizeof(float) * 3 * (size_t)N);
   }
   if (per_obstacle) std::memcpy(per_obstacle, sc->h_per, sizeof(float) * (size_t)N * sc->M);
+  return PSDF_OK;
+}
+
+psdf_status psdf_eval_windows(psdf_scene* sc, const float* poses, int N, const int* row_window, float* value,
+                              float* grad, void* cuda_stream) {
+  if (!sc || N < 0 || (N > 0 && (!poses || !value || !row_window))) return PSDF_ERR_INVALID_ARG;
+  if (N > sc->max_poses) return PSDF_ERR_CAPACITY;
+  return enqueue_eval(sc, poses, N, value, grad, nullptr, nullptr, 0.f, 0.f, 0.f, (cudaStream_t)cuda_stream, nullptr,
+                      row_window);
+}
+
+psdf_status psdf_eval_windows_host(psdf_scene* sc, const float* poses, int N, const int* row_window, float* value,
+                                   float* grad) {
+  if (!sc || N < 0 || (N > 0 && (!poses || !value || !row_window))) return PSDF_ERR_INVALID_ARG;
+  if (N > sc->max_poses) return PSDF_ERR_CAPACITY;
+  if (N == 0) return PSDF_OK;
+  psdf_status s = ensure_host_path(sc, false);
+  if (s != PSDF_OK) return s;
+  if (!sc->h_win) {
+    CU_TRY(cudaMallocHost(&sc->h_win, sizeof(int) * 2 * (size_t)sc->max_poses));
+    CU_TRY(cudaMalloc(&sc->d_win, sizeof(int) * 2 * (size_t)sc->max_poses));
+  }
+  std::memcpy(sc->h_in, poses, sizeof(float) * 3 * (size_t)N);
+  std::memcpy(sc->h_win, row_window, sizeof(int) * 2 * (size_t)N);
+  cudaStream_t st = sc->gstream;
+  CU_TRY(cudaMemcpyAsync(sc->d_in, sc->h_in, sizeof(float) * 3 * (size_t)N, cudaMemcpyHostToDevice, st));
+  CU_TRY(cudaMemcpyAsync(sc->d_win, sc->h_win, sizeof(int) * 2 * (size_t)N, cudaMemcpyHostToDevice, st));
+  s = enqueue_eval(sc, sc->d_in, N, sc->d_out, grad ? sc->d_out + N : nullptr, nullptr, nullptr, 0.f, 0.f, 0.f, st,
+                   nullptr, sc->d_win);
+  if (s != PSDF_OK) return s;
+  CU_TRY(cudaMemcpyAsync(sc->h_out, sc->d_out, sizeof(float) * (grad ? 4 : 1) * (size_t)N, cudaMemcpyDeviceToHost, st));
+  CU_TRY(cudaStreamSynchronize(st));
+  std::memcpy(value, sc->h_out, sizeof(float) * (size_t)N);
+  if (grad) std::memcpy(grad, sc->h_out + N, sizeof(float) * 3 * (size_t)N);
   return PSDF_OK;
 }
 

@@ -17,6 +17,8 @@ struct EvalParams {
   const PairRec* pairs;        // [n_pairs] the same edges two per record (tile-scan kernel)
   const int* row_begin;        // [Mv+1] packed obstacle -> first edge
   const int* empty_rows;       // [n_empty] obstacle rows with no valid edge
+  const int* row_slot;         // [M_rows+1] number of non-empty rows before each row (row -> packed slot)
+  const int* window;           // [N,2] per-pose obstacle ROW window [begin, end), or null = all rows
   const float4* bounds;        // [Mv] per-obstacle bounding circle + first pair record (culled path)
   const int* perm;             // [N] grid-sorted position -> pose index (culled path)
   int* sort_cell;              // pose-sort workspace, cleaned by the culled kernel
@@ -208,7 +210,15 @@ __global__ void __launch_bounds__(128) psdf_lanes_kernel(const __grid_constant__
   pose_setup<V>(fp, x, y, th, P);
   unsigned long long best = ~0ull;
   ObstacleAcc<V> acc;
-  for (int slot = lane; slot < p.Mv; slot += K) {
+  // per-pose obstacle window (time-varying environments: pose s sees the rows of E_{k+s},
+  // PAPER.md:293); rows outside [0, M_rows] are clamped, an empty window gives +inf
+  int s_begin = 0, s_end = p.Mv;
+  if (p.window) {
+    const int w0 = min(max(p.window[2 * n], 0), p.M_rows), w1 = min(max(p.window[2 * n + 1], w0), p.M_rows);
+    s_begin = __ldg(p.row_slot + w0);
+    s_end = __ldg(p.row_slot + w1);
+  }
+  for (int slot = s_begin + lane; slot < s_end; slot += K) {
     const int eb = __ldg(p.row_begin + slot), ee = __ldg(p.row_begin + slot + 1);
     acc.reset();
     float d2 = kInf;

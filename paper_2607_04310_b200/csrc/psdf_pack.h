@@ -18,6 +18,7 @@ struct PackedScene {
   std::vector<int> pair_begin;    // [Mv+1]
   std::vector<int> empty_rows;
   std::vector<float4> bounds;     // [Mv] bounding circle + first pair record per obstacle
+  std::vector<int> row_slot;      // [M+1] non-empty rows before each row
 };
 
 // Double-precision helpers that round identically on host and device: nvcc contracts a*b+c
@@ -149,10 +150,12 @@ inline int pack_scene(const float* A, const float* B, const uint8_t* S, int M, i
   out.pair_begin.assign(1, 0);
   out.empty_rows.clear();
   out.bounds.clear();
+  out.row_slot.assign((size_t)M + 1, 0);
   std::vector<EdgeRec> tmp((size_t)E);
   for (int i = 0; i < M; ++i) {
     int e = 0;
     const int slot = (int)out.row_begin.size() - 1;
+    out.row_slot[i] = slot;
     if (pack_row(A + (size_t)i * E * 2, B + (size_t)i * E * 2, S + (size_t)i * E, E, i, slot, tmp.data(), &e) != 0)
       return -2;
     if (e == 0) { out.empty_rows.push_back(i); continue; }
@@ -162,6 +165,7 @@ inline int pack_scene(const float* A, const float* B, const uint8_t* S, int M, i
     out.row_begin.push_back((int)out.edges.size());
     out.pair_begin.push_back((int)out.pairs.size());
   }
+  out.row_slot[M] = (int)out.row_begin.size() - 1;
   return 0;
 }
 

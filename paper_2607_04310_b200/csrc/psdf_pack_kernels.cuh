@@ -89,14 +89,17 @@ __global__ void pack_write_kernel(const float* __restrict__ A, const float* __re
                                   const int4* __restrict__ offs, const PackTotals* __restrict__ totals,
                                   EdgeRec* __restrict__ edges, PairRec* __restrict__ pairs,
                                   int* __restrict__ row_begin, int* __restrict__ pair_begin,
-                                  int* __restrict__ empty_rows, float4* __restrict__ bounds) {
+                                  int* __restrict__ empty_rows, float4* __restrict__ bounds,
+                                  int* __restrict__ row_slot) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i == 0) {
     row_begin[totals->Mv] = totals->n_edges;
     pair_begin[totals->Mv] = totals->n_pairs;
+    row_slot[M] = totals->Mv;
   }
   if (i >= M) return;
   const int4 o = offs[i];
+  row_slot[i] = o.x;
   int e = count[i];
   if (e == 0) { empty_rows[o.w] = i; return; }
   EdgeRec* er = edges + o.y;

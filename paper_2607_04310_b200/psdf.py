@@ -24,7 +24,7 @@ PSDF_MEM_HOST = 0
 PSDF_MEM_DEVICE = 1
 
 EXPORTS = ["psdf_create_scene", "psdf_update_scene", "psdf_eval", "psdf_eval_host",
-           "psdf_mpc_coeffs_host", "psdf_set_culling", "psdf_cull_stats", "psdf_destroy_scene", "psdf_scene_num_obstacles",
+           "psdf_eval_windows", "psdf_eval_windows_host", "psdf_mpc_coeffs_host", "psdf_set_culling", "psdf_cull_stats", "psdf_destroy_scene", "psdf_scene_num_obstacles",
            "psdf_scene_num_edges", "psdf_last_cuda_error", "psdf_kernel_launches",
            "psdf_status_string", "psdf_version", "psdf_measure_fp32_peak"]
 
@@ -58,6 +58,10 @@ def lib():
     L.psdf_eval.argtypes = [vp, fp_, i, fp_, fp_, fp_, vp]
     L.psdf_eval_host.restype = i
     L.psdf_eval_host.argtypes = [vp, fp_, i, fp_, fp_, fp_]
+    L.psdf_eval_windows.restype = i
+    L.psdf_eval_windows.argtypes = [vp, fp_, i, vp, fp_, fp_, vp]
+    L.psdf_eval_windows_host.restype = i
+    L.psdf_eval_windows_host.argtypes = [vp, fp_, i, vp, fp_, fp_]
     L.psdf_mpc_coeffs_host.restype = i
     L.psdf_mpc_coeffs_host.argtypes = [vp, fp_, i, ctypes.c_float, ctypes.c_float, ctypes.c_float, fp_]
     L.psdf_set_culling.restype = i
@@ -227,6 +231,29 @@ class Scene:
                                     po.ctypes.data if po is not None else None), "psdf_eval_host")
         return value, g, po
 
+    def eval_windows(self, poses, row_window, grad=True, stream=None):
+        """psdf_eval_windows: device poses [N,3] float32 and row windows [N,2] int32."""
+        import torch
+        N = int(poses.shape[0])
+        value = torch.empty(N, dtype=torch.float32, device=poses.device)
+        g = torch.empty((N, 3), dtype=torch.float32, device=poses.device) if grad else None
+        _check(lib().psdf_eval_windows(self._h, _dev_ptr(poses, "float32"), N, _dev_ptr(row_window, "int32"),
+                                       _dev_ptr(value, "float32"), _dev_ptr(g, "float32") if grad else None,
+                                       _stream_ptr(stream)), "psdf_eval_windows")
+        return value, g
+
+    def eval_windows_host(self, poses, row_window, grad=True):
+        """psdf_eval_windows_host on numpy arrays."""
+        poses, pp = _host(poses, np.float32)
+        win, pw = _host(row_window, np.int32)
+        N = int(poses.shape[0])
+        assert win.shape == (N, 2)
+        value = np.empty(N, np.float32)
+        g = np.empty((N, 3), np.float32) if grad else None
+        _check(lib().psdf_eval_windows_host(self._h, pp, N, pw, value.ctypes.data,
+                                            g.ctypes.data if grad else None), "psdf_eval_windows_host")
+        return value, g
+
     def eval_host_into(self, poses, value, grad=None, per_obstacle=None):
         """psdf_eval_host into caller-owned contiguous float32 numpy arrays (no allocation in
         the binding: the call an MPC loop makes every control cycle)."""
@@ -257,6 +284,14 @@ def psdf_eval(scene: Scene, poses, **kw):
 
 def psdf_eval_host(scene: Scene, poses, **kw):
     return scene.eval_host(poses, **kw)
+
+
+def psdf_eval_windows(scene: Scene, poses, row_window, **kw):
+    return scene.eval_windows(poses, row_window, **kw)
+
+
+def psdf_eval_windows_host(scene: Scene, poses, row_window, **kw):
+    return scene.eval_windows_host(poses, row_window, **kw)
 
 
 def psdf_update_scene(scene: Scene, A, B, S, stream=None):

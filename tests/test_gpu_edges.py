@@ -221,3 +221,50 @@ def test_device_encode_edges(env):
                 assert np.array_equal(x, y)
         host.close()
         dev.close()
+
+
+def test_time_varying_row_windows(env):
+    """Per-stage edge sets E_{k+s}: the scene holds H stage-wise obstacle sets,
+    pose s is evaluated against its own stage's rows only; oracle = one evaluation per stage."""
+    torch, O, psdf, W = env
+    rng = np.random.default_rng(321)
+    base = W.table1_case(12, 1, seed=777)
+    H, Ms, E = 15, base.M, base.E
+    vel = rng.uniform(-1.0, 1.0, (Ms, 1, 2)).astype(np.float32)
+    A = np.concatenate([(base.A + vel * np.float32(0.1 * s)).astype(np.float32) for s in range(H)])
+    B = A.copy()
+    S = np.concatenate([base.S] * H)
+    for i in range(H * Ms):
+        sl = np.nonzero(S[i])[0]
+        B[i, sl] = A[i, np.roll(sl, -1)]
+    n_per = 9
+    poses = np.stack([rng.uniform(0, 20, H * n_per), rng.uniform(0, 20, H * n_per),
+                      rng.uniform(-3.2, 3.2, H * n_per)], 1).astype(np.float32)
+    stage = np.repeat(np.arange(H), n_per)
+    win = np.stack([stage * Ms, (stage + 1) * Ms], 1).astype(np.int32)
+    for device_scene in (False, True):
+        if device_scene:
+            scene = psdf.Scene(base.footprint, torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(),
+                               torch.from_numpy(S).cuda(), max_poses=len(poses))
+        else:
+            scene = psdf.Scene(base.footprint, A, B, S, max_poses=len(poses))
+        v, g = scene.eval_windows(torch.from_numpy(poses).cuda(), torch.from_numpy(win).cuda())
+        torch.cuda.synchronize()
+        v, g = v.cpu().numpy(), g.cpu().numpy()
+        vh, gh = scene.eval_windows_host(poses, win)
+        assert np.array_equal(v, vh) and np.array_equal(g, gh)
+        for s in range(H):
+            rows = slice(s * Ms, (s + 1) * Ms)
+            ref = O.evaluate(base.footprint, A[rows], B[rows], S[rows], poses[stage == s])
+            compare(ref, v[stage == s], g[stage == s], what=f"stage {s}")
+        # full window == plain evaluation; clamped and empty windows
+        full = np.tile(np.array([[-5, 10 ** 6]], np.int32), (len(poses), 1))
+        vf, gf = scene.eval_windows_host(poses, full)
+        v0, g0, _ = scene.eval_host(poses)
+        assert np.array_equal(vf, v0) and np.array_equal(gf, g0)
+        empty = np.tile(np.array([[7, 7]], np.int32), (len(poses), 1))
+        ve, ge = scene.eval_windows_host(poses, empty)
+        assert np.isposinf(ve).all() and (ge == 0).all()
+        vv, gn = scene.eval_windows_host(poses, win, grad=False)
+        assert gn is None and np.array_equal(vv, v)
+        scene.close()
