@@ -113,6 +113,21 @@ psdf_status psdf_mpc_coeffs_host(psdf_scene* scene, const float* poses, int N, f
  * are bit-identical to the dense result.  Default: disabled (dense, branch-free evaluation). */
 psdf_status psdf_set_culling(psdf_scene* scene, int enable);
 
+/* Non-convex obstacles given as convex components (Assumption 1; eq.(6),
+ * PAPER.md:93-97): folds the per-component values of psdf_eval's `per_obstacle` output,
+ * per_component device [N,M], into out device [N,n_obstacles] with
+ * out[n,o] = min over rows i with comp_to_obstacle[i] == o (+INF if none); comp_to_obstacle is a
+ * device [M] int32 array, ids outside [0,n_obstacles) are ignored.  Asynchronous on the stream. */
+psdf_status psdf_component_min(const float* per_component, int N, int M, const int* comp_to_obstacle,
+                               int n_obstacles, float* out, void* cuda_stream);
+
+/* Sampled-trajectory batches (pose index = trajectory * H + stage): per trajectory the clearance
+ * min_value[t] = min_s phi, its first arg-min stage, and the soft penalty
+ * penalty[t] = sum_s max(0, d_safe - phi_s)^2 (fixed summation order: deterministic).  value is
+ * psdf_eval's device [T*H] output; any of the three device outputs may be NULL. */
+psdf_status psdf_trajectory_reduce(const float* value, int T, int H, float d_safe, float* min_value,
+                                   int* argmin_stage, float* penalty, void* cuda_stream);
+
 /* Culled-path statistics accumulated since the last call (then reset): out2[0] = number of
  * (warp of 32 poses, obstacle) evaluations, out2[1] = number of (warp, obstacle edge) steps.
  * Synchronises `cuda_stream`.  Used by bench.py for the evaluated-pair fraction and FLOPs. */

@@ -89,3 +89,25 @@ def evaluate_value_only(footprint, A, B, S, poses, nthreads=0) -> np.ndarray:
     if rc != 0:
         raise ValueError("psdf_oracle_eval: bad arguments")
     return value
+
+
+def component_min(per_component: np.ndarray, comp_to_obstacle, n_obstacles: int) -> np.ndarray:
+    """Non-convex obstacles as unions of convex components (Assumption 1): the
+    signed distance to obstacle o is the minimum over its components (eq.(6), PAPER.md:93-97,
+    restricted to the components of o).  Plain definition, float64; +inf where o has none."""
+    pc = np.asarray(per_component, np.float64)
+    ids = np.asarray(comp_to_obstacle)
+    out = np.full((pc.shape[0], int(n_obstacles)), np.inf)
+    for o in range(int(n_obstacles)):
+        cols = np.nonzero(ids == o)[0]
+        if cols.size:
+            out[:, o] = pc[:, cols].min(axis=1)
+    return out
+
+
+def trajectory_reduce(value: np.ndarray, T: int, H: int, d_safe: float):
+    """Sampled-trajectory reductions (pose index = trajectory * H + stage): clearance
+    min_s phi_s, its first arg-min stage, soft penalty sum_s max(0, d_safe - phi_s)^2.
+    Plain definitions in float64."""
+    v = np.asarray(value, np.float64).reshape(int(T), int(H))
+    return v.min(axis=1), v.argmin(axis=1), (np.maximum(float(d_safe) - v, 0.0) ** 2).sum(axis=1)

@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpsdf.so")
 SOURCES = ["psdf_api.cu"]
-DEPS = ["psdf_api.cu", "psdf_kernels.cuh", "psdf_device.cuh", "psdf_pack.h", "psdf_pack_kernels.cuh", "psdf_cull_kernels.cuh", "../../include/psdf.h"]
+DEPS = ["psdf_api.cu", "psdf_kernels.cuh", "psdf_device.cuh", "psdf_pack.h", "psdf_pack_kernels.cuh", "psdf_cull_kernels.cuh", "psdf_reduce_kernels.cuh", "../../include/psdf.h"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xptxas=-v", "-Xcompiler", "-fPIC", "-shared",

@@ -9,6 +9,7 @@
 #include "psdf_cull_kernels.cuh"
 #include "psdf_pack.h"
 #include "psdf_pack_kernels.cuh"
+#include "psdf_reduce_kernels.cuh"
 
 using namespace psdf;
 
@@ -604,6 +605,30 @@ psdf_status psdf_set_culling(psdf_scene* sc, int enable) {
     if (g.exec) cudaGraphExecDestroy(g.exec);
     g = GraphEntry();
   }
+  return PSDF_OK;
+}
+
+psdf_status psdf_component_min(const float* per_component, int N, int M, const int* comp_to_obstacle,
+                               int n_obstacles, float* out, void* cuda_stream) {
+  if (N < 0 || M < 1 || n_obstacles < 1 || (N > 0 && (!per_component || !comp_to_obstacle || !out)))
+    return PSDF_ERR_INVALID_ARG;
+  if (N == 0) return PSDF_OK;
+  const long long total = (long long)N * n_obstacles;
+  component_min_kernel<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(
+      per_component, N, M, comp_to_obstacle, n_obstacles, out);
+  g_launches.fetch_add(1);
+  CU_TRY(cudaGetLastError());
+  return PSDF_OK;
+}
+
+psdf_status psdf_trajectory_reduce(const float* value, int T, int H, float d_safe, float* min_value,
+                                   int* argmin_stage, float* penalty, void* cuda_stream) {
+  if (T < 0 || H < 1 || (T > 0 && !value)) return PSDF_ERR_INVALID_ARG;
+  if (T == 0) return PSDF_OK;
+  trajectory_reduce_kernel<<<(unsigned)((T + 3) / 4), 128, 0, (cudaStream_t)cuda_stream>>>(value, T, H, d_safe, min_value,
+                                                                                          argmin_stage, penalty);
+  g_launches.fetch_add(1);
+  CU_TRY(cudaGetLastError());
   return PSDF_OK;
 }
 

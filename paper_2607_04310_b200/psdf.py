@@ -24,7 +24,7 @@ PSDF_MEM_HOST = 0
 PSDF_MEM_DEVICE = 1
 
 EXPORTS = ["psdf_create_scene", "psdf_update_scene", "psdf_eval", "psdf_eval_host",
-           "psdf_eval_windows", "psdf_eval_windows_host", "psdf_mpc_coeffs_host", "psdf_set_culling", "psdf_cull_stats", "psdf_destroy_scene", "psdf_scene_num_obstacles",
+           "psdf_eval_windows", "psdf_eval_windows_host", "psdf_mpc_coeffs_host", "psdf_component_min", "psdf_trajectory_reduce", "psdf_set_culling", "psdf_cull_stats", "psdf_destroy_scene", "psdf_scene_num_obstacles",
            "psdf_scene_num_edges", "psdf_last_cuda_error", "psdf_kernel_launches",
            "psdf_status_string", "psdf_version", "psdf_measure_fp32_peak"]
 
@@ -66,6 +66,10 @@ def lib():
     L.psdf_mpc_coeffs_host.argtypes = [vp, fp_, i, ctypes.c_float, ctypes.c_float, ctypes.c_float, fp_]
     L.psdf_set_culling.restype = i
     L.psdf_set_culling.argtypes = [vp, i]
+    L.psdf_component_min.restype = i
+    L.psdf_component_min.argtypes = [fp_, i, i, vp, i, fp_, vp]
+    L.psdf_trajectory_reduce.restype = i
+    L.psdf_trajectory_reduce.argtypes = [fp_, i, i, ctypes.c_float, fp_, vp, fp_, vp]
     L.psdf_cull_stats.restype = i
     L.psdf_cull_stats.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_ulonglong)]
     L.psdf_destroy_scene.restype = None
@@ -300,6 +304,30 @@ def psdf_update_scene(scene: Scene, A, B, S, stream=None):
 
 def psdf_mpc_coeffs_host(scene: Scene, poses, d_min, rho_p, rho_theta):
     return scene.mpc_coeffs_host(poses, d_min, rho_p, rho_theta)
+
+
+def psdf_component_min(per_component, comp_to_obstacle, n_obstacles, stream=None):
+    """per_component: CUDA float32 [N,M]; comp_to_obstacle: CUDA int32 [M] -> float32 [N,n_obstacles]."""
+    import torch
+    N, M = int(per_component.shape[0]), int(per_component.shape[1])
+    out = torch.empty((N, int(n_obstacles)), dtype=torch.float32, device=per_component.device)
+    _check(lib().psdf_component_min(_dev_ptr(per_component, "float32"), N, M, _dev_ptr(comp_to_obstacle, "int32"),
+                                    int(n_obstacles), _dev_ptr(out, "float32"), _stream_ptr(stream)),
+           "psdf_component_min")
+    return out
+
+
+def psdf_trajectory_reduce(value, T, H, d_safe, stream=None):
+    """value: CUDA float32 [T*H] -> (min_value[T], argmin_stage[T] int32, penalty[T])."""
+    import torch
+    assert value.numel() == int(T) * int(H)
+    mn = torch.empty(int(T), dtype=torch.float32, device=value.device)
+    am = torch.empty(int(T), dtype=torch.int32, device=value.device)
+    pen = torch.empty(int(T), dtype=torch.float32, device=value.device)
+    _check(lib().psdf_trajectory_reduce(_dev_ptr(value, "float32"), int(T), int(H), float(d_safe),
+                                        _dev_ptr(mn, "float32"), _dev_ptr(am, "int32"), _dev_ptr(pen, "float32"),
+                                        _stream_ptr(stream)), "psdf_trajectory_reduce")
+    return mn, am, pen
 
 
 def psdf_set_culling(scene: Scene, enable: bool):

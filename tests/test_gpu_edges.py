@@ -268,3 +268,45 @@ def test_time_varying_row_windows(env):
         vv, gn = scene.eval_windows_host(poses, win, grad=False)
         assert gn is None and np.array_equal(vv, v)
         scene.close()
+
+
+def test_component_min_and_trajectory_reduce(env):
+    """NEXT-4 reductions through the C ABI vs the oracle's plain definitions."""
+    torch, O, psdf, W = env
+    rng = np.random.default_rng(55)
+    # non-convex obstacles: config-2 rows grouped 3 at a time into 22 obstacles (last group smaller)
+    w = W.make_config(2)
+    ids = (np.arange(w.M) // 3).astype(np.int32)
+    ids[5] = 99                                                    # an id outside the range is ignored
+    n_obs = int(np.ceil(w.M / 3)) + 1                              # plus one obstacle without components
+    scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=w.N)
+    v, g, po = scene.eval(torch.from_numpy(w.poses).cuda(), grad=True, per_obstacle=True)
+    out = psdf.psdf_component_min(po, torch.from_numpy(ids).cuda(), n_obs)
+    torch.cuda.synchronize()
+    ref = O.evaluate(w.footprint, w.A, w.B, w.S, w.poses, per_obstacle=True)
+    want = O.component_min(ref.per_obstacle, ids, n_obs)
+    got = out.cpu().numpy().astype(np.float64)
+    assert np.array_equal(np.isposinf(got), np.isposinf(want)) and np.isposinf(got[:, -1]).all()
+    fin = np.isfinite(want)
+    assert np.abs(got[fin] - want[fin]).max() <= 1e-5
+    assert np.array_equal(got, O.component_min(po.cpu().numpy(), ids, n_obs))   # exact fold of the GPU's own values
+    scene.close()
+    # sampled trajectories: config-3-like batch, T x H with H not a multiple of 32
+    w = W.make_config(3, n_traj=300)
+    T, H = 300, w.N // 300
+    scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=w.N)
+    v, _, _ = scene.eval(torch.from_numpy(w.poses).cuda(), grad=False)
+    d_safe = 0.5
+    mn, am, pen = psdf.psdf_trajectory_reduce(v, T, H, d_safe)
+    torch.cuda.synchronize()
+    vh = v.cpu().numpy()
+    rmn, ram, rpen = O.trajectory_reduce(vh, T, H, d_safe)         # definitions on the same fp32 values
+    assert np.array_equal(mn.cpu().numpy().astype(np.float64), rmn)
+    assert np.array_equal(am.cpu().numpy(), ram)
+    assert np.abs(pen.cpu().numpy() - rpen).max() <= 1e-5 * max(1.0, rpen.max())
+    ref = O.evaluate(w.footprint, w.A, w.B, w.S, w.poses)
+    omn, _, open_ = O.trajectory_reduce(ref.value, T, H, d_safe)   # and against the oracle end to end
+    assert np.abs(mn.cpu().numpy() - omn).max() <= 1e-5
+    assert np.abs(pen.cpu().numpy() - open_).max() <= 1e-4 * max(1.0, open_.max())
+    assert (rpen > 0).any()
+    scene.close()

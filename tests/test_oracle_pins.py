@@ -177,3 +177,31 @@ def test_window_mode_equals_full_duals():
     b = O.evaluate(w.footprint, w.A, w.B, w.S, w.poses, window=0.01)
     assert np.array_equal(a.value, b.value) and np.array_equal(a.grad, b.grad)
     assert np.array_equal(np.minimum(a.margin, 0.01), b.margin)
+
+
+def test_component_min_and_trajectory_reduce_definitions():
+    """NEXT-4 reductions: hand-worked values (the oracle's definitions against arithmetic done
+    by hand), and the union property phi(E1 u E2) = min(phi(E1), phi(E2)) on an L-shaped
+    obstacle given as two convex boxes."""
+    from oracle import psdf_oracle as O
+    pc = np.array([[3.0, -1.0, 2.0, 0.5], [0.25, 4.0, -2.0, np.inf]])
+    out = O.component_min(pc, [1, 0, 1, 5], 3)                    # id 5 ignored, obstacle 2 has no component
+    assert np.array_equal(out, np.array([[-1.0, 2.0, np.inf], [4.0, -2.0, np.inf]]))
+    v = np.array([1.0, 0.2, 0.2, 3.0, -0.5, 0.6, 0.7, 0.1])
+    mn, am, pen = O.trajectory_reduce(v, 2, 4, 0.5)
+    assert np.array_equal(mn, [0.2, -0.5]) and np.array_equal(am, [1, 0])
+    assert np.allclose(pen, [0.09 + 0.09, 1.0 + 0.16], rtol=0, atol=1e-15)
+    # L-shape = box[0,2]x[0,1] u box[0,1]x[1,2]; rect robot (0.6x0.4) at (2,2,0) spans
+    # [1.7,2.3]x[1.8,2.2]: it overlaps the first box in x (gap 0.8 in y) and the second in y
+    # (gap 0.7 in x), so the components give (0.8, 0.7) and the obstacle 0.7
+    rect = np.array([[-0.3, -0.2], [0.3, -0.2], [0.3, 0.2], [-0.3, 0.2]])
+    def box(x0, x1, y0, y1):
+        P = np.array([[x0, y0], [x1, y0], [x1, y1], [x0, y1]], np.float64)
+        return P, np.roll(P, -1, axis=0)
+    A1, B1 = box(0, 2, 0, 1); A2, B2 = box(0, 1, 1, 2)
+    A = np.stack([A1, A2]); B = np.stack([B1, B2]); S = np.ones((2, 4), np.uint8)
+    r = O.evaluate(rect, A, B, S, np.array([[2.0, 2.0, 0.0], [0.5, 0.5, 0.0]]), per_obstacle=True)
+    d = O.component_min(r.per_obstacle, [0, 0], 1)[:, 0]
+    assert np.allclose(r.per_obstacle[0], [0.8, 0.7], rtol=0, atol=1e-12)
+    assert abs(d[0] - 0.7) < 1e-12 and np.array_equal(d, r.value)
+    assert d[1] < 0                                                # inside the first component
