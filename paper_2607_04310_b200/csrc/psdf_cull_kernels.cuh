@@ -98,7 +98,11 @@ __device__ __forceinline__ void scan_cells(int* cell, int cells) {
 __global__ void __launch_bounds__(1024) pose_hist_kernel(const SortParams s) {
   __shared__ int is_last;
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
-  if (n < s.N) atomicAdd(s.cell + pose_cell(s, n), 1);
+  {  // warp-aggregated: neighbouring poses (same trajectory) share a cell, one atomic per distinct cell
+    const int c = n < s.N ? pose_cell(s, n) : -1;
+    const unsigned peers = __match_any_sync(0xffffffffu, c);
+    if (c >= 0 && (int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) atomicAdd(s.cell + c, __popc(peers));
+  }
   __threadfence();
   __syncthreads();
   if (threadIdx.x == 0) is_last = atomicAdd(s.cell + s.G * s.G, 1) == (int)gridDim.x - 1;
@@ -110,7 +114,14 @@ __global__ void __launch_bounds__(1024) pose_hist_kernel(const SortParams s) {
 
 __global__ void pose_scatter_kernel(const SortParams s) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
-  if (n < s.N) s.perm[atomicAdd(s.cell + pose_cell(s, n), 1)] = n;
+  const int lane = threadIdx.x & 31;
+  const int c = n < s.N ? pose_cell(s, n) : -1;
+  const unsigned peers = __match_any_sync(0xffffffffu, c);          // warp-aggregated cursor bump
+  const int leader = __ffs(peers) - 1;
+  int base = 0;
+  if (c >= 0 && leader == lane) base = atomicAdd(s.cell + c, __popc(peers));
+  base = __shfl_sync(0xffffffffu, base, leader);
+  if (c >= 0) s.perm[base + __popc(peers & ((1u << lane) - 1u))] = n;
 }
 
 // Per-obstacle bound, one float4 per packed obstacle: bounding circle (cx, cy, R) of its
