@@ -62,6 +62,7 @@ struct psdf_scene {
   int* d_pair_begin = nullptr;        // [M+1]
   PackTotals* d_totals = nullptr;
   // culled path (psdf_cull_kernels.cuh)
+  int tune_bd = 0, tune_chunks = 0, tune_cull_warps = 0;   // PSDF_BD / PSDF_CHUNKS / PSDF_CULL_WARPS, read once at create
   int culling = 0;                    // psdf_set_culling
   float4* d_bounds = nullptr;         // [M]
   int* d_perm = nullptr;              // [max_poses]
@@ -156,7 +157,7 @@ cudaError_t enqueue_culled(const psdf_scene* sc, EvalParams& p, int mode, cudaSt
   p.stats = sc->d_stats;
   const int groups = (p.N + 31) / 32;
   int C = 1;                                                // warps per pose group (1: measured best)
-  if (const char* ev = std::getenv("PSDF_CULL_WARPS")) C = std::atoi(ev);
+  if (sc->tune_cull_warps > 0) C = sc->tune_cull_warps;
   C = C < 1 ? 1 : (C > 8 ? 8 : C);
   p.n_chunks = C;
   return launch_cull_v(sc, p, mode, dim3((unsigned)groups), 32 * C, st);
@@ -236,8 +237,8 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
     const double warps_per_sm = (double)N / 32.0 / sc->sm_count;
     if (warps_per_sm < 80.0) C = (int)std::ceil(80.0 / warps_per_sm);
     const int maxC = sc->Mv / 16 > 0 ? sc->Mv / 16 : 1;
-    if (const char* e = std::getenv("PSDF_BD")) bd = std::atoi(e);           // tuning overrides
-    if (const char* e = std::getenv("PSDF_CHUNKS")) C = std::atoi(e);
+    if (sc->tune_bd > 0) bd = sc->tune_bd;                                   // tuning overrides
+    if (sc->tune_chunks > 0) C = sc->tune_chunks;
     if (bd != 32 && bd != 64 && bd != 128 && bd != 256) bd = 64;
     if (C < 1) C = 1;
     if (C > maxC) C = maxC;
@@ -348,6 +349,9 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
   psdf_scene* sc = new (std::nothrow) psdf_scene();
   if (!sc) return PSDF_ERR_ALLOC;
   sc->V = V; sc->M = M; sc->E = E; sc->max_poses = max_poses;
+  if (const char* e = std::getenv("PSDF_BD")) sc->tune_bd = std::atoi(e);             // measurement sweeps only
+  if (const char* e = std::getenv("PSDF_CHUNKS")) sc->tune_chunks = std::atoi(e);
+  if (const char* e = std::getenv("PSDF_CULL_WARPS")) sc->tune_cull_warps = std::atoi(e);
   const int rc = pack_footprint(footprint, V, sc->fp, sc->Vp);
   if (rc != 0) { delete sc; return rc == -1 ? PSDF_ERR_INVALID_ARG : PSDF_ERR_DEGENERATE; }
   if (where == PSDF_MEM_HOST) {   // validate before touching CUDA (Assumption 1)
