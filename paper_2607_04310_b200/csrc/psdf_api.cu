@@ -210,10 +210,11 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
   const int mode = coeff ? kCoeff : ((grad ? kGrad : 0) | (per_obs ? kPerObs : 0));
 
   const long long pairs = (long long)N * (sc->Mv > 0 ? sc->Mv : 1);
-  const bool lanes = N <= 2048 || pairs <= (1 << 16) || window != nullptr;
+  // lane-split kernel: few poses or little work (measured crossover against the tile-scan kernel)
+  const bool lanes = N <= 128 || pairs <= (1 << 17) || window != nullptr;
   dim3 grid;
   int bd;
-  if (sc->culling && !lanes && !per_obs && sc->Mv >= 64) {
+  if (sc->culling && !lanes && N > 2048 && !per_obs && sc->Mv >= 64) {
     cudaError_t e = enqueue_culled(sc, p, mode, st);
     if (e != cudaSuccess) {
       g_last_cuda_error.store((int)e);
@@ -222,12 +223,19 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
     return PSDF_OK;
   }
   if (lanes) {
-    int K = 1;
-    while (K < 32 && K < sc->Mv && (long long)N * K < 148LL * 4 * 128) K <<= 1;
+    // lanes per pose: enough to put ~148 x 1024 lanes in flight, at most one lane per obstacle;
+    // K of them inside a CTA (<= 256), the rest as C CTAs per pose group (<= 16)
+    long long want = (long long)sc->sm_count * 1024 / N;
+    int L = 1;
+    while (L < 4096 && L < sc->Mv && L * 2 <= want) L <<= 1;
+    const int K = L < 256 ? L : 256;
+    int C = L / K;
+    if (C > 16) C = 16;
     p.lanes = K;
-    p.n_chunks = 1;
-    bd = 64;
-    grid = dim3((unsigned)(((long long)N * K + bd - 1) / bd));
+    p.n_chunks = C;
+    bd = K <= 64 ? 64 : K;
+    const int ppc = bd / K;
+    grid = dim3((unsigned)((N + ppc - 1) / ppc), (unsigned)C);
   } else {
     // One thread per pose leaves only N/32 warps; the loop is issue/operand-bound and wants
     // >= ~64 resident warps per SM to hide FMA/ALU latency (measured, profiles/r01_sweep.md),
@@ -384,7 +392,7 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
     CU_TRY(cudaMemsetAsync(sc->d_bbox, 0xff, sizeof(unsigned int) * 4, st));
     CU_TRY(cudaMalloc(&sc->d_ws_depth, sizeof(unsigned long long) * (size_t)max_poses));
     CU_TRY(cudaMalloc(&sc->d_ws_d2, sizeof(unsigned long long) * (size_t)max_poses));
-    const size_t n_cnt = (size_t)(max_poses + 63) / 64 + 1;
+    const size_t n_cnt = (size_t)max_poses + 1;          // scan: one per pose tile; lanes: one per pose group
     CU_TRY(cudaMalloc(&sc->d_ws_count, sizeof(unsigned int) * n_cnt));
     CU_TRY(cudaMemsetAsync(sc->d_ws_depth, 0x00, sizeof(unsigned long long) * (size_t)max_poses, st));
     CU_TRY(cudaMemsetAsync(sc->d_ws_d2, 0xff, sizeof(unsigned long long) * (size_t)max_poses, st));

@@ -188,14 +188,20 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
 }
 
 // ------------------------------------------------------------------------------------------
-// Lane-split kernel for small batches: K = p.lanes lanes per pose, lane k takes obstacles
-// k, k+K, ...; (sd^i, i) arg-min by warp shuffle; lane 0 of the group finalises.
+// Lane-split kernel for small batches: K = p.lanes lanes per pose inside a CTA (power of two,
+// <= blockDim) times p.n_chunks CTAs per pose group (grid.y); lane k of CTA c takes obstacles
+// k + K (c + n_chunks t); (sd^i, i) arg-min by warp shuffle, then (K > 32) through shared
+// memory, then (n_chunks > 1) through a 64-bit global key with the last-arriving CTA of the
+// group finalising; so that even one pose against thousands of obstacles fills the GPU.
 template <int V, int MODE>
-__global__ void __launch_bounds__(128) psdf_lanes_kernel(const __grid_constant__ Footprint fp,
+__global__ void __launch_bounds__(256) psdf_lanes_kernel(const __grid_constant__ Footprint fp,
                                                          const __grid_constant__ EvalParams p) {
-  const int K = p.lanes;
-  const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
-  const int n_raw = gtid / K, lane = gtid % K;
+  __shared__ unsigned long long s_best[256];
+  __shared__ int s_is_last;
+  const int K = p.lanes, C = p.n_chunks;
+  const int ppc = blockDim.x / K;                     // poses per CTA
+  const int g = threadIdx.x / K, lane = threadIdx.x % K;
+  const int n_raw = blockIdx.x * ppc + g;
   const int n = min(n_raw, p.N - 1);
   float x, y, th;
   if (p.packed) {
@@ -218,7 +224,7 @@ __global__ void __launch_bounds__(128) psdf_lanes_kernel(const __grid_constant__
     s_begin = __ldg(p.row_slot + w0);
     s_end = __ldg(p.row_slot + w1);
   }
-  for (int slot = s_begin + lane; slot < s_end; slot += K) {
+  for (int slot = s_begin + lane + K * (int)blockIdx.y; slot < s_end; slot += K * C) {
     const int eb = __ldg(p.row_begin + slot), ee = __ldg(p.row_begin + slot + 1);
     acc.reset();
     float d2 = kInf;
@@ -233,11 +239,33 @@ __global__ void __launch_bounds__(128) psdf_lanes_kernel(const __grid_constant__
     const unsigned long long key = ((unsigned long long)fkey(sd) << 32) | (unsigned)slot;
     best = key < best ? key : best;
   }
-  if ((MODE & kPerObs) && n_raw < p.N)
+  if ((MODE & kPerObs) && n_raw < p.N && blockIdx.y == 0)
     for (int r = lane; r < p.n_empty; r += K) p.per_obs[(size_t)n * p.M_rows + __ldg(p.empty_rows + r)] = kInf;
-  for (int o = K >> 1; o > 0; o >>= 1) {
+  // arg-min over the lanes of the group: within the warp ...
+  for (int o = (K < 32 ? K : 32) >> 1; o > 0; o >>= 1) {
     const unsigned long long other = __shfl_xor_sync(0xffffffffu, best, o);
     best = other < best ? other : best;
+  }
+  if (K > 32) {                                        // ... across the group's warps ...
+    if (lane == 0) s_best[g] = ~0ull;
+    __syncthreads();
+    if ((lane & 31) == 0) atomicMin(&s_best[g], best);
+    __syncthreads();
+    best = s_best[g];
+  }
+  if (C > 1) {                                         // ... and across the group's CTAs
+    if (lane == 0 && n_raw < p.N && best != ~0ull) atomicMin(p.ws_d2 + n, best);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_is_last = (atomicAdd(p.ws_count + blockIdx.x, 1u) == (unsigned)C - 1u);
+    __syncthreads();
+    if (!s_is_last) return;
+    __threadfence();
+    if (threadIdx.x == 0) p.ws_count[blockIdx.x] = 0u; // leave the workspace clean for the next call
+    if (lane == 0 && n_raw < p.N) {
+      best = __ldcg(p.ws_d2 + n);
+      p.ws_d2[n] = ~0ull;
+    }
   }
   if (lane != 0 || n_raw >= p.N) return;
   const bool any = best != ~0ull;

@@ -139,3 +139,25 @@ def test_culled_path_bit_identical_to_dense(env, workloads_cache, cfg, n):
     v3, _, _ = scene.eval(p, grad=False)
     assert np.array_equal(v3.cpu().numpy(), v)
     scene.close()
+
+
+@pytest.mark.parametrize("cfg,n", [(5, 1), (5, 7), (4, 33), (5, 100), (3, 3)])
+def test_few_poses_many_obstacles(env, workloads_cache, cfg, n):
+    """Lane-split kernel with more than one warp (K > 32) and more than one CTA (C > 1) per
+    pose: a handful of poses against up to 4096 obstacles, all outputs, twice (the cross-CTA
+    workspace must be left clean), device and host paths."""
+    torch, O, psdf = env
+    w = workloads_cache(cfg)
+    rng = np.random.default_rng(1000 * cfg + n)
+    poses = w.poses[np.sort(rng.choice(w.N, n, replace=False))]
+    ref = _oracle(O, w, poses=poses, per_obstacle=True)
+    scene, (v, g, po) = _gpu_eval(torch, psdf, w, grad=True, per_obstacle=True, poses=poses)
+    print(w.name, n, compare(ref, v, g, po, what=f"{w.name} n={n}"))
+    p = torch.from_numpy(poses).cuda()
+    v1, g1, _ = scene.eval(p, grad=True)
+    assert np.array_equal(v1.cpu().numpy(), v) and np.array_equal(g1.cpu().numpy(), g)
+    v2, _, _ = scene.eval(p, grad=False)
+    assert np.array_equal(v2.cpu().numpy(), v)
+    vh, gh, poh = scene.eval_host(poses, grad=True, per_obstacle=True)
+    assert np.array_equal(vh, v) and np.array_equal(gh, g) and np.array_equal(poh, po)
+    scene.close()
