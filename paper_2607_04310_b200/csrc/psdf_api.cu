@@ -46,13 +46,19 @@ struct psdf_scene {
   int sm_count = 148;
   std::vector<int> h_pair_begin;      // host copy for chunk planning
   int n_pairs = 0;
-  EdgeRec* d_edges = nullptr;
-  PairRec* d_pairs = nullptr;
-  int* d_row_begin = nullptr;
-  int* d_row_slot = nullptr;          // [M+1]
+  // packed scene, double buffered: an update writes the inactive set and flips `cur` only
+  // after validation has passed (a rejected update leaves the old scene in force)
+  struct Packed {
+    EdgeRec* edges = nullptr;
+    PairRec* pairs = nullptr;
+    int* row_begin = nullptr;
+    int* row_slot = nullptr;          // [M+1]
+    int* empty = nullptr;
+    float4* bounds = nullptr;         // [M]
+  } pk[2];
+  int cur = 0;
   int* h_win = nullptr;               // pinned [max_poses,2]  (psdf_eval_windows_host)
   int* d_win = nullptr;
-  int* d_empty = nullptr;
   unsigned long long* d_ws_depth = nullptr;
   unsigned long long* d_ws_d2 = nullptr;
   unsigned int* d_ws_count = nullptr;
@@ -61,10 +67,11 @@ struct psdf_scene {
   int4* d_offs = nullptr;             // [M] scanned offsets
   int* d_pair_begin = nullptr;        // [M+1]
   PackTotals* d_totals = nullptr;
+  PackTotals* h_totals = nullptr;     // pinned
+  int* h_pair_begin_pinned = nullptr; // pinned [M+1]
   // culled path (psdf_cull_kernels.cuh)
   int tune_bd = 0, tune_chunks = 0, tune_cull_warps = 0;   // PSDF_BD / PSDF_CHUNKS / PSDF_CULL_WARPS, read once at create
   int culling = 0;                    // psdf_set_culling
-  float4* d_bounds = nullptr;         // [M]
   int* d_perm = nullptr;              // [max_poses]
   int* d_cell = nullptr;              // [kSortGridMax^2 + 1]
   unsigned int* d_bbox = nullptr;     // [4]
@@ -150,7 +157,7 @@ cudaError_t enqueue_culled(const psdf_scene* sc, EvalParams& p, int mode, cudaSt
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   p.perm = sc->d_perm;
-  p.bounds = sc->d_bounds;
+  p.bounds = sc->pk[sc->cur].bounds;
   p.sort_cell = sc->d_cell;
   p.sort_bbox = sc->d_bbox;
   p.sort_cells = s.G * s.G;
@@ -184,12 +191,12 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
                          cudaStream_t st, float* packed = nullptr, const int* window = nullptr) {
   if (N == 0) return PSDF_OK;
   EvalParams p{};
-  p.edges = sc->d_edges;
-  p.pairs = sc->d_pairs;
-  p.row_begin = sc->d_row_begin;
-  p.row_slot = sc->d_row_slot;
+  p.edges = sc->pk[sc->cur].edges;
+  p.pairs = sc->pk[sc->cur].pairs;
+  p.row_begin = sc->pk[sc->cur].row_begin;
+  p.row_slot = sc->pk[sc->cur].row_slot;
   p.window = window;
-  p.empty_rows = sc->d_empty;
+  p.empty_rows = sc->pk[sc->cur].empty;
   p.poses = poses;
   p.value = value;
   p.grad = grad;
@@ -277,27 +284,32 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
 psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const uint8_t* S, cudaStream_t st) {
   const int M = sc->M, E = sc->E;
   const int bd = 128, gd = (M + bd - 1) / bd;
-  CU_TRY(cudaMemsetAsync(sc->d_totals, 0, sizeof(PackTotals), st));
-  pack_count_kernel<<<gd, bd, 0, st>>>(A, B, S, M, E, sc->d_cnt, sc->d_totals);
-  pack_scan_kernel<<<1, 1024, 0, st>>>(sc->d_cnt, M, sc->d_offs, sc->d_totals);
-  g_launches.fetch_add(2);
-  PackTotals t{};
-  CU_TRY(cudaMemcpyAsync(&t, sc->d_totals, sizeof(t), cudaMemcpyDeviceToHost, st));
-  CU_TRY(cudaStreamSynchronize(st));
-  CU_TRY(cudaGetLastError());
-  if (t.status != 0) return PSDF_ERR_DEGENERATE;          // nothing live has been touched yet
-  pack_write_kernel<<<gd, bd, 0, st>>>(A, B, S, M, E, sc->d_cnt, sc->d_offs, sc->d_totals, sc->d_edges, sc->d_pairs,
-                                       sc->d_row_begin, sc->d_pair_begin, sc->d_empty, sc->d_bounds, sc->d_row_slot);
-  g_launches.fetch_add(1);
-  sc->h_pair_begin.resize((size_t)t.Mv + 1);
-  CU_TRY(cudaMemcpyAsync(sc->h_pair_begin.data(), sc->d_pair_begin, sizeof(int) * ((size_t)t.Mv + 1),
+  const psdf_scene::Packed& dst = sc->pk[sc->cur ^ 1];      // the inactive set
+  // d_totals and d_pair_begin are one allocation [PackTotals | pair_begin[M+1]]: one copy back
+  if (M <= 256) {                                            // measured: fused wins below ~256 rows
+    pack_fused_kernel<<<1, 1024, 0, st>>>(A, B, S, M, E, sc->d_totals, dst.edges, dst.pairs, dst.row_begin,
+                                          sc->d_pair_begin, dst.empty, dst.bounds, dst.row_slot);
+    g_launches.fetch_add(1);
+  } else {
+    CU_TRY(cudaMemsetAsync(sc->d_totals, 0, sizeof(PackTotals), st));
+    pack_count_kernel<<<gd, bd, 0, st>>>(A, B, S, M, E, sc->d_cnt, sc->d_totals);
+    pack_scan_kernel<<<1, 1024, 0, st>>>(sc->d_cnt, M, sc->d_offs, sc->d_totals);
+    pack_write_kernel<<<gd, bd, 0, st>>>(A, B, S, M, E, sc->d_cnt, sc->d_offs, sc->d_totals, dst.edges, dst.pairs,
+                                         dst.row_begin, sc->d_pair_begin, dst.empty, dst.bounds, dst.row_slot);
+    g_launches.fetch_add(3);
+  }
+  CU_TRY(cudaMemcpyAsync(sc->h_totals, sc->d_totals, sizeof(PackTotals) + sizeof(int) * ((size_t)M + 1),
                          cudaMemcpyDeviceToHost, st));
-  CU_TRY(cudaStreamSynchronize(st));
+  CU_TRY(cudaStreamSynchronize(st));                         // the only synchronisation of an update
   CU_TRY(cudaGetLastError());
+  const PackTotals t = *sc->h_totals;
+  if (t.status != 0) return PSDF_ERR_DEGENERATE;             // the live set has not been touched
+  sc->h_pair_begin.assign(sc->h_pair_begin_pinned, sc->h_pair_begin_pinned + t.Mv + 1);
   sc->n_edges = t.n_edges;
   sc->Mv = t.Mv;
   sc->n_empty = t.n_empty;
   sc->n_pairs = t.n_pairs;
+  sc->cur ^= 1;
   return PSDF_OK;
 }
 
@@ -306,22 +318,24 @@ psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const u
   if (where == PSDF_MEM_DEVICE) return pack_on_device(sc, A, B, S, st);
   PackedScene ps;
   if (pack_scene(A, B, S, sc->M, sc->E, ps) != 0) return PSDF_ERR_DEGENERATE;
-  sc->n_edges = (int)ps.edges.size();
-  sc->Mv = (int)ps.row_begin.size() - 1;
-  sc->n_empty = (int)ps.empty_rows.size();
-  sc->h_pair_begin = ps.pair_begin;
-  sc->n_pairs = (int)ps.pairs.size();
-  if (sc->n_edges) {
-    CU_TRY(cudaMemcpyAsync(sc->d_edges, ps.edges.data(), sizeof(EdgeRec) * sc->n_edges, cudaMemcpyHostToDevice, st));
-    CU_TRY(cudaMemcpyAsync(sc->d_pairs, ps.pairs.data(), sizeof(PairRec) * sc->n_pairs, cudaMemcpyHostToDevice, st));
+  const psdf_scene::Packed& dst = sc->pk[sc->cur ^ 1];
+  const int n_edges = (int)ps.edges.size(), Mv = (int)ps.row_begin.size() - 1, n_empty = (int)ps.empty_rows.size();
+  const int n_pairs = (int)ps.pairs.size();
+  if (n_edges) {
+    CU_TRY(cudaMemcpyAsync(dst.edges, ps.edges.data(), sizeof(EdgeRec) * n_edges, cudaMemcpyHostToDevice, st));
+    CU_TRY(cudaMemcpyAsync(dst.pairs, ps.pairs.data(), sizeof(PairRec) * n_pairs, cudaMemcpyHostToDevice, st));
   }
-  CU_TRY(cudaMemcpyAsync(sc->d_row_slot, ps.row_slot.data(), sizeof(int) * (size_t)(sc->M + 1), cudaMemcpyHostToDevice, st));
-  if (sc->Mv)
-    CU_TRY(cudaMemcpyAsync(sc->d_bounds, ps.bounds.data(), sizeof(float4) * sc->Mv, cudaMemcpyHostToDevice, st));
-  CU_TRY(cudaMemcpyAsync(sc->d_row_begin, ps.row_begin.data(), sizeof(int) * (sc->Mv + 1), cudaMemcpyHostToDevice, st));
-  if (sc->n_empty)
-    CU_TRY(cudaMemcpyAsync(sc->d_empty, ps.empty_rows.data(), sizeof(int) * sc->n_empty, cudaMemcpyHostToDevice, st));
+  CU_TRY(cudaMemcpyAsync(dst.row_slot, ps.row_slot.data(), sizeof(int) * (size_t)(sc->M + 1), cudaMemcpyHostToDevice, st));
+  if (Mv) CU_TRY(cudaMemcpyAsync(dst.bounds, ps.bounds.data(), sizeof(float4) * Mv, cudaMemcpyHostToDevice, st));
+  CU_TRY(cudaMemcpyAsync(dst.row_begin, ps.row_begin.data(), sizeof(int) * (Mv + 1), cudaMemcpyHostToDevice, st));
+  if (n_empty) CU_TRY(cudaMemcpyAsync(dst.empty, ps.empty_rows.data(), sizeof(int) * n_empty, cudaMemcpyHostToDevice, st));
   CU_TRY(cudaStreamSynchronize(st));       // the staging vectors die here
+  sc->n_edges = n_edges;
+  sc->Mv = Mv;
+  sc->n_empty = n_empty;
+  sc->n_pairs = n_pairs;
+  sc->h_pair_begin.swap(ps.pair_begin);
+  sc->cur ^= 1;
   return PSDF_OK;
 }
 
@@ -335,12 +349,15 @@ void psdf_destroy_scene(psdf_scene* sc) {
   for (auto& g : sc->graphs)
     if (g.exec) cudaGraphExecDestroy(g.exec);
   if (sc->gstream) cudaStreamDestroy(sc->gstream);
-  cudaFree(sc->d_edges); cudaFree(sc->d_pairs); cudaFree(sc->d_row_begin); cudaFree(sc->d_empty);
-  cudaFree(sc->d_row_slot); cudaFree(sc->d_win);
+  for (auto& b : sc->pk) {
+    cudaFree(b.edges); cudaFree(b.pairs); cudaFree(b.row_begin); cudaFree(b.row_slot); cudaFree(b.empty); cudaFree(b.bounds);
+  }
+  cudaFree(sc->d_win);
+  if (sc->h_totals) cudaFreeHost(sc->h_totals);
   if (sc->h_win) cudaFreeHost(sc->h_win);
   cudaFree(sc->d_ws_depth); cudaFree(sc->d_ws_d2); cudaFree(sc->d_ws_count);
-  cudaFree(sc->d_stats); cudaFree(sc->d_bounds); cudaFree(sc->d_perm); cudaFree(sc->d_cell); cudaFree(sc->d_bbox);
-  cudaFree(sc->d_cnt); cudaFree(sc->d_offs); cudaFree(sc->d_pair_begin); cudaFree(sc->d_totals);
+  cudaFree(sc->d_stats); cudaFree(sc->d_perm); cudaFree(sc->d_cell); cudaFree(sc->d_bbox);
+  cudaFree(sc->d_cnt); cudaFree(sc->d_offs); cudaFree(sc->d_totals);   // d_pair_begin lives inside d_totals' block
   cudaFree(sc->d_in); cudaFree(sc->d_out); cudaFree(sc->d_per);
   if (sc->h_in) cudaFreeHost(sc->h_in);
   if (sc->h_out) cudaFreeHost(sc->h_out);
@@ -373,16 +390,20 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
   auto body = [&]() -> psdf_status {
     CU_TRY(cudaGetDevice(&dev));
     CU_TRY(cudaDeviceGetAttribute(&sc->sm_count, cudaDevAttrMultiProcessorCount, dev));
-    CU_TRY(cudaMalloc(&sc->d_edges, sizeof(EdgeRec) * (size_t)sc->edge_cap));
-    CU_TRY(cudaMalloc(&sc->d_pairs, sizeof(PairRec) * (size_t)(sc->edge_cap / 2 + M)));
-    CU_TRY(cudaMalloc(&sc->d_row_begin, sizeof(int) * (size_t)(M + 1)));
-    CU_TRY(cudaMalloc(&sc->d_row_slot, sizeof(int) * (size_t)(M + 1)));
-    CU_TRY(cudaMalloc(&sc->d_empty, sizeof(int) * (size_t)M));
+    for (auto& b : sc->pk) {
+      CU_TRY(cudaMalloc(&b.edges, sizeof(EdgeRec) * (size_t)sc->edge_cap));
+      CU_TRY(cudaMalloc(&b.pairs, sizeof(PairRec) * (size_t)(sc->edge_cap / 2 + M)));
+      CU_TRY(cudaMalloc(&b.row_begin, sizeof(int) * (size_t)(M + 1)));
+      CU_TRY(cudaMalloc(&b.row_slot, sizeof(int) * (size_t)(M + 1)));
+      CU_TRY(cudaMalloc(&b.empty, sizeof(int) * (size_t)M));
+      CU_TRY(cudaMalloc(&b.bounds, sizeof(float4) * (size_t)M));
+    }
+    CU_TRY(cudaMallocHost(&sc->h_totals, sizeof(PackTotals) + sizeof(int) * (size_t)(M + 1)));
+    sc->h_pair_begin_pinned = reinterpret_cast<int*>(sc->h_totals + 1);
     CU_TRY(cudaMalloc(&sc->d_cnt, sizeof(int) * (size_t)M));
     CU_TRY(cudaMalloc(&sc->d_offs, sizeof(int4) * (size_t)M));
-    CU_TRY(cudaMalloc(&sc->d_pair_begin, sizeof(int) * (size_t)(M + 1)));
-    CU_TRY(cudaMalloc(&sc->d_totals, sizeof(PackTotals)));
-    CU_TRY(cudaMalloc(&sc->d_bounds, sizeof(float4) * (size_t)M));
+    CU_TRY(cudaMalloc(&sc->d_totals, sizeof(PackTotals) + sizeof(int) * (size_t)(M + 1)));
+    sc->d_pair_begin = reinterpret_cast<int*>(sc->d_totals + 1);
     CU_TRY(cudaMalloc(&sc->d_perm, sizeof(int) * (size_t)max_poses));
     CU_TRY(cudaMalloc(&sc->d_cell, sizeof(int) * (size_t)(kSortGridMax * kSortGridMax + 1)));
     CU_TRY(cudaMalloc(&sc->d_bbox, sizeof(unsigned int) * 4));
@@ -408,12 +429,9 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
 psdf_status psdf_update_scene(psdf_scene* sc, const float* A, const float* B, const uint8_t* S,
                               psdf_mem where, void* cuda_stream) {
   if (!sc || !A || !B || !S) return PSDF_ERR_INVALID_ARG;
-  // validate on the host first so that a bad update leaves the old scene in force
+  // both paths validate before anything live changes (host: pack_scene; device: status word
+  // checked before the buffer flip), so a bad update leaves the old scene in force
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (where == PSDF_MEM_HOST) {
-    PackedScene probe;
-    if (pack_scene(A, B, S, sc->M, sc->E, probe) != 0) return PSDF_ERR_DEGENERATE;
-  }
   if (sc->gstream) CU_TRY(cudaStreamSynchronize(sc->gstream));
   psdf_status s = upload_scene(sc, A, B, S, where, st);
   if (s != PSDF_OK) return s;

@@ -7,8 +7,8 @@
 //   pack_scan_kernel    one CTA: exclusive scans of (slot, edge, pair, empty) offsets;
 //   pack_write_kernel   one thread per row: writes the records, row_begin, pair_begin and
 //                       the empty-row list at the scanned offsets.
-// Nothing live is overwritten before validation has passed (the host checks *status between
-// the scan and the write), so a rejected update leaves the old scene in force.
+// The records go to the scene's INACTIVE buffer set and the host flips the sets only if *status
+// is still 0 after its single synchronisation, so a rejected update leaves the old scene in force.
 #pragma once
 #include "psdf_pack.h"
 
@@ -92,6 +92,7 @@ __global__ void pack_write_kernel(const float* __restrict__ A, const float* __re
                                   int* __restrict__ empty_rows, float4* __restrict__ bounds,
                                   int* __restrict__ row_slot) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (totals->status != 0) return;                    // rejected: the host will not flip the buffers
   if (i == 0) {
     row_begin[totals->Mv] = totals->n_edges;
     pair_begin[totals->Mv] = totals->n_pairs;
@@ -101,6 +102,59 @@ __global__ void pack_write_kernel(const float* __restrict__ A, const float* __re
   const int4 o = offs[i];
   row_slot[i] = o.x;
   int e = count[i];
+  if (e == 0) { empty_rows[o.w] = i; return; }
+  EdgeRec* er = edges + o.y;
+  pack_row(A + (size_t)i * E * 2, B + (size_t)i * E * 2, S + (size_t)i * E, E, i, o.x, er, &e);
+  for (int k2 = 0; k2 < (e + 1) >> 1; ++k2) pairs[o.z + k2] = make_pair_rec(er, e, k2, o.x);
+  bounds[o.x] = obstacle_bound(er, e, o.z);
+  row_begin[o.x] = o.y;
+  pair_begin[o.x] = o.z;
+}
+
+// Small scenes (the MPC case; used for M <= 256, valid up to 1024): count + scan + write fused into ONE single-CTA
+// launch (1024 threads, one per row), so a perception update costs one kernel and one copy.
+__global__ void __launch_bounds__(1024) pack_fused_kernel(const float* __restrict__ A, const float* __restrict__ B,
+                                                          const uint8_t* __restrict__ S, int M, int E,
+                                                          PackTotals* __restrict__ totals, EdgeRec* __restrict__ edges,
+                                                          PairRec* __restrict__ pairs, int* __restrict__ row_begin,
+                                                          int* __restrict__ pair_begin, int* __restrict__ empty_rows,
+                                                          float4* __restrict__ bounds, int* __restrict__ row_slot) {
+  __shared__ int4 warp_sum[32];
+  const int i = threadIdx.x, lane = i & 31, wid = i >> 5;
+  int e = 0, rc = 0;
+  if (i < M) rc = pack_row(A + (size_t)i * E * 2, B + (size_t)i * E * 2, S + (size_t)i * E, E, i, 0, nullptr, &e);
+  const int bad = __syncthreads_or(rc != 0);
+  const int4 v = make_int4(e > 0 ? 1 : 0, e, (e + 1) >> 1, (i < M && e == 0) ? 1 : 0);
+  int4 inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int a = __shfl_up_sync(0xffffffffu, inc.x, o), b = __shfl_up_sync(0xffffffffu, inc.y, o);
+    const int c = __shfl_up_sync(0xffffffffu, inc.z, o), d = __shfl_up_sync(0xffffffffu, inc.w, o);
+    if (lane >= o) { inc.x += a; inc.y += b; inc.z += c; inc.w += d; }
+  }
+  if (lane == 31) warp_sum[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    const int4 w = warp_sum[lane];
+    int4 winc = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int a = __shfl_up_sync(0xffffffffu, winc.x, o), b = __shfl_up_sync(0xffffffffu, winc.y, o);
+      const int c = __shfl_up_sync(0xffffffffu, winc.z, o), d = __shfl_up_sync(0xffffffffu, winc.w, o);
+      if (lane >= o) { winc.x += a; winc.y += b; winc.z += c; winc.w += d; }
+    }
+    warp_sum[lane] = make_int4(winc.x - w.x, winc.y - w.y, winc.z - w.z, winc.w - w.w);
+    if (lane == 31) {
+      totals->status = bad ? -2 : 0;
+      totals->Mv = winc.x; totals->n_edges = winc.y; totals->n_pairs = winc.z; totals->n_empty = winc.w;
+      if (!bad) { row_begin[winc.x] = winc.y; pair_begin[winc.x] = winc.z; row_slot[M] = winc.x; }
+    }
+  }
+  __syncthreads();
+  if (bad || i >= M) return;
+  const int4 wb = warp_sum[wid];
+  const int4 o = make_int4(wb.x + inc.x - v.x, wb.y + inc.y - v.y, wb.z + inc.z - v.z, wb.w + inc.w - v.w);
+  row_slot[i] = o.x;
   if (e == 0) { empty_rows[o.w] = i; return; }
   EdgeRec* er = edges + o.y;
   pack_row(A + (size_t)i * E * 2, B + (size_t)i * E * 2, S + (size_t)i * E, E, i, o.x, er, &e);
