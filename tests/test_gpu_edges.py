@@ -310,3 +310,38 @@ def test_component_min_and_trajectory_reduce(env):
     assert np.abs(pen.cpu().numpy() - open_).max() <= 1e-4 * max(1.0, open_.max())
     assert (rpen > 0).any()
     scene.close()
+
+
+def test_eval_is_cuda_graph_capturable(env):
+    """psdf_eval only enqueues (no allocation, no synchronisation): it can be captured into a
+    CUDA graph on the caller's stream and replayed on new pose contents; dense (chunked
+    tile-scan), lane-split and culled paths."""
+    torch, O, psdf, W = env
+    for cfg, n, cull in ((3, 6000, False), (3, 6000, True), (2, 50, False)):
+        w = W.make_config(cfg) if cfg == 2 else W.make_config(cfg, n_traj=n // 50)
+        scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=w.N)
+        scene.set_culling(cull)
+        poses = torch.from_numpy(w.poses).cuda()
+        value = torch.empty(w.N, dtype=torch.float32, device="cuda")
+        grad = torch.empty((w.N, 3), dtype=torch.float32, device="cuda")
+        scene.eval(poses, value=value, grad=grad)                   # warm-up outside capture
+        torch.cuda.synchronize()
+        want_v, want_g = value.clone(), grad.clone()
+        static = poses.clone()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            scene.eval(static, value=value, grad=grad)
+        value.zero_(); grad.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(value, want_v) and torch.equal(grad, want_g)
+        # new contents through the same graph
+        shifted = w.poses.copy()
+        shifted[:, 2] += np.float32(0.5)
+        static.copy_(torch.from_numpy(shifted).cuda())
+        g.replay()
+        torch.cuda.synchronize()
+        v2, g2, _ = scene.eval(torch.from_numpy(shifted).cuda(), grad=True)
+        assert torch.equal(value, v2) and torch.equal(grad, g2)
+        del g
+        scene.close()
