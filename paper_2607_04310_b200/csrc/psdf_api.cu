@@ -70,7 +70,7 @@ struct psdf_scene {
   PackTotals* h_totals = nullptr;     // pinned
   int* h_pair_begin_pinned = nullptr; // pinned [M+1]
   // culled path (psdf_cull_kernels.cuh)
-  int tune_bd = 0, tune_chunks = 0, tune_cull_warps = 0;   // PSDF_BD / PSDF_CHUNKS / PSDF_CULL_WARPS, read once at create
+  int tune_bd = 0, tune_chunks = 0;   // PSDF_BD / PSDF_CHUNKS, read once at create
   int culling = 0;                    // psdf_set_culling
   int* d_perm = nullptr;              // [max_poses]
   int* d_cell = nullptr;              // [kSortGridMax^2 + 1]
@@ -163,11 +163,8 @@ cudaError_t enqueue_culled(const psdf_scene* sc, EvalParams& p, int mode, cudaSt
   p.sort_cells = s.G * s.G;
   p.stats = sc->d_stats;
   const int groups = (p.N + 31) / 32;
-  int C = 1;                                                // warps per pose group (1: measured best)
-  if (sc->tune_cull_warps > 0) C = sc->tune_cull_warps;
-  C = C < 1 ? 1 : (C > 8 ? 8 : C);
-  p.n_chunks = C;
-  return launch_cull_v(sc, p, mode, dim3((unsigned)groups), 32 * C, st);
+  p.n_chunks = 1;
+  return launch_cull_v(sc, p, mode, dim3((unsigned)groups), 32, st);
 }
 
 cudaError_t launch_v(const psdf_scene* sc, const EvalParams& p, int mode, bool lanes, dim3 grid, int bd,
@@ -376,7 +373,6 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
   sc->V = V; sc->M = M; sc->E = E; sc->max_poses = max_poses;
   if (const char* e = std::getenv("PSDF_BD")) sc->tune_bd = std::atoi(e);             // measurement sweeps only
   if (const char* e = std::getenv("PSDF_CHUNKS")) sc->tune_chunks = std::atoi(e);
-  if (const char* e = std::getenv("PSDF_CULL_WARPS")) sc->tune_cull_warps = std::atoi(e);
   const int rc = pack_footprint(footprint, V, sc->fp, sc->Vp);
   if (rc != 0) { delete sc; return rc == -1 ? PSDF_ERR_INVALID_ARG : PSDF_ERR_DEGENERATE; }
   if (where == PSDF_MEM_HOST) {   // validate before touching CUDA (Assumption 1)
@@ -407,7 +403,11 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
     CU_TRY(cudaMalloc(&sc->d_perm, sizeof(int) * (size_t)max_poses));
     CU_TRY(cudaMalloc(&sc->d_cell, sizeof(int) * (size_t)(kSortGridMax * kSortGridMax + 1)));
     CU_TRY(cudaMalloc(&sc->d_bbox, sizeof(unsigned int) * 4));
+#ifdef PSDF_CULL_LOG
+    CU_TRY(cudaMalloc(&sc->d_stats, sizeof(unsigned long long) * (2 + 4 * (size_t)(max_poses / 32 + 1))));
+#else
     CU_TRY(cudaMalloc(&sc->d_stats, sizeof(unsigned long long) * 2));
+#endif
     CU_TRY(cudaMemsetAsync(sc->d_stats, 0, sizeof(unsigned long long) * 2, st));
     CU_TRY(cudaMemsetAsync(sc->d_cell, 0x00, sizeof(int) * (size_t)(kSortGridMax * kSortGridMax + 1), st));
     CU_TRY(cudaMemsetAsync(sc->d_bbox, 0xff, sizeof(unsigned int) * 4, st));
@@ -665,6 +665,16 @@ psdf_status psdf_trajectory_reduce(const float* value, int T, int H, float d_saf
 psdf_status psdf_cull_stats(psdf_scene* sc, void* cuda_stream, unsigned long long* out2) {
   if (!sc || !out2) return PSDF_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
+#ifdef PSDF_CULL_LOG
+  if (const char* f = std::getenv("PSDF_CULL_LOG_FILE")) {
+    const size_t n = 2 + 4 * (size_t)(sc->max_poses / 32 + 1);
+    std::vector<unsigned long long> h(n);
+    cudaMemcpy(h.data(), sc->d_stats, n * 8, cudaMemcpyDeviceToHost);
+    FILE* fp = std::fopen(f, "wb");
+    std::fwrite(h.data(), 8, n, fp);
+    std::fclose(fp);
+  }
+#endif
   CU_TRY(cudaMemcpyAsync(out2, sc->d_stats, sizeof(unsigned long long) * 2, cudaMemcpyDeviceToHost, st));
   CU_TRY(cudaMemsetAsync(sc->d_stats, 0, sizeof(unsigned long long) * 2, st));
   CU_TRY(cudaStreamSynchronize(st));

@@ -127,17 +127,16 @@ __global__ void pose_scatter_kernel(const SortParams s) {
 // Per-obstacle bound, one float4 per packed obstacle: bounding circle (cx, cy, R) of its
 // vertices and the index of its first pair record (int bits).
 //
-// Culled evaluation.  CTA = C warps that own the SAME 32 sorted poses (lane = pose); warp c
-// walks the obstacle batches c, c+C, ... and the warps share the per-pose running upper bound
-// through shared memory (monotone atomicMin on an ordered key: a stale read is merely less
-// tight).  MODE in {0, kGrad, kCoeff}.  The workspace left dirty by the pose sort is cleaned
-// here for the next call.
+// Culled evaluation: one warp (= one CTA) per 32 sorted poses, lane = pose.  MODE in
+// {0, kGrad, kCoeff}.  The workspace left dirty by the pose sort is cleaned here for the next
+// call.  (Several warps per pose group sharing the running bound were measured: never faster.)
 template <int V, int MODE>
-__global__ void __launch_bounds__(256) psdf_cull_kernel(const __grid_constant__ Footprint fp,
+__global__ void __launch_bounds__(32) psdf_cull_kernel(const __grid_constant__ Footprint fp,
                                                         const __grid_constant__ EvalParams p) {
-  __shared__ unsigned int s_ub[32];
-  __shared__ unsigned long long s_depth[32], s_d2[32];
-  const int lane = threadIdx.x & 31, wc = threadIdx.x >> 5, C = blockDim.x >> 5;
+  const int lane = threadIdx.x & 31;
+#ifdef PSDF_CULL_LOG
+  const long long t_start = clock64();
+#endif
   {  // clean the sort workspace (its last reader, pose_scatter_kernel, has completed)
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t <= p.sort_cells) p.sort_cell[t] = 0;
@@ -159,10 +158,6 @@ __global__ void __launch_bounds__(256) psdf_cull_kernel(const __grid_constant__ 
   float ub = finite ? kInf : -kInf;                        // running upper bound of phi for this lane
   int idD2 = -1, idDepth = -1;
   unsigned n_visit = 0, n_edge = 0;                        // statistics (psdf_cull_stats)
-  if (C > 1) {
-    if (wc == 0) { s_ub[lane] = fkey(ub); s_depth[lane] = 0ull; s_d2[lane] = ~0ull; }
-    __syncthreads();
-  }
   const float4* __restrict__ bounds = p.bounds;
   const float4* __restrict__ recs = reinterpret_cast<const float4*>(p.pairs);
 
@@ -198,7 +193,6 @@ __global__ void __launch_bounds__(256) psdf_cull_kernel(const __grid_constant__ 
     if (depth > maxDepth) { maxDepth = depth; idDepth = slot; }
     if (finite) {
       const float nub = fminf(ub, maxDepth >= 0.f ? -maxDepth : sqrtf(minD2));
-      if (C > 1 && nub < ub) atomicMin(&s_ub[lane], fkey(nub));
       ub = nub;
     }
   };
@@ -211,7 +205,7 @@ __global__ void __launch_bounds__(256) psdf_cull_kernel(const __grid_constant__ 
   // Phase A: the two obstacles nearest to the pose box go first, so that the running upper
   // bound is tight before the memory-order walk (evaluated obstacles per warp drop ~2x).
   int first0 = -1, first1 = -1;
-  if (wc == 0) {
+  {
     unsigned k0 = 0xffffffffu, k1 = 0xffffffffu;           // this lane's two smallest keys
     int i0 = -1, i1 = -1;
     // (ordering heuristic only: squared box distance minus squared radius, no sqrt)
@@ -235,45 +229,52 @@ __global__ void __launch_bounds__(256) psdf_cull_kernel(const __grid_constant__ 
     }
   }
 
-  // Phase B: memory-order walk, 32 obstacles per step: one box test per obstacle per warp
-  const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
-  float4 bn0 = 32 * wc + lane < p.Mv ? __ldg(bounds + 32 * wc + lane) : zero4;            // two batches in flight
-  float4 bn1 = 32 * (wc + C) + lane < p.Mv ? __ldg(bounds + 32 * (wc + C) + lane) : zero4;
-  for (int base = 32 * wc; base < p.Mv; base += 32 * C) {
-    const int i = base + lane;
-    const float4 b = bn0;
-    bn0 = bn1;
-    bn1 = i + 64 * C < p.Mv ? __ldg(bounds + i + 64 * C) : zero4;
-    if (C > 1) ub = fminf(ub, fkey_inv(*reinterpret_cast<volatile unsigned int*>(&s_ub[lane])));
+#ifdef PSDF_CULL_LOG
+  const long long t_phaseA = clock64();
+#endif
+  // Phase B: memory-order walk, 4 x 32 obstacles per step (four independent loads, tests and
+  // ballots in flight: the walk is latency bound): one box test per obstacle per warp.  A
+  // survivor of a stale warp-level bound is still re-tested per lane inside visit().
+  for (int base = 0; base < p.Mv; base += 128) {
+    float4 b[4];
+    unsigned mask[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = base + 32 * u + lane;
+      b[u] = i < p.Mv ? __ldg(bounds + i) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
     const float ubmax = warp_max_f(ub);
-    const float thr = (ubmax + b.z) * 1.0001f + rpad;
-    const bool skip = (i >= p.Mv) || (i == first0) || (i == first1) || (thr < 0.f) || (box_d2(b) > thr * thr);
-    unsigned mask = __ballot_sync(0xffffffffu, !skip);
-    while (mask) {
-      const int j = __ffs(mask) - 1;
-      mask &= mask - 1;
-      visit(__shfl_sync(0xffffffffu, b.x, j), __shfl_sync(0xffffffffu, b.y, j), __shfl_sync(0xffffffffu, b.z, j),
-            __shfl_sync(0xffffffffu, __float_as_int(b.w), j));
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = base + 32 * u + lane;
+      const float thr = (ubmax + b[u].z) * 1.0001f + rpad;
+      const bool skip = (i >= p.Mv) || (i == first0) || (i == first1) || (thr < 0.f) || (box_d2(b[u]) > thr * thr);
+      mask[u] = __ballot_sync(0xffffffffu, !skip);
+    }
+    if ((mask[0] | mask[1] | mask[2] | mask[3]) == 0u) continue;
+#pragma unroll 1
+    for (int u = 0; u < 4; ++u) {
+      const float4 bu = u == 0 ? b[0] : (u == 1 ? b[1] : (u == 2 ? b[2] : b[3]));
+      unsigned m = u == 0 ? mask[0] : (u == 1 ? mask[1] : (u == 2 ? mask[2] : mask[3]));
+      while (m) {
+        const int j = __ffs(m) - 1;
+        m &= m - 1;
+        visit(__shfl_sync(0xffffffffu, bu.x, j), __shfl_sync(0xffffffffu, bu.y, j), __shfl_sync(0xffffffffu, bu.z, j),
+              __shfl_sync(0xffffffffu, __float_as_int(bu.w), j));
+      }
     }
   }
+#ifdef PSDF_CULL_LOG
+  if (p.stats && lane == 0) {   // per-warp log after the two counters: (cycles, visits, tA, tB)
+    unsigned long long* lg = p.stats + 2 + 4 * (size_t)blockIdx.x;
+    lg[0] = clock64() - t_start; lg[1] = n_visit; lg[2] = t_phaseA - t_start; lg[3] = clock64() - t_phaseA;
+  }
+#endif
   if (p.stats && lane == 0) {
     atomicAdd(p.stats, (unsigned long long)n_visit);
     atomicAdd(p.stats + 1, (unsigned long long)n_edge);
   }
   if (!(MODE & (kGrad | kCoeff))) idD2 = minD2 < kInf ? 0 : -1;
-  if (C > 1) {
-    // combine the C partial (arg-)results of each pose; same keys as the dense kernel
-    if (idDepth >= 0)
-      atomicMax(&s_depth[lane], ((unsigned long long)fkey(maxDepth) << 32) | (0xffffffffu - (unsigned)idDepth));
-    if (idD2 >= 0) atomicMin(&s_d2[lane], ((unsigned long long)__float_as_uint(minD2) << 32) | (unsigned)idD2);
-    __syncthreads();
-    if (wc != 0) return;
-    const unsigned long long kd = s_depth[lane], k2 = s_d2[lane];
-    maxDepth = kd ? fkey_inv((uint32_t)(kd >> 32)) : -kInf;
-    idDepth = kd ? (int)(0xffffffffu - (uint32_t)kd) : -1;
-    minD2 = (k2 != ~0ull) ? __uint_as_float((uint32_t)(k2 >> 32)) : kInf;
-    idD2 = (k2 != ~0ull) ? (int)(uint32_t)k2 : -1;
-  }
   if (k >= p.N) return;
   const bool separated = !(maxDepth >= 0.f);
   const float value = separated ? sqrtf(minD2) : -maxDepth;
