@@ -299,7 +299,7 @@ def main():
     scene.cull_stats()
     k_cull = max(args.steps // 2, 10)
     cull_times = timed(k_cull, True)
-    visits, edge_steps = scene.cull_stats()
+    eval_pairs, edge_steps = scene.cull_stats()
     v_cull = value.clone()
     scene.set_culling(False)
     timed(1, True)
@@ -350,13 +350,14 @@ def main():
             "e2e": {"value": pairs * world / t_e2e, "unit": UNIT, "ms_per_step": t_e2e * 1e3,
                     "h2d_bytes_per_step": w.N * 12, "d2h_bytes_per_step": w.N * 16,
                     "api": "psdf_eval_host (host buffers -> pinned staging -> CUDA graph {H2D, kernel, D2H} -> host)"},
-            "culling": {"what": "psdf_set_culling(1): pose grid sort + warp-level bounding-circle culling, value+grad; "
-                                "outputs bit-identical to the dense path (checked in this run: %s)" % culled_same,
+            "culling": {"what": "psdf_set_culling(1): obstacle grid + bounding-circle / oriented-box lower bounds, "
+                                "pair-queue kernel, value+grad; outputs bit-identical to the dense path "
+                                "(checked in this run: %s)" % culled_same,
                         "ms_per_step": float(np.mean(cull_times)), "value": pairs / (float(np.mean(cull_times)) * 1e-3),
                         "unit": UNIT, "speedup_vs_dense": t_kernel * 1e3 / float(np.mean(cull_times)),
-                        "evaluated_pair_fraction": 32.0 * visits / k_cull / pairs,
-                        "evaluated_flops_per_step": 32.0 * ((32.0 * w.V + 6.0) * edge_steps + (4.0 * w.V + 6.0) * visits) / k_cull,
-                        "note": "pairs/s counts all pairs (SURVEY.md 8(d)); culled pairs cost one bound test per warp"},
+                        "evaluated_pair_fraction": eval_pairs / k_cull / pairs,
+                        "evaluated_flops_per_step": ((32.0 * w.V + 6.0) * edge_steps + (4.0 * w.V + 6.0) * eval_pairs) / k_cull,
+                        "note": "pairs/s counts all pairs (SURVEY.md 8(d)); culled pairs cost at most two bound tests"},
             "gpu_launches": int(launches), "wall_s_timed_region": t_wall, "clocks": clocks,
             "paper_context": {"psdf_rtx4090_M100_B100_ms": 2.207, "implied_pairs_per_s": 4.5e6,
                               "source": "PAPER.md:419 Table I (other hardware, context only)"},

@@ -106,11 +106,13 @@ psdf_status psdf_mpc_coeffs_host(psdf_scene* scene, const float* poses, int N, f
                                  float rho_p, float rho_theta, float* coeff);
 
 /* Exact broad-phase culling (beyond the paper; valid because phi is a minimum over obstacles,
- * eq.(6)).  When enabled, large batches (N > 2048) evaluated without
- * per_obstacle output go through a grid sort of the poses and a warp-per-32-poses kernel that
- * skips every obstacle whose bounding-circle lower bound |p - c_i| - R_i - r_max exceeds the
- * running value; surviving pairs use the same arithmetic as the dense path, so value and grad
- * are bit-identical to the dense result.  Default: disabled (dense, branch-free evaluation). */
+ * eq.(6)).  When enabled, large batches (N > 2048, >= 64 obstacles) evaluated without
+ * per_obstacle output go through one kernel that looks obstacles up in a uniform grid (rebuilt on
+ * the device at every create/update) and skips every obstacle whose lower bound on sd^i (bounding
+ * circles, then oriented bounding boxes of footprint and obstacle) exceeds an upper bound of phi
+ * obtained from a nearby obstacle; surviving pairs use the same arithmetic and reductions as the
+ * dense path, so value and grad are bit-identical to the dense result.  Default: disabled (dense,
+ * branch-free evaluation). */
 psdf_status psdf_set_culling(psdf_scene* scene, int enable);
 
 /* Non-convex obstacles given as convex components (Assumption 1; eq.(6),
@@ -129,7 +131,7 @@ psdf_status psdf_trajectory_reduce(const float* value, int T, int H, float d_saf
                                    int* argmin_stage, float* penalty, void* cuda_stream);
 
 /* Culled-path statistics accumulated since the last call (then reset): out2[0] = number of
- * (warp of 32 poses, obstacle) evaluations, out2[1] = number of (warp, obstacle edge) steps.
+ * evaluated (pose, obstacle) pairs, out2[1] = number of (pose, obstacle edge) steps.
  * Synchronises `cuda_stream`.  Used by bench.py for the evaluated-pair fraction and FLOPs. */
 psdf_status psdf_cull_stats(psdf_scene* scene, void* cuda_stream, unsigned long long* out2);
 

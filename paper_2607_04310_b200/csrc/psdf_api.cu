@@ -54,7 +54,10 @@ struct psdf_scene {
     int* row_begin = nullptr;
     int* row_slot = nullptr;          // [M+1]
     int* empty = nullptr;
-    float4* bounds = nullptr;         // [M]
+    float4* bounds = nullptr;         // [2 M] circle, box per obstacle
+    float4* gbounds = nullptr;        // [2 M] bounds in obstacle-grid order
+    int* gcell = nullptr;             // [kObsGridMax^2 + 1]
+    GridHdr* ghdr = nullptr;
   } pk[2];
   int cur = 0;
   int* h_win = nullptr;               // pinned [max_poses,2]  (psdf_eval_windows_host)
@@ -72,9 +75,6 @@ struct psdf_scene {
   // culled path (psdf_cull_kernels.cuh)
   int tune_bd = 0, tune_chunks = 0;   // PSDF_BD / PSDF_CHUNKS, read once at create
   int culling = 0;                    // psdf_set_culling
-  int* d_perm = nullptr;              // [max_poses]
-  int* d_cell = nullptr;              // [kSortGridMax^2 + 1]
-  unsigned int* d_bbox = nullptr;     // [4]
   unsigned long long* d_stats = nullptr;   // [2] psdf_cull_stats
   // host (graph) path
   cudaStream_t gstream = nullptr;
@@ -114,57 +114,42 @@ cudaError_t launch_mode(const psdf_scene* sc, const EvalParams& p, int mode, boo
   }
 }
 
-template <int V>
-cudaError_t launch_cull_mode(const psdf_scene* sc, const EvalParams& p, int mode, dim3 grid, int bd, cudaStream_t st) {
+template <int V, int NP>
+cudaError_t launch_cull_mode(const psdf_scene* sc, const EvalParams& p, int mode, cudaStream_t st) {
+  const dim3 grid((unsigned)((p.N + NP - 1) / NP));
   switch (mode) {
-    case 0: psdf_cull_kernel<V, 0><<<grid, bd, 0, st>>>(sc->fp, p); break;
-    case kGrad: psdf_cull_kernel<V, kGrad><<<grid, bd, 0, st>>>(sc->fp, p); break;
-    case kCoeff: psdf_cull_kernel<V, kCoeff><<<grid, bd, 0, st>>>(sc->fp, p); break;
+    case 0: psdf_cull_kernel<V, 0, NP><<<grid, NP, 0, st>>>(sc->fp, p); break;
+    case kGrad: psdf_cull_kernel<V, kGrad, NP><<<grid, NP, 0, st>>>(sc->fp, p); break;
+    case kCoeff: psdf_cull_kernel<V, kCoeff, NP><<<grid, NP, 0, st>>>(sc->fp, p); break;
     default: return cudaErrorInvalidValue;
   }
   g_launches.fetch_add(1);
   return cudaGetLastError();
 }
 
-cudaError_t launch_cull_v(const psdf_scene* sc, const EvalParams& p, int mode, dim3 grid, int bd, cudaStream_t st) {
+template <int NP>
+cudaError_t launch_cull_v(const psdf_scene* sc, const EvalParams& p, int mode, cudaStream_t st) {
   switch (sc->Vp) {
-    case 4: return launch_cull_mode<4>(sc, p, mode, grid, bd, st);
-    case 6: return launch_cull_mode<6>(sc, p, mode, grid, bd, st);
-    case 8: return launch_cull_mode<8>(sc, p, mode, grid, bd, st);
-    case 10: return launch_cull_mode<10>(sc, p, mode, grid, bd, st);
-    case 12: return launch_cull_mode<12>(sc, p, mode, grid, bd, st);
-    case 16: return launch_cull_mode<16>(sc, p, mode, grid, bd, st);
+    case 4: return launch_cull_mode<4, NP>(sc, p, mode, st);
+    case 6: return launch_cull_mode<6, NP>(sc, p, mode, st);
+    case 8: return launch_cull_mode<8, NP>(sc, p, mode, st);
+    case 10: return launch_cull_mode<10, NP>(sc, p, mode, st);
+    case 12: return launch_cull_mode<12, NP>(sc, p, mode, st);
+    case 16: return launch_cull_mode<16, NP>(sc, p, mode, st);
     default: return cudaErrorInvalidValue;
   }
 }
 
-// Culled path: grid-sort the poses (4 small kernels), then one warp per 32 sorted poses.
+// Culled path: one launch.  Small batches take one warp per CTA so that they
+// still spread over all SMs; large ones 128 poses per CTA (measured: cfg4 133 vs 146 us).
 cudaError_t enqueue_culled(const psdf_scene* sc, EvalParams& p, int mode, cudaStream_t st) {
-  SortParams s{};
-  s.poses = p.poses;
-  s.N = p.N;
-  int G = (int)std::floor(std::sqrt((double)p.N / 32.0));
-  s.G = G < 1 ? 1 : (G > kSortGridMax ? kSortGridMax : G);
-  s.bbox = sc->d_bbox;
-  s.cell = sc->d_cell;
-  s.perm = sc->d_perm;
-  // the sort workspace is clean on entry (create, or the previous culled kernel, cleaned it)
-  const int gd = (p.N + 255) / 256;
-  pose_bbox_kernel<<<gd < 2 * sc->sm_count ? gd : 2 * sc->sm_count, 256, 0, st>>>(s);
-  pose_hist_kernel<<<(p.N + 1023) / 1024, 1024, 0, st>>>(s);
-  pose_scatter_kernel<<<gd, 256, 0, st>>>(s);
-  g_launches.fetch_add(3);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
-  p.perm = sc->d_perm;
-  p.bounds = sc->pk[sc->cur].bounds;
-  p.sort_cell = sc->d_cell;
-  p.sort_bbox = sc->d_bbox;
-  p.sort_cells = s.G * s.G;
+  p.gbounds = sc->pk[sc->cur].gbounds;
+  p.gcell = sc->pk[sc->cur].gcell;
+  p.ghdr = sc->pk[sc->cur].ghdr;
   p.stats = sc->d_stats;
-  const int groups = (p.N + 31) / 32;
   p.n_chunks = 1;
-  return launch_cull_v(sc, p, mode, dim3((unsigned)groups), 32, st);
+  if (p.N <= 32768) return launch_cull_v<32>(sc, p, mode, st);
+  return launch_cull_v<128>(sc, p, mode, st);
 }
 
 cudaError_t launch_v(const psdf_scene* sc, const EvalParams& p, int mode, bool lanes, dim3 grid, int bd,
@@ -295,6 +280,9 @@ psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const
                                          dst.row_begin, sc->d_pair_begin, dst.empty, dst.bounds, dst.row_slot);
     g_launches.fetch_add(3);
   }
+  obstacle_grid_kernel<<<1, 1024, 0, st>>>(dst.bounds, 0, reinterpret_cast<const int*>(sc->d_totals), dst.gbounds,
+                                           dst.gcell, dst.ghdr);
+  g_launches.fetch_add(1);
   CU_TRY(cudaMemcpyAsync(sc->h_totals, sc->d_totals, sizeof(PackTotals) + sizeof(int) * ((size_t)M + 1),
                          cudaMemcpyDeviceToHost, st));
   CU_TRY(cudaStreamSynchronize(st));                         // the only synchronisation of an update
@@ -323,9 +311,11 @@ psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const u
     CU_TRY(cudaMemcpyAsync(dst.pairs, ps.pairs.data(), sizeof(PairRec) * n_pairs, cudaMemcpyHostToDevice, st));
   }
   CU_TRY(cudaMemcpyAsync(dst.row_slot, ps.row_slot.data(), sizeof(int) * (size_t)(sc->M + 1), cudaMemcpyHostToDevice, st));
-  if (Mv) CU_TRY(cudaMemcpyAsync(dst.bounds, ps.bounds.data(), sizeof(float4) * Mv, cudaMemcpyHostToDevice, st));
+  if (Mv) CU_TRY(cudaMemcpyAsync(dst.bounds, ps.bounds.data(), sizeof(float4) * 2 * Mv, cudaMemcpyHostToDevice, st));
   CU_TRY(cudaMemcpyAsync(dst.row_begin, ps.row_begin.data(), sizeof(int) * (Mv + 1), cudaMemcpyHostToDevice, st));
   if (n_empty) CU_TRY(cudaMemcpyAsync(dst.empty, ps.empty_rows.data(), sizeof(int) * n_empty, cudaMemcpyHostToDevice, st));
+  obstacle_grid_kernel<<<1, 1024, 0, st>>>(dst.bounds, Mv, nullptr, dst.gbounds, dst.gcell, dst.ghdr);
+  g_launches.fetch_add(1);
   CU_TRY(cudaStreamSynchronize(st));       // the staging vectors die here
   sc->n_edges = n_edges;
   sc->Mv = Mv;
@@ -348,12 +338,13 @@ void psdf_destroy_scene(psdf_scene* sc) {
   if (sc->gstream) cudaStreamDestroy(sc->gstream);
   for (auto& b : sc->pk) {
     cudaFree(b.edges); cudaFree(b.pairs); cudaFree(b.row_begin); cudaFree(b.row_slot); cudaFree(b.empty); cudaFree(b.bounds);
+    cudaFree(b.gbounds); cudaFree(b.gcell); cudaFree(b.ghdr);
   }
   cudaFree(sc->d_win);
   if (sc->h_totals) cudaFreeHost(sc->h_totals);
   if (sc->h_win) cudaFreeHost(sc->h_win);
   cudaFree(sc->d_ws_depth); cudaFree(sc->d_ws_d2); cudaFree(sc->d_ws_count);
-  cudaFree(sc->d_stats); cudaFree(sc->d_perm); cudaFree(sc->d_cell); cudaFree(sc->d_bbox);
+  cudaFree(sc->d_stats);
   cudaFree(sc->d_cnt); cudaFree(sc->d_offs); cudaFree(sc->d_totals);   // d_pair_begin lives inside d_totals' block
   cudaFree(sc->d_in); cudaFree(sc->d_out); cudaFree(sc->d_per);
   if (sc->h_in) cudaFreeHost(sc->h_in);
@@ -392,7 +383,10 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
       CU_TRY(cudaMalloc(&b.row_begin, sizeof(int) * (size_t)(M + 1)));
       CU_TRY(cudaMalloc(&b.row_slot, sizeof(int) * (size_t)(M + 1)));
       CU_TRY(cudaMalloc(&b.empty, sizeof(int) * (size_t)M));
-      CU_TRY(cudaMalloc(&b.bounds, sizeof(float4) * (size_t)M));
+      CU_TRY(cudaMalloc(&b.bounds, sizeof(float4) * 2 * (size_t)M));
+      CU_TRY(cudaMalloc(&b.gbounds, sizeof(float4) * 2 * (size_t)M));
+      CU_TRY(cudaMalloc(&b.gcell, sizeof(int) * (size_t)(kObsGridMax * kObsGridMax + 1)));
+      CU_TRY(cudaMalloc(&b.ghdr, sizeof(GridHdr)));
     }
     CU_TRY(cudaMallocHost(&sc->h_totals, sizeof(PackTotals) + sizeof(int) * (size_t)(M + 1)));
     sc->h_pair_begin_pinned = reinterpret_cast<int*>(sc->h_totals + 1);
@@ -400,17 +394,8 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
     CU_TRY(cudaMalloc(&sc->d_offs, sizeof(int4) * (size_t)M));
     CU_TRY(cudaMalloc(&sc->d_totals, sizeof(PackTotals) + sizeof(int) * (size_t)(M + 1)));
     sc->d_pair_begin = reinterpret_cast<int*>(sc->d_totals + 1);
-    CU_TRY(cudaMalloc(&sc->d_perm, sizeof(int) * (size_t)max_poses));
-    CU_TRY(cudaMalloc(&sc->d_cell, sizeof(int) * (size_t)(kSortGridMax * kSortGridMax + 1)));
-    CU_TRY(cudaMalloc(&sc->d_bbox, sizeof(unsigned int) * 4));
-#ifdef PSDF_CULL_LOG
-    CU_TRY(cudaMalloc(&sc->d_stats, sizeof(unsigned long long) * (2 + 4 * (size_t)(max_poses / 32 + 1))));
-#else
     CU_TRY(cudaMalloc(&sc->d_stats, sizeof(unsigned long long) * 2));
-#endif
     CU_TRY(cudaMemsetAsync(sc->d_stats, 0, sizeof(unsigned long long) * 2, st));
-    CU_TRY(cudaMemsetAsync(sc->d_cell, 0x00, sizeof(int) * (size_t)(kSortGridMax * kSortGridMax + 1), st));
-    CU_TRY(cudaMemsetAsync(sc->d_bbox, 0xff, sizeof(unsigned int) * 4, st));
     CU_TRY(cudaMalloc(&sc->d_ws_depth, sizeof(unsigned long long) * (size_t)max_poses));
     CU_TRY(cudaMalloc(&sc->d_ws_d2, sizeof(unsigned long long) * (size_t)max_poses));
     const size_t n_cnt = (size_t)max_poses + 1;          // scan: one per pose tile; lanes: one per pose group
@@ -665,16 +650,6 @@ psdf_status psdf_trajectory_reduce(const float* value, int T, int H, float d_saf
 psdf_status psdf_cull_stats(psdf_scene* sc, void* cuda_stream, unsigned long long* out2) {
   if (!sc || !out2) return PSDF_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-#ifdef PSDF_CULL_LOG
-  if (const char* f = std::getenv("PSDF_CULL_LOG_FILE")) {
-    const size_t n = 2 + 4 * (size_t)(sc->max_poses / 32 + 1);
-    std::vector<unsigned long long> h(n);
-    cudaMemcpy(h.data(), sc->d_stats, n * 8, cudaMemcpyDeviceToHost);
-    FILE* fp = std::fopen(f, "wb");
-    std::fwrite(h.data(), 8, n, fp);
-    std::fclose(fp);
-  }
-#endif
   CU_TRY(cudaMemcpyAsync(out2, sc->d_stats, sizeof(unsigned long long) * 2, cudaMemcpyDeviceToHost, st));
   CU_TRY(cudaMemsetAsync(sc->d_stats, 0, sizeof(unsigned long long) * 2, st));
   CU_TRY(cudaStreamSynchronize(st));

@@ -1,285 +1,351 @@
 // Exact broad-phase culling (beyond the paper).  phi is a minimum
-// over obstacles (eq.(6)), so an obstacle whose lower bound
-//     sd^i >= |p - c_i| - R_i - r_max          (bounding circles of obstacle and footprint)
-// exceeds an upper bound of phi already in hand cannot be the arg-min and cannot change the
-// value: skipping it is exact.  The culled path evaluates every surviving (pose, obstacle)
-// pair with the same arithmetic as the dense tile-scan kernel (edge_step2), so its outputs
-// are bit-identical to the dense path.
-//
-//   * poses are bucketed into a uniform grid (counting sort: bbox -> histogram -> scan ->
-//     scatter) so that the 32 poses of a warp are spatially close;
-//   * one warp owns 32 sorted poses and walks the obstacle bounds 32 at a time: lane j tests
-//     obstacle j against the warp's pose box and its largest running upper bound (one test per
-//     obstacle per WARP), the ballot gives the survivors, each survivor is re-tested per lane
-//     and evaluated only if some lane still needs it; records are read straight from L2/L1
-//     with warp-uniform 128-bit loads (no shared memory, no block barriers);
-//   * the running upper bound is the exact value over the obstacles evaluated so far.
+// over obstacles (eq.(6)), so an obstacle whose lower bound on sd^i exceeds an
+// upper bound of phi already in hand cannot be the arg-min and cannot change the value:
+// skipping it is exact.  Two lower bounds are used, cheapest first:
+//     sd^i >= |c_R - c_i| - R_i - r_R            (bounding circles of obstacle and footprint)
+//     sd^i >= sd(box_R, box_i)                   (oriented bounding boxes, separating axes)
+// Every surviving (pose, obstacle) pair is evaluated with the same arithmetic as the dense
+// tile-scan kernel (edge_step2) and reduced with the same keys, so the outputs are
+// bit-identical to the dense path.
 #pragma once
 #include "psdf_kernels.cuh"
 
 namespace psdf {
 
-constexpr int kSortGridMax = 64;      // pose grid is G x G cells, G <= 64
-
 __device__ __forceinline__ float warp_min_f(float v) { return fkey_inv(__reduce_min_sync(0xffffffffu, fkey(v))); }
 __device__ __forceinline__ float warp_max_f(float v) { return fkey_inv(__reduce_max_sync(0xffffffffu, fkey(v))); }
 
-struct SortParams {
-  const float* poses;
-  int N, G;
-  unsigned int* bbox;      // [4] ordered keys: min x, min y, ~max x, ~max y  (all atomicMin; clean = 0xff..)
-  int* cell;               // [G*G + 1] histogram -> offsets -> cursors
-  int* perm;               // [N] sorted position -> pose index
+// ------------------------------------------------------------------------------------------
+// Obstacle grid: the bounds re-ordered by cell of a G x G grid over the obstacle centres
+// (row-major: a rectangle of cells is one contiguous range of `gbounds` per grid row), built on
+// the device after every pack (host or device packer) by one CTA.
+struct GridHdr {
+  float x0, y0, sx, sy;    // cell(x) = clamp((int)((x - x0) * sx), 0, G-1)
+  float rmax;              // largest bounding-circle radius
+  float cell;              // larger cell edge [m]
+  int G, Mv;
 };
+constexpr int kObsGridMax = 64;
 
-__device__ __forceinline__ bool pose_finite(float x, float y) { return isfinite(x) && isfinite(y); }
-
-__global__ void __launch_bounds__(256) pose_bbox_kernel(const SortParams s) {
-  __shared__ float red[4][8];
-  float x0 = kInf, y0 = kInf, x1 = -kInf, y1 = -kInf;
-  for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < s.N; n += gridDim.x * blockDim.x) {
-    const float x = __ldg(s.poses + 3 * n), y = __ldg(s.poses + 3 * n + 1);
-    if (pose_finite(x, y)) { x0 = fminf(x0, x); y0 = fminf(y0, y); x1 = fmaxf(x1, x); y1 = fmaxf(y1, y); }
-  }
-  x0 = warp_min_f(x0); y0 = warp_min_f(y0); x1 = warp_max_f(x1); y1 = warp_max_f(y1);
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  if (lane == 0) { red[0][wid] = x0; red[1][wid] = y0; red[2][wid] = x1; red[3][wid] = y1; }
-  __syncthreads();
-  if (wid == 0) {                                         // one atomic per quantity per block
-    const int nw = blockDim.x >> 5;
-    x0 = warp_min_f(lane < nw ? red[0][lane] : kInf); y0 = warp_min_f(lane < nw ? red[1][lane] : kInf);
-    x1 = warp_max_f(lane < nw ? red[2][lane] : -kInf); y1 = warp_max_f(lane < nw ? red[3][lane] : -kInf);
-    if (lane == 0) {
-      atomicMin(s.bbox + 0, fkey(x0)); atomicMin(s.bbox + 1, fkey(y0));
-      atomicMin(s.bbox + 2, ~fkey(x1)); atomicMin(s.bbox + 3, ~fkey(y1));
-    }
-  }
+__device__ __forceinline__ int grid_coord(float v, float v0, float s, int G) {
+  return min(max((int)((v - v0) * s), 0), G - 1);      // monotone non-decreasing in v
 }
 
-__device__ __forceinline__ int pose_cell(const SortParams& s, int n) {
-  const float x = __ldg(s.poses + 3 * n), y = __ldg(s.poses + 3 * n + 1);
-  if (!pose_finite(x, y)) return 0;
-  const float x0 = fkey_inv(s.bbox[0]), y0 = fkey_inv(s.bbox[1]);
-  const float x1 = fkey_inv(~s.bbox[2]), y1 = fkey_inv(~s.bbox[3]);
-  const float sx = (float)s.G / fmaxf(x1 - x0, 1e-6f), sy = (float)s.G / fmaxf(y1 - y0, 1e-6f);
-  const int gx = min(max((int)((x - x0) * sx), 0), s.G - 1);
-  int gy = min(max((int)((y - y0) * sy), 0), s.G - 1);
-  if (gx & 1) gy = s.G - 1 - gy;                          // snake order: neighbours stay neighbours
-  return gx * s.G + gy;
-}
-
-// exclusive scan of the (<= 4096) cell counts, in place, by one CTA of 1024 threads
-__device__ __forceinline__ void scan_cells(int* cell, int cells) {
+// totals2 = {status, Mv} written by the device packer (or null: Mv_host is used)
+__global__ void __launch_bounds__(1024) obstacle_grid_kernel(const float4* __restrict__ bounds, int Mv_host,
+                                                             const int* __restrict__ totals2,
+                                                             float4* __restrict__ gbounds, int* __restrict__ gcell,
+                                                             GridHdr* __restrict__ hdr) {
+  __shared__ int cnt[kObsGridMax * kObsGridMax + 1];
+  __shared__ float red[5][32];
   __shared__ int wsum[32];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  int v[4], sum = 0;
-#pragma unroll
-  for (int k = 0; k < 4; ++k) { const int c = 4 * tid + k; v[k] = c < cells ? __ldcg(cell + c) : 0; sum += v[k]; }
-  int inc = sum;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
-  if (lane == 31) wsum[wid] = inc;
+  const int Mv = totals2 ? (totals2[0] == 0 ? totals2[1] : 0) : Mv_host;
+  float x0 = kInf, y0 = kInf, x1 = -kInf, y1 = -kInf, rm = 0.f;
+  for (int i = tid; i < Mv; i += 1024) {
+    const float4 b = bounds[2 * i];
+    x0 = fminf(x0, b.x); y0 = fminf(y0, b.y); x1 = fmaxf(x1, b.x); y1 = fmaxf(y1, b.y); rm = fmaxf(rm, b.z);
+  }
+  x0 = warp_min_f(x0); y0 = warp_min_f(y0); x1 = warp_max_f(x1); y1 = warp_max_f(y1); rm = warp_max_f(rm);
+  if (lane == 0) { red[0][wid] = x0; red[1][wid] = y0; red[2][wid] = x1; red[3][wid] = y1; red[4][wid] = rm; }
   __syncthreads();
-  if (wid == 0) {
-    const int w = wsum[lane];
-    int winc = w;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += t; }
-    wsum[lane] = winc - w;
+  x0 = warp_min_f(red[0][lane]); y0 = warp_min_f(red[1][lane]);
+  x1 = warp_max_f(red[2][lane]); y1 = warp_max_f(red[3][lane]); rm = warp_max_f(red[4][lane]);
+  int G = (int)sqrtf(0.5f * (float)Mv);
+  G = G < 1 ? 1 : (G > kObsGridMax ? kObsGridMax : G);
+  const float wx = fmaxf(x1 - x0, 1e-6f), wy = fmaxf(y1 - y0, 1e-6f);
+  const float sx = (float)G / wx, sy = (float)G / wy;
+  const int cells = G * G;
+  for (int c = tid; c <= cells; c += 1024) cnt[c] = 0;
+  __syncthreads();
+  for (int i = tid; i < Mv; i += 1024) {
+    const float4 b = bounds[2 * i];
+    atomicAdd(&cnt[grid_coord(b.y, y0, sy, G) * G + grid_coord(b.x, x0, sx, G)], 1);
   }
   __syncthreads();
-  int run = wsum[wid] + inc - sum;
+  {  // exclusive scan of cnt[0..cells) in place, four cells per thread
+    int v[4], sum = 0;
 #pragma unroll
-  for (int k = 0; k < 4; ++k) { const int c = 4 * tid + k; if (c < cells) cell[c] = run; run += v[k]; }
-}
-
-// histogram of the pose cells; the last block to arrive turns the counts into offsets
-// (cell[G*G] is the arrival counter).  block = 1024 threads.
-__global__ void __launch_bounds__(1024) pose_hist_kernel(const SortParams s) {
-  __shared__ int is_last;
-  const int n = blockIdx.x * blockDim.x + threadIdx.x;
-  {  // warp-aggregated: neighbouring poses (same trajectory) share a cell, one atomic per distinct cell
-    const int c = n < s.N ? pose_cell(s, n) : -1;
-    const unsigned peers = __match_any_sync(0xffffffffu, c);
-    if (c >= 0 && (int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) atomicAdd(s.cell + c, __popc(peers));
+    for (int k = 0; k < 4; ++k) { const int c = 4 * tid + k; v[k] = c < cells ? cnt[c] : 0; sum += v[k]; }
+    int inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+    if (lane == 31) wsum[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+      const int w = wsum[lane];
+      int winc = w;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += t; }
+      wsum[lane] = winc - w;
+    }
+    __syncthreads();
+    int run = wsum[wid] + inc - sum;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int c = 4 * tid + k;
+      if (c < cells) { cnt[c] = run; gcell[c] = run; }
+      run += v[k];
+    }
+    if (tid == 0) gcell[cells] = Mv;
   }
-  __threadfence();
   __syncthreads();
-  if (threadIdx.x == 0) is_last = atomicAdd(s.cell + s.G * s.G, 1) == (int)gridDim.x - 1;
+  for (int i = tid; i < Mv; i += 1024) {                   // scatter (cnt = cursors)
+    const float4 b = bounds[2 * i];
+    const int pos = atomicAdd(&cnt[grid_coord(b.y, y0, sy, G) * G + grid_coord(b.x, x0, sx, G)], 1);
+    gbounds[pos] = b;
+    gbounds[Mv + pos] = bounds[2 * i + 1];
+  }
   __syncthreads();
-  if (!is_last) return;
-  __threadfence();
-  scan_cells(s.cell, s.G * s.G);
+  // deterministic order inside a cell (by first pair record = packed order): after the scatter
+  // cnt[c] is the END of cell c, its begin is the end of cell c-1
+  for (int c = tid; c < cells; c += 1024) {
+    const int b0 = c ? cnt[c - 1] : 0, b1 = cnt[c];
+    for (int i = b0 + 1; i < b1; ++i) {
+      const float4 key = gbounds[i], key2 = gbounds[Mv + i];
+      int j = i - 1;
+      while (j >= b0 && __float_as_int(gbounds[j].w) > __float_as_int(key.w)) {
+        gbounds[j + 1] = gbounds[j];
+        gbounds[Mv + j + 1] = gbounds[Mv + j];
+        --j;
+      }
+      gbounds[j + 1] = key;
+      gbounds[Mv + j + 1] = key2;
+    }
+  }
+  if (tid == 0) {
+    GridHdr h;
+    h.x0 = x0; h.y0 = y0; h.sx = sx; h.sy = sy; h.rmax = rm;
+    h.cell = fmaxf(wx, wy) / (float)G;
+    h.G = G; h.Mv = Mv;
+    *hdr = h;
+  }
 }
 
-__global__ void pose_scatter_kernel(const SortParams s) {
-  const int n = blockIdx.x * blockDim.x + threadIdx.x;
-  const int lane = threadIdx.x & 31;
-  const int c = n < s.N ? pose_cell(s, n) : -1;
-  const unsigned peers = __match_any_sync(0xffffffffu, c);          // warp-aggregated cursor bump
-  const int leader = __ffs(peers) - 1;
-  int base = 0;
-  if (c >= 0 && leader == lane) base = atomicAdd(s.cell + c, __popc(peers));
-  base = __shfl_sync(0xffffffffu, base, leader);
-  if (c >= 0) s.perm[base + __popc(peers & ((1u << lane) - 1u))] = n;
-}
 
-// Per-obstacle bound, one float4 per packed obstacle: bounding circle (cx, cy, R) of its
-// vertices and the index of its first pair record (int bits).
-//
-// Culled evaluation: one warp (= one CTA) per 32 sorted poses, lane = pose.  MODE in
-// {0, kGrad, kCoeff}.  The workspace left dirty by the pose sort is cleaned here for the next
-// call.  (Several warps per pose group sharing the running bound were measured: never faster.)
-template <int V, int MODE>
-__global__ void __launch_bounds__(32) psdf_cull_kernel(const __grid_constant__ Footprint fp,
+// ------------------------------------------------------------------------------------------
+// Culled evaluation over the obstacle grid, pair-queue formulation.  CTA = NP poses, one per
+// thread.  Every thread walks the grid cells around ITS pose and pushes the
+// obstacles that pass the bounding-circle test as (pose, obstacle) pairs into a shared-memory
+// queue; the CTA then evaluates the queued pairs one per lane, whatever pose they belong to
+// (the posed footprints sit in shared memory), with the dense kernel's arithmetic (edge_step2),
+// and folds each result into its pose's 64-bit arg-max / arg-min keys with shared-memory
+// atomics (same keys as the dense kernel: lowest slot on ties).  Two rounds: a seed round (one
+// near obstacle per pose) gives every pose a finite upper bound, the main round queues whatever
+// that bound cannot exclude.  The last step is the dense kernel's tail (finalize_pose).
+template <int V>
+struct __align__(16) PosedSlot {      // one posed footprint in shared memory
+  float2 rx[V / 2], ry[V / 2], Tx[V / 2], Ty[V / 2];
+  float px, py, ub, pad;
+};
+
+// NP = poses (= threads) per CTA; NP = 32 makes every warp an independent unit (no block barriers)
+template <int V, int MODE, int NP>
+__global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ Footprint fp,
                                                         const __grid_constant__ EvalParams p) {
-  const int lane = threadIdx.x & 31;
-#ifdef PSDF_CULL_LOG
-  const long long t_start = clock64();
-#endif
-  {  // clean the sort workspace (its last reader, pose_scatter_kernel, has completed)
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t <= p.sort_cells) p.sort_cell[t] = 0;
-    if (t < 4) p.sort_bbox[t] = 0xffffffffu;
-  }
-  const int k = blockIdx.x * 32 + lane;
-  const int n = __ldg(p.perm + min(k, p.N - 1));           // tail lanes recompute the last pose
+  constexpr int kCullQueue = (NP * 16 * (int)sizeof(int2) + NP * (int)sizeof(PosedSlot<V>) > 44 * 1024) ? NP * 8 : NP * 16;
+  __shared__ PosedSlot<V> s_pose[NP];
+  __shared__ unsigned long long s_kd[NP], s_k2[NP];
+  __shared__ int2 s_queue[kCullQueue];
+  __shared__ int s_count;
+  __shared__ unsigned int s_stat[2];
+  const int tid = threadIdx.x;
+  const int k = blockIdx.x * NP + tid;
+  const int n = min(k, p.N - 1);                           // tail threads recompute the last pose
   const float x = __ldg(p.poses + 3 * n), y = __ldg(p.poses + 3 * n + 1), th = __ldg(p.poses + 3 * n + 2);
-  const bool finite = isfinite(x) && isfinite(y) && isfinite(th);
-  Posed2<V> P;
-  pose_setup2<V>(fp, x, y, th, P);
-  // pose box of the 32 poses (non-finite poses take no part; they are finalised to NaN)
-  const float xmin = warp_min_f(finite ? x : kInf), xmax = warp_max_f(finite ? x : -kInf);
-  const float ymin = warp_min_f(finite ? y : kInf), ymax = warp_max_f(finite ? y : -kInf);
-  const float rpad = fp.rmax * 1.0001f + 1e-4f;            // footprint radius + safety for fp32 rounding
-
-  ObstacleAcc<V> acc;
-  float minD2 = kInf, prevD2 = kInf, maxDepth = -kInf;
-  float ub = finite ? kInf : -kInf;                        // running upper bound of phi for this lane
-  int idD2 = -1, idDepth = -1;
-  unsigned n_visit = 0, n_edge = 0;                        // statistics (psdf_cull_stats)
-  const float4* __restrict__ bounds = p.bounds;
-  const float4* __restrict__ recs = reinterpret_cast<const float4*>(p.pairs);
-
-  // evaluates one obstacle for the whole warp if some lane still needs it (exact per-lane test)
-  auto visit = [&](const float cx, const float cy, const float R, const int rec) {
-    const float dx = cx - x, dy = cy - y;
-    const float t = (ub + R) * 1.0001f + rpad;
-    const bool need = !((t < 0.f) || (fmaf(dx, dx, dy * dy) > t * t));
-    if (!__any_sync(0xffffffffu, need)) return;
-    acc.reset();
-    const float4* src = recs + 3 * (size_t)rec;
-    float4 q0 = __ldg(src), q1 = __ldg(src + 1), q2 = __ldg(src + 2);
-    int last, slot;
-    while (true) {
-      last = __float_as_int(q2.z);
-      slot = __float_as_int(q2.w);
-      const float4 c0 = q0, c1 = q1;
-      const float h0 = q2.x, h1 = q2.y;
-      if (last < 0) {                                      // prefetch the next record of this obstacle
-        src += 3;
-        q0 = __ldg(src); q1 = __ldg(src + 1); q2 = __ldg(src + 2);
-      }
-      edge_step2<V>(fp, P, c0, h0, acc, minD2);
-      if (h1 >= 0.f) edge_step2<V>(fp, P, c1, h1, acc, minD2);
-      n_edge += h1 >= 0.f ? 2u : 1u;
-      if (last >= 0) break;
-    }
-    ++n_visit;
-    const float depth = acc.depth();
-    if (MODE & (kGrad | kCoeff)) {
-      if (minD2 < prevD2) { prevD2 = minD2; idD2 = slot; }
-    }
-    if (depth > maxDepth) { maxDepth = depth; idDepth = slot; }
-    if (finite) {
-      const float nub = fminf(ub, maxDepth >= 0.f ? -maxDepth : sqrtf(minD2));
-      ub = nub;
-    }
-  };
-  // squared distance from an obstacle centre to the pose box of the warp
-  auto box_d2 = [&](const float4 b) {
-    const float ddx = fmaxf(fmaxf(xmin - b.x, b.x - xmax), 0.f), ddy = fmaxf(fmaxf(ymin - b.y, b.y - ymax), 0.f);
-    return fmaf(ddx, ddx, ddy * ddy);
-  };
-
-  // Phase A: the two obstacles nearest to the pose box go first, so that the running upper
-  // bound is tight before the memory-order walk (evaluated obstacles per warp drop ~2x).
-  int first0 = -1, first1 = -1;
+  const bool active = k < p.N && isfinite(x) && isfinite(y) && isfinite(th);
+  float sn, cs;
+  sincosf(th, &sn, &cs);
   {
-    unsigned k0 = 0xffffffffu, k1 = 0xffffffffu;           // this lane's two smallest keys
-    int i0 = -1, i1 = -1;
-    // (ordering heuristic only: squared box distance minus squared radius, no sqrt)
-#pragma unroll 4
-    for (int i = lane; i < p.Mv; i += 32) {
-      const float4 b = __ldg(bounds + i);
-      const unsigned key = fkey(box_d2(b) - b.z * b.z);
-      if (key < k0) { k1 = k0; i1 = i0; k0 = key; i0 = i; }
-      else if (key < k1) { k1 = key; i1 = i; }
-    }
+    Posed2<V> P;
+    pose_setup2_sc<V>(fp, x, y, sn, cs, P);
+    PosedSlot<V>& d = s_pose[tid];
 #pragma unroll
-    for (int r = 0; r < 2; ++r) {
-      const unsigned m = __reduce_min_sync(0xffffffffu, k0);
-      const int owner = __ffs(__ballot_sync(0xffffffffu, k0 == m && i0 >= 0)) - 1;
-      if (owner < 0) break;
-      const int idx = __shfl_sync(0xffffffffu, i0, owner);
-      if (lane == owner) { k0 = k1; i0 = i1; k1 = 0xffffffffu; i1 = -1; }
-      if (r == 0) first0 = idx; else first1 = idx;
-      const float4 b = __ldg(bounds + idx);
-      visit(b.x, b.y, b.z, __float_as_int(b.w));
+    for (int l = 0; l < V / 2; ++l) { d.rx[l] = P.rx[l]; d.ry[l] = P.ry[l]; d.Tx[l] = P.Tx[l]; d.Ty[l] = P.Ty[l]; }
+    d.px = x; d.py = y;
+  }
+  s_kd[tid] = 0ull;
+  s_k2[tid] = ~0ull;
+  if (tid == 0) { s_count = 0; s_stat[0] = 0u; s_stat[1] = 0u; }
+  __syncthreads();
+  // broad-phase proxies of the posed footprint: its bounding box (centre bx,by; axes (cs,sn),
+  // (-sn,cs); half extents fp.bhx, fp.bhy) and the circle of radius fp.rbox around the box centre
+  const float bx = fmaf(cs, fp.bcx, fmaf(-sn, fp.bcy, x)), by = fmaf(sn, fp.bcx, fmaf(cs, fp.bcy, y));
+  const float rpad = fp.rbox * 1.0001f + 1e-4f;            // footprint radius + safety for fp32 rounding
+  const GridHdr gh = *p.ghdr;
+  const int G = gh.G;
+  const float4* __restrict__ gcirc = p.gbounds;            // (cx, cy, R, first pair record), grid order
+  const float4* __restrict__ gobb = p.gbounds + gh.Mv;     // (ux, uy, hx, hy), grid order
+  const int* __restrict__ gcell = p.gcell;
+  const float4* __restrict__ recs = reinterpret_cast<const float4*>(p.pairs);
+  unsigned n_pair = 0, n_edge = 0;
+
+  // evaluates the first nq queued pairs, one per lane
+  auto drain = [&](int nq) {
+    for (int j = tid; j < nq; j += NP) {
+      const int2 pr = s_queue[j];
+      const PosedSlot<V>& sp = s_pose[pr.x];
+      Posed2<V> P;
+#pragma unroll
+      for (int l = 0; l < V / 2; ++l) { P.rx[l] = sp.rx[l]; P.ry[l] = sp.ry[l]; P.Tx[l] = sp.Tx[l]; P.Ty[l] = sp.Ty[l]; }
+      P.px = sp.px; P.py = sp.py;
+      ObstacleAcc<V> acc;
+      acc.reset();
+      float minD2 = kInf;
+      const float4* src = recs + 3 * (size_t)pr.y;
+      float4 q0 = __ldg(src), q1 = __ldg(src + 1), q2 = __ldg(src + 2);
+      int last, slot;
+      while (true) {
+        last = __float_as_int(q2.z);
+        slot = __float_as_int(q2.w);
+        const float4 c0 = q0, c1 = q1;
+        const float h0 = q2.x, h1 = q2.y;
+        if (last < 0) {                                    // prefetch the next record of this obstacle
+          src += 3;
+          q0 = __ldg(src); q1 = __ldg(src + 1); q2 = __ldg(src + 2);
+        }
+        edge_step2<V>(fp, P, c0, h0, acc, minD2);
+        if (h1 >= 0.f) edge_step2<V>(fp, P, c1, h1, acc, minD2);
+        n_edge += h1 >= 0.f ? 2u : 1u;
+        if (last >= 0) break;
+      }
+      ++n_pair;
+      const float depth = acc.depth();
+      atomicMax(&s_kd[pr.x], ((unsigned long long)fkey(depth) << 32) | (0xffffffffu - (unsigned)slot));
+      atomicMin(&s_k2[pr.x], ((unsigned long long)__float_as_uint(minD2) << 32) | (unsigned)slot);
     }
+  };
+  // this pose's upper bound of phi from its keys
+  auto bound_now = [&]() {
+    const unsigned long long kd = s_kd[tid], k2 = s_k2[tid];
+    const float depth = kd ? fkey_inv((uint32_t)(kd >> 32)) : -kInf;
+    const float d2 = (k2 != ~0ull) ? __uint_as_float((uint32_t)(k2 >> 32)) : kInf;
+    return depth >= 0.f ? -depth : sqrtf(d2);
+  };
+
+  // ---- seed round: the entry with the smallest (d^2 - R^2) in a growing rectangle of cells
+  int seed_rec = -1;
+  if (active) {
+    float ext = rpad + 0.5f * gh.cell;
+    int px0 = 0, px1 = -1, py0 = 0, py1 = -1;
+    float best = kInf;
+    auto scan = [&](int s, int e) {                        // four independent loads in flight
+      for (int i = s; i < e; i += 4) {
+        float4 b[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) b[u] = __ldg(gcirc + min(i + u, e - 1));
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const float dx = b[u].x - bx, dy = b[u].y - by;
+          const float key = fmaf(dx, dx, fmaf(dy, dy, -b[u].z * b[u].z));
+          if (key < best) { best = key; seed_rec = __float_as_int(b[u].w); }   // (a repeated last entry is harmless)
+        }
+      }
+    };
+    while (true) {
+      const int cx0 = grid_coord(bx - ext, gh.x0, gh.sx, G), cx1 = grid_coord(bx + ext, gh.x0, gh.sx, G);
+      const int cy0 = grid_coord(by - ext, gh.y0, gh.sy, G), cy1 = grid_coord(by + ext, gh.y0, gh.sy, G);
+      for (int row = cy0; row <= cy1; ++row) {
+        const int s = __ldg(gcell + row * G + cx0), e = __ldg(gcell + row * G + cx1 + 1);
+        if (row >= py0 && row <= py1) {                    // skip what the previous rectangle covered
+          scan(s, __ldg(gcell + row * G + px0));
+          scan(__ldg(gcell + row * G + px1 + 1), e);
+        } else {
+          scan(s, e);
+        }
+      }
+      if (seed_rec >= 0 || (cx0 == 0 && cy0 == 0 && cx1 == G - 1 && cy1 == G - 1)) break;
+      px0 = cx0; px1 = cx1; py0 = cy0; py1 = cy1;
+      ext *= 2.f;
+    }
+  }
+  if (seed_rec >= 0) s_queue[atomicAdd(&s_count, 1)] = make_int2(tid, seed_rec);
+  __syncthreads();
+  drain(s_count);
+  __syncthreads();
+  if (tid == 0) s_count = 0;
+  __syncthreads();
+
+  // ---- main round: everything the seed bound cannot exclude, resumable when the queue fills
+  const float ub = active ? bound_now() : -kInf;
+  const float need = (ub + gh.rmax) * 1.0001f + rpad;
+  const float ub_pad = fmaf(fabsf(ub), 1e-4f, ub) + 2e-4f;
+  bool done = !active || !(need >= 0.f);
+  int cx0 = 0, cx1 = 0, cy1 = -1, row = 0, i = 0, e = 0;
+  if (!done) {
+    cx0 = grid_coord(bx - need, gh.x0, gh.sx, G); cx1 = grid_coord(bx + need, gh.x0, gh.sx, G);
+    row = grid_coord(by - need, gh.y0, gh.sy, G) - 1; cy1 = grid_coord(by + need, gh.y0, gh.sy, G);
+  }
+  while (true) {
+    while (!done) {
+      if (i >= e) {
+        if (++row > cy1) { done = true; break; }
+        i = __ldg(gcell + row * G + cx0);
+        e = __ldg(gcell + row * G + cx1 + 1);
+        continue;
+      }
+      float4 b[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) b[u] = __ldg(gcirc + min(i + u, e - 1));   // four independent loads in flight
+      bool full = false;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (full || i + u >= e) continue;
+        const float dx = b[u].x - bx, dy = b[u].y - by;
+        const float t = (ub + b[u].z) * 1.0001f + rpad;
+        if ((t < 0.f) || (fmaf(dx, dx, dy * dy) > t * t) || __float_as_int(b[u].w) == seed_rec) continue;
+        // box-box separating-axis bound: sd(boxes) = max over the four box axes of the gap of the
+        // projections (exact when they overlap, a lower bound of the distance otherwise), and
+        // sd(footprint, obstacle) >= sd(boxes) because each polygon lies inside its box
+        const float4 o = __ldg(gobb + i + u);              // (ux, uy, hx, hy)
+        const float a1 = fabsf(fmaf(o.x, cs, o.y * sn)), a2 = fabsf(fmaf(o.y, cs, -o.x * sn));
+        const float g0 = fabsf(fmaf(dx, o.x, dy * o.y)) - (o.z + fmaf(fp.bhx, a1, fp.bhy * a2));
+        const float g1 = fabsf(fmaf(dy, o.x, -dx * o.y)) - (o.w + fmaf(fp.bhx, a2, fp.bhy * a1));
+        const float g2 = fabsf(fmaf(dx, cs, dy * sn)) - (fp.bhx + fmaf(o.z, a1, o.w * a2));
+        const float g3 = fabsf(fmaf(dy, cs, -dx * sn)) - (fp.bhy + fmaf(o.z, a2, o.w * a1));
+        if (fmaxf(fmaxf(g0, g1), fmaxf(g2, g3)) > ub_pad) continue;
+        const int at = atomicAdd(&s_count, 1);
+        if (at >= kCullQueue) { full = true; i += u; continue; }   // queue full: retry this entry next round
+        s_queue[at] = make_int2(tid, __float_as_int(b[u].w));
+      }
+      if (full) break;
+      i += 4;
+    }
+    __syncthreads();
+    const int nq = min(s_count, kCullQueue);
+    drain(nq);
+    __syncthreads();
+    if (tid == 0) s_count = 0;
+    if (__syncthreads_and(done)) break;
   }
 
-#ifdef PSDF_CULL_LOG
-  const long long t_phaseA = clock64();
-#endif
-  // Phase B: memory-order walk, 4 x 32 obstacles per step (four independent loads, tests and
-  // ballots in flight: the walk is latency bound): one box test per obstacle per warp.  A
-  // survivor of a stale warp-level bound is still re-tested per lane inside visit().
-  for (int base = 0; base < p.Mv; base += 128) {
-    float4 b[4];
-    unsigned mask[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int i = base + 32 * u + lane;
-      b[u] = i < p.Mv ? __ldg(bounds + i) : make_float4(0.f, 0.f, 0.f, 0.f);
-    }
-    const float ubmax = warp_max_f(ub);
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int i = base + 32 * u + lane;
-      const float thr = (ubmax + b[u].z) * 1.0001f + rpad;
-      const bool skip = (i >= p.Mv) || (i == first0) || (i == first1) || (thr < 0.f) || (box_d2(b[u]) > thr * thr);
-      mask[u] = __ballot_sync(0xffffffffu, !skip);
-    }
-    if ((mask[0] | mask[1] | mask[2] | mask[3]) == 0u) continue;
-#pragma unroll 1
-    for (int u = 0; u < 4; ++u) {
-      const float4 bu = u == 0 ? b[0] : (u == 1 ? b[1] : (u == 2 ? b[2] : b[3]));
-      unsigned m = u == 0 ? mask[0] : (u == 1 ? mask[1] : (u == 2 ? mask[2] : mask[3]));
-      while (m) {
-        const int j = __ffs(m) - 1;
-        m &= m - 1;
-        visit(__shfl_sync(0xffffffffu, bu.x, j), __shfl_sync(0xffffffffu, bu.y, j), __shfl_sync(0xffffffffu, bu.z, j),
-              __shfl_sync(0xffffffffu, __float_as_int(bu.w), j));
-      }
+  if (p.stats) {
+    atomicAdd(&s_stat[0], n_pair);
+    atomicAdd(&s_stat[1], n_edge);
+    __syncthreads();
+    if (tid == 0) {
+      atomicAdd(p.stats, (unsigned long long)s_stat[0]);
+      atomicAdd(p.stats + 1, (unsigned long long)s_stat[1]);
     }
   }
-#ifdef PSDF_CULL_LOG
-  if (p.stats && lane == 0) {   // per-warp log after the two counters: (cycles, visits, tA, tB)
-    unsigned long long* lg = p.stats + 2 + 4 * (size_t)blockIdx.x;
-    lg[0] = clock64() - t_start; lg[1] = n_visit; lg[2] = t_phaseA - t_start; lg[3] = clock64() - t_phaseA;
-  }
-#endif
-  if (p.stats && lane == 0) {
-    atomicAdd(p.stats, (unsigned long long)n_visit);
-    atomicAdd(p.stats + 1, (unsigned long long)n_edge);
-  }
-  if (!(MODE & (kGrad | kCoeff))) idD2 = minD2 < kInf ? 0 : -1;
   if (k >= p.N) return;
+  const unsigned long long kd = s_kd[tid], k2 = s_k2[tid];
+  const float maxDepth = kd ? fkey_inv((uint32_t)(kd >> 32)) : -kInf;
+  const int idDepth = kd ? (int)(0xffffffffu - (uint32_t)kd) : -1;
+  const float minD2 = (k2 != ~0ull) ? __uint_as_float((uint32_t)(k2 >> 32)) : kInf;
+  const int idD2 = (k2 != ~0ull) ? (int)(uint32_t)k2 : -1;
   const bool separated = !(maxDepth >= 0.f);
   const float value = separated ? sqrtf(minD2) : -maxDepth;
   Posed<V> Ps;
-  unpack_pose<V>(P, Ps);
+  {
+    const PosedSlot<V>& sp = s_pose[tid];
+    Ps.px = x; Ps.py = y;
+#pragma unroll
+    for (int l = 0; l < V / 2; ++l) {
+      Ps.rx[2 * l] = sp.rx[l].x; Ps.rx[2 * l + 1] = sp.rx[l].y; Ps.ry[2 * l] = sp.ry[l].x; Ps.ry[2 * l + 1] = sp.ry[l].y;
+      Ps.Tx[2 * l] = sp.Tx[l].x; Ps.Tx[2 * l + 1] = sp.Tx[l].y; Ps.Ty[2 * l] = sp.Ty[l].x; Ps.Ty[2 * l + 1] = sp.Ty[l].y;
+    }
+  }
   finalize_pose<V, MODE>(fp, p, Ps, n, th, value, separated ? idD2 : idDepth, separated);
 }
 

@@ -47,6 +47,8 @@ struct __align__(16) Footprint {
   float cT[kMaxV];              // v_l . t~_l + h_l
   float ncN[kMaxV], ncT[kMaxV], nh[kMaxV];   // negated copies (f32x2 constant operands)
   float rmax;                   // max_l |v_l|  (Prop.1)
+  float bcx, bcy, bhx, bhy;     // robot-frame bounding box: centre, half extents (culled path)
+  float rbox;                   // max_l |v_l - box centre|
 };
 
 // Per-pose state: posed footprint in registers (H1).
@@ -146,9 +148,7 @@ struct Posed2 {
 };
 
 template <int V>
-__device__ __forceinline__ void pose_setup2(const Footprint& fp, float x, float y, float th, Posed2<V>& P) {
-  float s, c;
-  sincosf(th, &s, &c);
+__device__ __forceinline__ void pose_setup2_sc(const Footprint& fp, float x, float y, float s, float c, Posed2<V>& P) {
   P.px = x;
   P.py = y;
 #pragma unroll
@@ -158,6 +158,13 @@ __device__ __forceinline__ void pose_setup2(const Footprint& fp, float x, float 
     P.Tx[l] = make_float2(c * fp.tx[2 * l] - s * fp.ty[2 * l], c * fp.tx[2 * l + 1] - s * fp.ty[2 * l + 1]);
     P.Ty[l] = make_float2(s * fp.tx[2 * l] + c * fp.ty[2 * l], s * fp.tx[2 * l + 1] + c * fp.ty[2 * l + 1]);
   }
+}
+
+template <int V>
+__device__ __forceinline__ void pose_setup2(const Footprint& fp, float x, float y, float th, Posed2<V>& P) {
+  float s, c;
+  sincosf(th, &s, &c);
+  pose_setup2_sc<V>(fp, x, y, s, c, P);
 }
 
 template <int V>

@@ -19,12 +19,10 @@ struct EvalParams {
   const int* empty_rows;       // [n_empty] obstacle rows with no valid edge
   const int* row_slot;         // [M_rows+1] number of non-empty rows before each row (row -> packed slot)
   const int* window;           // [N,2] per-pose obstacle ROW window [begin, end), or null = all rows
-  const float4* bounds;        // [Mv] per-obstacle bounding circle + first pair record (culled path)
-  const int* perm;             // [N] grid-sorted position -> pose index (culled path)
-  int* sort_cell;              // pose-sort workspace, cleaned by the culled kernel
-  unsigned int* sort_bbox;
-  int sort_cells;
-  unsigned long long* stats;   // [2] culled path: (warp x obstacle) visits, (warp x edge) steps; or null
+  const float4* gbounds;       // [2 Mv] obstacle bounds in grid order: circles, then boxes (culled path)
+  const int* gcell;            // [G*G+1] obstacle-grid cell -> first entry of gbounds
+  const struct GridHdr* ghdr;  // obstacle-grid geometry
+  unsigned long long* stats;   // [2] culled path: evaluated (pose, obstacle) pairs, (pose, edge) steps; or null
   const float* poses;          // [N,3]
   float* value;                // [N]
   float* grad;                 // [N,3] or null

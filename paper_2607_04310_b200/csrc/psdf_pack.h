@@ -17,7 +17,7 @@ struct PackedScene {
   std::vector<PairRec> pairs;     // tile-scan records: two edges each, grouped by obstacle
   std::vector<int> pair_begin;    // [Mv+1]
   std::vector<int> empty_rows;
-  std::vector<float4> bounds;     // [Mv] bounding circle + first pair record per obstacle
+  std::vector<float4> bounds;     // [2 Mv] per obstacle: bounding circle + first pair record, oriented box
   std::vector<int> row_slot;      // [M+1] non-empty rows before each row
 };
 
@@ -122,24 +122,47 @@ PSDF_HD PairRec make_pair_rec(const EdgeRec* er, int e, int k2, int slot) {
   return pr;
 }
 
-// Bounding circle of an obstacle's vertices (culled path, psdf_cull_kernels.cuh): centre of the
-// vertex bounding box, radius rounded up; .w = index of the obstacle's first pair record.
-PSDF_HD float4 obstacle_bound(const EdgeRec* er, int e, int pair_begin) {
-  double x0 = er[0].ax, x1 = er[0].ax, y0 = er[0].ay, y1 = er[0].ay;
-  for (int k = 1; k < e; ++k) {
-    const double x = er[k].ax, y = er[k].ay;
-    x0 = x < x0 ? x : x0; x1 = x > x1 ? x : x1;
-    y0 = y < y0 ? y : y0; y1 = y > y1 ? y : y1;
+// Bounds of an obstacle for the culled path (psdf_cull_kernels.cuh), two float4:
+//   obb  = (ux, uy, hx, hy): the smallest-area box among those aligned with one of the
+//          obstacle's own edges: axis u (unit), half extents along u and rot90(u);
+//   circ = (cx, cy, R, first pair record): box centre and the radius of the circle around it
+//          that holds every vertex.
+// Extents and radius are measured from the float-rounded centre/axis and rounded up.
+struct ObstacleBound { float4 circ, obb; };
+PSDF_HD ObstacleBound obstacle_bound(const EdgeRec* er, int e, int pair_begin) {
+  double best_area = 0.0, b_lt = 0, b_ht = 0, b_ln = 0, b_hn = 0;
+  int best = -1;
+  for (int k = 0; k < e; ++k) {
+    const double tx = er[k].tx, ty = er[k].ty;
+    double lt = 0, ht = 0, ln = 0, hn = 0;
+    for (int m = 0; m < e; ++m) {
+      const double x = er[m].ax, y = er[m].ay;
+      const double pt = pk_add(pk_mul(x, tx), pk_mul(y, ty)), pn = pk_sub(pk_mul(y, tx), pk_mul(x, ty));
+      if (m == 0) { lt = ht = pt; ln = hn = pn; }
+      lt = pt < lt ? pt : lt; ht = pt > ht ? pt : ht;
+      ln = pn < ln ? pn : ln; hn = pn > hn ? pn : hn;
+    }
+    const double area = pk_mul(pk_sub(ht, lt), pk_sub(hn, ln));
+    if (best < 0 || area < best_area) { best = k; best_area = area; b_lt = lt; b_ht = ht; b_ln = ln; b_hn = hn; }
   }
-  const float cx = (float)pk_mul(0.5, pk_add(x0, x1)), cy = (float)pk_mul(0.5, pk_add(y0, y1));
-  double r2 = 0.0;
+  const float ux = er[best].tx, uy = er[best].ty;
+  const double mt = pk_mul(0.5, pk_add(b_lt, b_ht)), mn = pk_mul(0.5, pk_add(b_ln, b_hn));
+  const float cx = (float)pk_sub(pk_mul(mt, (double)ux), pk_mul(mn, (double)uy));
+  const float cy = (float)pk_add(pk_mul(mt, (double)uy), pk_mul(mn, (double)ux));
+  double hx = 0.0, hy = 0.0, r2 = 0.0;
   for (int k = 0; k < e; ++k) {
     const double dx = pk_sub((double)er[k].ax, (double)cx), dy = pk_sub((double)er[k].ay, (double)cy);
+    double a = pk_add(pk_mul(dx, (double)ux), pk_mul(dy, (double)uy));
+    double b = pk_sub(pk_mul(dy, (double)ux), pk_mul(dx, (double)uy));
+    a = a < 0 ? -a : a; b = b < 0 ? -b : b;
+    hx = a > hx ? a : hx; hy = b > hy ? b : hy;
     const double d2 = pk_add(pk_mul(dx, dx), pk_mul(dy, dy));
     r2 = d2 > r2 ? d2 : r2;
   }
-  const float R = (float)pk_add(pk_mul(pk_sqrt(r2), 1.000001), 1e-6);     // rounded up
-  return make_float4(cx, cy, R, __builtin_bit_cast(float, pair_begin));
+  ObstacleBound ob;
+  ob.circ = make_float4(cx, cy, (float)pk_add(pk_mul(pk_sqrt(r2), 1.000001), 1e-6), __builtin_bit_cast(float, pair_begin));
+  ob.obb = make_float4(ux, uy, (float)pk_add(pk_mul(hx, 1.000001), 1e-6), (float)pk_add(pk_mul(hy, 1.000001), 1e-6));
+  return ob;
 }
 
 // Host packer.  returns 0 ok, -2 degenerate
@@ -160,7 +183,9 @@ inline int pack_scene(const float* A, const float* B, const uint8_t* S, int M, i
       return -2;
     if (e == 0) { out.empty_rows.push_back(i); continue; }
     out.edges.insert(out.edges.end(), tmp.begin(), tmp.begin() + e);
-    out.bounds.push_back(obstacle_bound(tmp.data(), e, (int)out.pairs.size()));
+    const ObstacleBound ob = obstacle_bound(tmp.data(), e, (int)out.pairs.size());
+    out.bounds.push_back(ob.circ);
+    out.bounds.push_back(ob.obb);
     for (int k2 = 0; k2 < (e + 1) / 2; ++k2) out.pairs.push_back(make_pair_rec(tmp.data(), e, k2, slot));
     out.row_begin.push_back((int)out.edges.size());
     out.pair_begin.push_back((int)out.pairs.size());
@@ -220,6 +245,16 @@ inline int pack_footprint(const float* fpv, int V, Footprint& fp, int& Vp) {
   }
   for (int l = 0; l < V; ++l) rmax = std::fmax(rmax, std::hypot((double)fpv[2 * l], (double)fpv[2 * l + 1]));
   fp.rmax = (float)rmax;
+  // robot-frame bounding box and the circle around its centre (culled path), rounded up
+  double x0 = x[0], x1 = x[0], y0 = y[0], y1 = y[0];
+  for (int l = 1; l < Vp; ++l) { x0 = std::fmin(x0, x[l]); x1 = std::fmax(x1, x[l]); y0 = std::fmin(y0, y[l]); y1 = std::fmax(y1, y[l]); }
+  fp.bcx = (float)(0.5 * (x0 + x1)); fp.bcy = (float)(0.5 * (y0 + y1));
+  double hx = 0, hy = 0, rb = 0;
+  for (int l = 0; l < Vp; ++l) {
+    hx = std::fmax(hx, std::fabs(x[l] - (double)fp.bcx)); hy = std::fmax(hy, std::fabs(y[l] - (double)fp.bcy));
+    rb = std::fmax(rb, std::hypot(x[l] - (double)fp.bcx, y[l] - (double)fp.bcy));
+  }
+  fp.bhx = (float)(hx * 1.000001 + 1e-6); fp.bhy = (float)(hy * 1.000001 + 1e-6); fp.rbox = (float)(rb * 1.000001 + 1e-6);
   return 0;
 }
 

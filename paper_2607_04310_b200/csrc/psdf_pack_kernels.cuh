@@ -106,7 +106,7 @@ __global__ void pack_write_kernel(const float* __restrict__ A, const float* __re
   EdgeRec* er = edges + o.y;
   pack_row(A + (size_t)i * E * 2, B + (size_t)i * E * 2, S + (size_t)i * E, E, i, o.x, er, &e);
   for (int k2 = 0; k2 < (e + 1) >> 1; ++k2) pairs[o.z + k2] = make_pair_rec(er, e, k2, o.x);
-  bounds[o.x] = obstacle_bound(er, e, o.z);
+  { const ObstacleBound ob = obstacle_bound(er, e, o.z); bounds[2 * o.x] = ob.circ; bounds[2 * o.x + 1] = ob.obb; }
   row_begin[o.x] = o.y;
   pair_begin[o.x] = o.z;
 }
@@ -159,7 +159,7 @@ __global__ void __launch_bounds__(1024) pack_fused_kernel(const float* __restric
   EdgeRec* er = edges + o.y;
   pack_row(A + (size_t)i * E * 2, B + (size_t)i * E * 2, S + (size_t)i * E, E, i, o.x, er, &e);
   for (int k2 = 0; k2 < (e + 1) >> 1; ++k2) pairs[o.z + k2] = make_pair_rec(er, e, k2, o.x);
-  bounds[o.x] = obstacle_bound(er, e, o.z);
+  { const ObstacleBound ob = obstacle_bound(er, e, o.z); bounds[2 * o.x] = ob.circ; bounds[2 * o.x + 1] = ob.obb; }
   row_begin[o.x] = o.y;
   pair_begin[o.x] = o.z;
 }

@@ -186,7 +186,7 @@ class Scene:
         _check(lib().psdf_set_culling(self._h, int(bool(enable))), "psdf_set_culling")
 
     def cull_stats(self, stream=None):
-        """psdf_cull_stats: (warp x obstacle visits, warp x edge steps) since the last call."""
+        """psdf_cull_stats: (evaluated (pose, obstacle) pairs, (pose, edge) steps) since the last call."""
         out = (ctypes.c_ulonglong * 2)()
         _check(lib().psdf_cull_stats(self._h, _stream_ptr(stream), out), "psdf_cull_stats")
         return int(out[0]), int(out[1])

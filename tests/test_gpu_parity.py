@@ -161,3 +161,68 @@ def test_few_poses_many_obstacles(env, workloads_cache, cfg, n):
     vh, gh, poh = scene.eval_host(poses, grad=True, per_obstacle=True)
     assert np.array_equal(vh, v) and np.array_equal(gh, g) and np.array_equal(poh, po)
     scene.close()
+
+
+@pytest.mark.parametrize("n_poses,V", [(4500, 4), (40000, 6), (6000, 16)])
+def test_culled_path_stress_cases(env, n_poses, V):
+    """Culled path where its machinery is stressed: 600 near-duplicates of four overlapping
+    obstacles (no bound can separate them: hundreds of candidate pairs per pose, so the
+    shared-memory pair queue overflows and the walk resumes), poses far outside the obstacle grid, both CTA shapes (N below / above 32768), the
+    smaller queue of 16-vertex footprints, a device-encoded scene, and a scene update (grid
+    rebuilt).  Unique results: bit-identical to the dense path."""
+    torch, O, psdf = env
+    from paper_2607_04310_b200 import workloads as W
+    rng = np.random.default_rng(4310 + n_poses)
+    polys = []
+    base = [(W.convex_kgon(rng, int(rng.integers(3, 9)), float(rng.uniform(0.6, 1.2))), rng.uniform(-1.0, 1.0, 2),
+             float(rng.uniform(-np.pi, np.pi))) for _ in range(4)]
+    for i in range(700):
+        if i < 600:
+            poly, centre, yaw = base[i % 4]
+            polys.append(W.place(poly, centre + rng.uniform(-1e-3, 1e-3, 2), yaw))
+        else:
+            polys.append(W.place(W.convex_kgon(rng, int(rng.integers(3, 9)), float(rng.uniform(0.3, 1.2))),
+                                 rng.uniform(-60, 60, 2), float(rng.uniform(-np.pi, np.pi))))
+    A, B, S = W.pad_scene(rng, polys, 8, extra_rows=3)
+    ang = np.linspace(0, 2 * np.pi, V, endpoint=False) + 0.1
+    footprint = np.stack([0.7 * np.cos(ang), 0.35 * np.sin(ang)], 1).astype(np.float32)
+    poses = np.empty((n_poses, 3), np.float32)
+    poses[:, :2] = rng.uniform(-14, 14, (n_poses, 2))          # ring around the cluster: ub ~ distance to it
+    poses[::7, :2] = rng.uniform(-2.5, 2.5, (len(poses[::7]), 2))   # inside the cluster (penetrating)
+    poses[::31, :2] = rng.uniform(-80, 80, (len(poses[::31]), 2))
+    poses[5, :2] = (1.0e4, -3.0e4)                              # far outside the obstacle grid
+    poses[:, 2] = rng.uniform(-np.pi, np.pi, n_poses)
+    p = torch.from_numpy(poses).cuda()
+
+    def both(scene):
+        scene.set_culling(False)
+        v, g, _ = scene.eval(p, grad=True)
+        scene.set_culling(True)
+        scene.cull_stats()
+        v1, g1, _ = scene.eval(p, grad=True)
+        v2, _, _ = scene.eval(p, grad=False)
+        torch.cuda.synchronize()
+        pairs, edge_steps = scene.cull_stats()
+        assert torch.equal(v1, v) and torch.equal(g1, g) and torch.equal(v2, v)
+        return v.cpu().numpy(), pairs / 2.0 / n_poses
+
+    scene = psdf.Scene(footprint, A, B, S, max_poses=n_poses)
+    v, per_pose = both(scene)
+    print(f"N={n_poses} V={V}: evaluated pairs per pose {per_pose:.1f}, penetrating {float((v < 0).mean()):.2f}")
+    assert per_pose > 16.0                                      # the queue (16 or 8 entries per pose) did overflow
+    # a sample against the oracle
+    idx = np.sort(rng.choice(n_poses, 300, replace=False))
+    idx = idx[idx != 5]                                         # fp32 cannot hold 1e-5 m at 3e4 m from the origin
+    ref = O.evaluate(footprint, A, B, S, poses[idx])
+    compare(ref, v[idx], what="culled stress")
+    # scene update (values only): obstacles shifted, grid rebuilt
+    shift = np.array([3.0, -2.0], np.float32)
+    scene.update(A + shift, B + shift, S)
+    both(scene)
+    scene.close()
+    # device-encoded scene
+    s2 = psdf.Scene(footprint, torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), torch.from_numpy(S).cuda(),
+                    max_poses=n_poses)
+    v_dev, _ = both(s2)
+    assert np.array_equal(v_dev, v)
+    s2.close()
