@@ -85,6 +85,8 @@ struct psdf_scene {
   float* d_out = nullptr;
   float* d_per = nullptr;
   int zero_copy = 1;                  // pinned staging is device-accessible (UVA): see run_zero_copy
+  const PoseArgs* arg_poses = nullptr;   // set around a launch whose poses travel as a kernel parameter
+  PoseArgs h_args;                    // the MPC host path's poses (N <= kArgPoses)
   GraphEntry graphs[kGraphCache];
   unsigned long long stamp = 0;
 };
@@ -93,7 +95,9 @@ namespace {
 
 template <int V, int MODE>
 cudaError_t launch_one(const psdf_scene* sc, const EvalParams& p, bool lanes, dim3 grid, int bd, cudaStream_t st) {
-  if (lanes)
+  if (lanes && sc->arg_poses)
+    psdf_lanes_args_kernel<V, MODE><<<grid, bd, 0, st>>>(sc->fp, p, *sc->arg_poses);
+  else if (lanes)
     psdf_lanes_kernel<V, MODE><<<grid, bd, 0, st>>>(sc->fp, p);
   else
     psdf_scan_kernel<V, MODE><<<grid, bd, 0, st>>>(sc->fp, p);
@@ -177,6 +181,7 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
   p.pairs = sc->pk[sc->cur].pairs;
   p.row_begin = sc->pk[sc->cur].row_begin;
   p.row_slot = sc->pk[sc->cur].row_slot;
+  p.bounds = sc->pk[sc->cur].bounds;
   p.window = window;
   p.empty_rows = sc->pk[sc->cur].empty;
   p.poses = poses;
@@ -226,13 +231,14 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
     const int ppc = bd / K;
     grid = dim3((unsigned)((N + ppc - 1) / ppc), (unsigned)C);
   } else {
-    // One thread per pose leaves only N/32 warps; the loop is issue/operand-bound and wants
-    // >= ~64 resident warps per SM to hide FMA/ALU latency (measured, profiles/r01_sweep.md),
-    // so the obstacle range is cut into C chunks (C CTAs per pose tile, combined by atomics).
-    bd = N >= 32768 ? 128 : 64;
+    // One thread per pose leaves only N/32 warps; the loop is issue/operand-bound and wants many
+    // resident warps, and many small CTAs balance the tail: the obstacle range is cut into C
+    // chunks (C CTAs of 64 poses per pose tile, combined by atomics) so that ~256 warps per SM are
+    // launched in total (measured sweep: cfg5 64x19, cfg4 64x12, cfg3 64x6).
+    bd = 64;
     int C = 1;
     const double warps_per_sm = (double)N / 32.0 / sc->sm_count;
-    if (warps_per_sm < 80.0) C = (int)std::ceil(80.0 / warps_per_sm);
+    if (warps_per_sm < 256.0) C = (int)std::ceil(256.0 / warps_per_sm);
     const int maxC = sc->Mv / 16 > 0 ? sc->Mv / 16 : 1;
     if (sc->tune_bd > 0) bd = sc->tune_bd;                                   // tuning overrides
     if (sc->tune_chunks > 0) C = sc->tune_chunks;
@@ -468,10 +474,13 @@ static inline bool use_zero_copy(const psdf_scene* sc, int N) {
 }
 
 static psdf_status run_zero_copy(psdf_scene* sc, int N, int mode, float d_min, float rho_p, float rho_theta) {
-  // staging layout: h_in [N,4] poses (padded), h_out [N,4] = (value, grad) or coefficients
+  // staging layout: h_in [N,4] poses (padded), h_out [N,4] = (value, grad) or coefficients;
+  // up to kArgPoses poses go into the launch itself (kernel parameter) instead
+  sc->arg_poses = N <= kArgPoses ? &sc->h_args : nullptr;
   psdf_status s = enqueue_eval(sc, sc->h_in, N, sc->d_in /*unused*/, (mode & kGrad) ? sc->d_out : nullptr,
                                (mode & kPerObs) ? sc->h_per : nullptr, (mode & kCoeff) ? sc->h_out : nullptr, d_min,
                                rho_p, rho_theta, sc->gstream, sc->h_out);
+  sc->arg_poses = nullptr;
   if (s != PSDF_OK) return s;
   CU_TRY(cudaStreamSynchronize(sc->gstream));
   return PSDF_OK;
@@ -534,6 +543,10 @@ static psdf_status run_graph(psdf_scene* sc, int N, int mode, float d_min, float
 
 static void stage_poses(psdf_scene* sc, const float* poses, int N) {
   if (!use_zero_copy(sc, N)) { std::memcpy(sc->h_in, poses, sizeof(float) * 3 * (size_t)N); return; }
+  if (N <= kArgPoses) {
+    for (int n = 0; n < N; ++n) sc->h_args.q[n] = make_float4(poses[3 * n], poses[3 * n + 1], poses[3 * n + 2], 0.f);
+    return;
+  }
   for (int n = 0; n < N; ++n) {
     sc->h_in[4 * n] = poses[3 * n]; sc->h_in[4 * n + 1] = poses[3 * n + 1];
     sc->h_in[4 * n + 2] = poses[3 * n + 2]; sc->h_in[4 * n + 3] = 0.f;

@@ -19,6 +19,7 @@ struct EvalParams {
   const int* empty_rows;       // [n_empty] obstacle rows with no valid edge
   const int* row_slot;         // [M_rows+1] number of non-empty rows before each row (row -> packed slot)
   const int* window;           // [N,2] per-pose obstacle ROW window [begin, end), or null = all rows
+  const float4* bounds;        // [2 Mv] per packed obstacle: (circle, first pair record), oriented box
   const float4* gbounds;       // [2 Mv] obstacle bounds in grid order: circles, then boxes (culled path)
   const int* gcell;            // [G*G+1] obstacle-grid cell -> first entry of gbounds
   const struct GridHdr* ghdr;  // obstacle-grid geometry
@@ -59,7 +60,7 @@ __device__ __forceinline__ void finalize_pose(const Footprint& fp, const EvalPar
   } else if (slot < 0) {
     value = kInf;                                  // no valid obstacle at all
   } else if (MODE & (kGrad | kCoeff)) {
-    witness_gradient<V>(fp, P, p.edges, __ldg(p.row_begin + slot), __ldg(p.row_begin + slot + 1),
+    witness_gradient<V>(fp, P, reinterpret_cast<const float4*>(p.pairs), __float_as_int(__ldg(&p.bounds[2 * slot].w)),
                         separated, g);
   }
   if (p.packed) {                                   // zero-copy staging: one 16-byte store per pose
@@ -191,9 +192,15 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
 // k + K (c + n_chunks t); (sd^i, i) arg-min by warp shuffle, then (K > 32) through shared
 // memory, then (n_chunks > 1) through a 64-bit global key with the last-arriving CTA of the
 // group finalising; so that even one pose against thousands of obstacles fills the GPU.
-template <int V, int MODE>
-__global__ void __launch_bounds__(256) psdf_lanes_kernel(const __grid_constant__ Footprint fp,
-                                                         const __grid_constant__ EvalParams p) {
+// The kernel is a latency chain, so the scene-side loads (first pair record of the lane's
+// obstacle, then the records, each one record ahead) are issued before the pose is needed and
+// overlap with its arrival and with sincosf.  ARGS: the poses travel as a kernel parameter
+// (MPC host path, N <= kArgPoses: no read over PCIe inside the kernel).
+constexpr int kArgPoses = 128;
+struct PoseArgs { float4 q[kArgPoses]; };
+
+template <int V, int MODE, bool ARGS>
+__device__ __forceinline__ void lanes_body(const Footprint& fp, const EvalParams& p, const float4* arg_poses) {
   __shared__ unsigned long long s_best[256];
   __shared__ int s_is_last;
   const int K = p.lanes, C = p.n_chunks;
@@ -201,19 +208,6 @@ __global__ void __launch_bounds__(256) psdf_lanes_kernel(const __grid_constant__
   const int g = threadIdx.x / K, lane = threadIdx.x % K;
   const int n_raw = blockIdx.x * ppc + g;
   const int n = min(n_raw, p.N - 1);
-  float x, y, th;
-  if (p.packed) {
-    // zero-copy staging (host-mapped [N,4] poses): one 16-byte read per pose (L1-cached
-    // within the launch, so the K lanes of a group share one PCIe read)
-    const float4 q = __ldg(reinterpret_cast<const float4*>(p.poses) + n);
-    x = q.x; y = q.y; th = q.z;
-  } else {
-    x = __ldg(p.poses + 3 * n); y = __ldg(p.poses + 3 * n + 1); th = __ldg(p.poses + 3 * n + 2);
-  }
-  Posed<V> P;
-  pose_setup<V>(fp, x, y, th, P);
-  unsigned long long best = ~0ull;
-  ObstacleAcc<V> acc;
   // per-pose obstacle window (time-varying environments: pose s sees the rows of E_{k+s},
   // PAPER.md:293); rows outside [0, M_rows] are clamped, an empty window gives +inf
   int s_begin = 0, s_end = p.Mv;
@@ -222,20 +216,57 @@ __global__ void __launch_bounds__(256) psdf_lanes_kernel(const __grid_constant__
     s_begin = __ldg(p.row_slot + w0);
     s_end = __ldg(p.row_slot + w1);
   }
-  for (int slot = s_begin + lane + K * (int)blockIdx.y; slot < s_end; slot += K * C) {
-    const int eb = __ldg(p.row_begin + slot), ee = __ldg(p.row_begin + slot + 1);
+  const float4* __restrict__ recs = reinterpret_cast<const float4*>(p.pairs);
+  int slot = s_begin + lane + K * (int)blockIdx.y;
+  // scene-side loads first: they do not depend on the pose
+  int rec = slot < s_end ? __float_as_int(__ldg(&p.bounds[2 * slot].w)) : 0;
+  float4 q0 = make_float4(0.f, 0.f, 0.f, 0.f), q1 = q0, q2 = q0;
+  if (slot < s_end) { q0 = __ldg(recs + 3 * (size_t)rec); q1 = __ldg(recs + 3 * (size_t)rec + 1); q2 = __ldg(recs + 3 * (size_t)rec + 2); }
+  float x, y, th;
+  if (ARGS) {
+    const float4 q = arg_poses[n];
+    x = q.x; y = q.y; th = q.z;
+  } else if (p.packed) {
+    // zero-copy staging (host-mapped [N,4] poses): one 16-byte read per pose (L1-cached
+    // within the launch, so the K lanes of a group share one PCIe read)
+    const float4 q = __ldg(reinterpret_cast<const float4*>(p.poses) + n);
+    x = q.x; y = q.y; th = q.z;
+  } else {
+    x = __ldg(p.poses + 3 * n); y = __ldg(p.poses + 3 * n + 1); th = __ldg(p.poses + 3 * n + 2);
+  }
+  Posed2<V> P;
+  pose_setup2<V>(fp, x, y, th, P);
+  unsigned long long best = ~0ull;
+  ObstacleAcc<V> acc;
+  while (slot < s_end) {
+    const int slot_next = slot + K * C;
+    const int rec_next = slot_next < s_end ? __float_as_int(__ldg(&p.bounds[2 * slot_next].w)) : 0;
     acc.reset();
     float d2 = kInf;
-    for (int k = eb; k < ee; ++k) {
-      const float4 e0 = __ldg(reinterpret_cast<const float4*>(p.edges + k));
-      edge_step<V>(fp, P, e0, __ldg(&p.edges[k].h), acc, d2);
+    int last;
+    const float4* src = recs + 3 * (size_t)rec;
+    while (true) {
+      last = __float_as_int(q2.z);
+      const float4 c0 = q0, c1 = q1;
+      const float h0 = q2.x, h1 = q2.y;
+      if (last < 0) {                                  // next record of this obstacle
+        src += 3;
+        q0 = __ldg(src); q1 = __ldg(src + 1); q2 = __ldg(src + 2);
+      } else if (slot_next < s_end) {                  // first record of the lane's next obstacle
+        src = recs + 3 * (size_t)rec_next;
+        q0 = __ldg(src); q1 = __ldg(src + 1); q2 = __ldg(src + 2);
+      }
+      edge_step2<V>(fp, P, c0, h0, acc, d2);
+      if (h1 >= 0.f) edge_step2<V>(fp, P, c1, h1, acc, d2);
+      if (last >= 0) break;
     }
     const float depth = acc.depth();
     const float sd = depth >= 0.f ? -depth : sqrtf(d2);            // eq.(23)
-    if ((MODE & kPerObs) && n_raw < p.N)
-      p.per_obs[(size_t)n * p.M_rows + __ldg(&p.edges[ee - 1].last)] = sd;
+    if ((MODE & kPerObs) && n_raw < p.N) p.per_obs[(size_t)n * p.M_rows + last] = sd;
     const unsigned long long key = ((unsigned long long)fkey(sd) << 32) | (unsigned)slot;
     best = key < best ? key : best;
+    slot = slot_next;
+    rec = rec_next;
   }
   if ((MODE & kPerObs) && n_raw < p.N && blockIdx.y == 0)
     for (int r = lane; r < p.n_empty; r += K) p.per_obs[(size_t)n * p.M_rows + __ldg(p.empty_rows + r)] = kInf;
@@ -268,7 +299,22 @@ __global__ void __launch_bounds__(256) psdf_lanes_kernel(const __grid_constant__
   if (lane != 0 || n_raw >= p.N) return;
   const bool any = best != ~0ull;
   const float value = any ? fkey_inv((uint32_t)(best >> 32)) : kInf;
-  finalize_pose<V, MODE>(fp, p, P, n, th, value, any ? (int)(uint32_t)best : -1, value > 0.f);
+  Posed<V> Ps;
+  unpack_pose<V>(P, Ps);
+  finalize_pose<V, MODE>(fp, p, Ps, n, th, value, any ? (int)(uint32_t)best : -1, value > 0.f);
+}
+
+template <int V, int MODE>
+__global__ void __launch_bounds__(256) psdf_lanes_kernel(const __grid_constant__ Footprint fp,
+                                                         const __grid_constant__ EvalParams p) {
+  lanes_body<V, MODE, false>(fp, p, nullptr);
+}
+
+template <int V, int MODE>
+__global__ void __launch_bounds__(256) psdf_lanes_args_kernel(const __grid_constant__ Footprint fp,
+                                                              const __grid_constant__ EvalParams p,
+                                                              const __grid_constant__ PoseArgs a) {
+  lanes_body<V, MODE, true>(fp, p, a.q);
 }
 
 // FP32 FMA-only micro-kernel for the measured roofline denominator (bench.py).
