@@ -49,7 +49,7 @@ struct psdf_scene {
   // packed scene, double buffered: an update writes the inactive set and flips `cur` only
   // after validation has passed (a rejected update leaves the old scene in force)
   struct Packed {
-    EdgeRec* edges = nullptr;
+    EdgeRec* edges = nullptr;         // device packer scratch (one record per valid edge)
     PairRec* pairs = nullptr;
     int* row_begin = nullptr;
     int* row_slot = nullptr;          // [M+1]
@@ -177,9 +177,7 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
                          cudaStream_t st, float* packed = nullptr, const int* window = nullptr) {
   if (N == 0) return PSDF_OK;
   EvalParams p{};
-  p.edges = sc->pk[sc->cur].edges;
   p.pairs = sc->pk[sc->cur].pairs;
-  p.row_begin = sc->pk[sc->cur].row_begin;
   p.row_slot = sc->pk[sc->cur].row_slot;
   p.bounds = sc->pk[sc->cur].bounds;
   p.window = window;
@@ -312,13 +310,10 @@ psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const u
   const psdf_scene::Packed& dst = sc->pk[sc->cur ^ 1];
   const int n_edges = (int)ps.edges.size(), Mv = (int)ps.row_begin.size() - 1, n_empty = (int)ps.empty_rows.size();
   const int n_pairs = (int)ps.pairs.size();
-  if (n_edges) {
-    CU_TRY(cudaMemcpyAsync(dst.edges, ps.edges.data(), sizeof(EdgeRec) * n_edges, cudaMemcpyHostToDevice, st));
-    CU_TRY(cudaMemcpyAsync(dst.pairs, ps.pairs.data(), sizeof(PairRec) * n_pairs, cudaMemcpyHostToDevice, st));
-  }
+  // (dst.edges / dst.row_begin are the device packer's scratch: the kernels read pair records only)
+  if (n_edges) CU_TRY(cudaMemcpyAsync(dst.pairs, ps.pairs.data(), sizeof(PairRec) * n_pairs, cudaMemcpyHostToDevice, st));
   CU_TRY(cudaMemcpyAsync(dst.row_slot, ps.row_slot.data(), sizeof(int) * (size_t)(sc->M + 1), cudaMemcpyHostToDevice, st));
   if (Mv) CU_TRY(cudaMemcpyAsync(dst.bounds, ps.bounds.data(), sizeof(float4) * 2 * Mv, cudaMemcpyHostToDevice, st));
-  CU_TRY(cudaMemcpyAsync(dst.row_begin, ps.row_begin.data(), sizeof(int) * (Mv + 1), cudaMemcpyHostToDevice, st));
   if (n_empty) CU_TRY(cudaMemcpyAsync(dst.empty, ps.empty_rows.data(), sizeof(int) * n_empty, cudaMemcpyHostToDevice, st));
   obstacle_grid_kernel<<<1, 1024, 0, st>>>(dst.bounds, Mv, nullptr, dst.gbounds, dst.gcell, dst.ghdr);
   g_launches.fetch_add(1);

@@ -13,9 +13,7 @@ constexpr int kMaxChunks = 64;
 enum Mode : int { kGrad = 1, kPerObs = 2, kCoeff = 4 };
 
 struct EvalParams {
-  const EdgeRec* edges;        // [n_edges] packed valid edges, grouped by obstacle
-  const PairRec* pairs;        // [n_pairs] the same edges two per record (tile-scan kernel)
-  const int* row_begin;        // [Mv+1] packed obstacle -> first edge
+  const PairRec* pairs;        // [n_pairs] packed valid edges, two per record, grouped by obstacle
   const int* empty_rows;       // [n_empty] obstacle rows with no valid edge
   const int* row_slot;         // [M_rows+1] number of non-empty rows before each row (row -> packed slot)
   const int* window;           // [N,2] per-pose obstacle ROW window [begin, end), or null = all rows
@@ -296,12 +294,13 @@ __device__ __forceinline__ void lanes_body(const Footprint& fp, const EvalParams
       p.ws_d2[n] = ~0ull;
     }
   }
-  if (lane != 0 || n_raw >= p.N) return;
-  const bool any = best != ~0ull;
-  const float value = any ? fkey_inv((uint32_t)(best >> 32)) : kInf;
-  Posed<V> Ps;
-  unpack_pose<V>(P, Ps);
-  finalize_pose<V, MODE>(fp, p, Ps, n, th, value, any ? (int)(uint32_t)best : -1, value > 0.f);
+  if (lane == 0 && n_raw < p.N) {
+    const bool any = best != ~0ull;
+    const float value = any ? fkey_inv((uint32_t)(best >> 32)) : kInf;
+    Posed<V> Ps;
+    unpack_pose<V>(P, Ps);
+    finalize_pose<V, MODE>(fp, p, Ps, n, th, value, any ? (int)(uint32_t)best : -1, value > 0.f);
+  }
 }
 
 template <int V, int MODE>
