@@ -35,6 +35,7 @@ struct GraphEntry {
   unsigned long long stamp = 0;
 };
 constexpr int kGraphCache = 8;
+constexpr int kCullMinPoses = 2048;     // the culled path serves larger batches only
 
 }  // namespace
 
@@ -206,7 +207,7 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
   const bool lanes = N <= 128 || pairs <= (1 << 17) || window != nullptr;
   dim3 grid;
   int bd;
-  if (sc->culling && !lanes && N > 2048 && !per_obs && sc->Mv >= 64) {
+  if (sc->culling && !lanes && N > kCullMinPoses && !per_obs && sc->Mv >= 64) {
     cudaError_t e = enqueue_culled(sc, p, mode, st);
     if (e != cudaSuccess) {
       g_last_cuda_error.store((int)e);
@@ -284,9 +285,11 @@ psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const
                                          dst.row_begin, sc->d_pair_begin, dst.empty, dst.bounds, dst.row_slot);
     g_launches.fetch_add(3);
   }
-  obstacle_grid_kernel<<<1, 1024, 0, st>>>(dst.bounds, 0, reinterpret_cast<const int*>(sc->d_totals), dst.gbounds,
-                                           dst.gcell, dst.ghdr);
-  g_launches.fetch_add(1);
+  if (sc->max_poses > kCullMinPoses) {                       // the culled path's grid (never used by small scenes)
+    obstacle_grid_kernel<<<1, 1024, 0, st>>>(dst.bounds, 0, reinterpret_cast<const int*>(sc->d_totals), dst.gbounds,
+                                             dst.gcell, dst.ghdr);
+    g_launches.fetch_add(1);
+  }
   CU_TRY(cudaMemcpyAsync(sc->h_totals, sc->d_totals, sizeof(PackTotals) + sizeof(int) * ((size_t)M + 1),
                          cudaMemcpyDeviceToHost, st));
   CU_TRY(cudaStreamSynchronize(st));                         // the only synchronisation of an update
@@ -315,8 +318,10 @@ psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const u
   CU_TRY(cudaMemcpyAsync(dst.row_slot, ps.row_slot.data(), sizeof(int) * (size_t)(sc->M + 1), cudaMemcpyHostToDevice, st));
   if (Mv) CU_TRY(cudaMemcpyAsync(dst.bounds, ps.bounds.data(), sizeof(float4) * 2 * Mv, cudaMemcpyHostToDevice, st));
   if (n_empty) CU_TRY(cudaMemcpyAsync(dst.empty, ps.empty_rows.data(), sizeof(int) * n_empty, cudaMemcpyHostToDevice, st));
-  obstacle_grid_kernel<<<1, 1024, 0, st>>>(dst.bounds, Mv, nullptr, dst.gbounds, dst.gcell, dst.ghdr);
-  g_launches.fetch_add(1);
+  if (sc->max_poses > kCullMinPoses) {                       // the culled path's grid (never used by small scenes)
+    obstacle_grid_kernel<<<1, 1024, 0, st>>>(dst.bounds, Mv, nullptr, dst.gbounds, dst.gcell, dst.ghdr);
+    g_launches.fetch_add(1);
+  }
   CU_TRY(cudaStreamSynchronize(st));       // the staging vectors die here
   sc->n_edges = n_edges;
   sc->Mv = Mv;
