@@ -287,7 +287,7 @@ psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const
   }
   if (sc->max_poses > kCullMinPoses) {                       // the culled path's grid (never used by small scenes)
     obstacle_grid_kernel<<<1, 1024, 0, st>>>(dst.bounds, 0, reinterpret_cast<const int*>(sc->d_totals), dst.gbounds,
-                                             dst.gcell, dst.ghdr);
+                                             dst.gcell, sc->d_cnt, dst.ghdr);
     g_launches.fetch_add(1);
   }
   CU_TRY(cudaMemcpyAsync(sc->h_totals, sc->d_totals, sizeof(PackTotals) + sizeof(int) * ((size_t)M + 1),
@@ -319,7 +319,7 @@ psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const u
   if (Mv) CU_TRY(cudaMemcpyAsync(dst.bounds, ps.bounds.data(), sizeof(float4) * 2 * Mv, cudaMemcpyHostToDevice, st));
   if (n_empty) CU_TRY(cudaMemcpyAsync(dst.empty, ps.empty_rows.data(), sizeof(int) * n_empty, cudaMemcpyHostToDevice, st));
   if (sc->max_poses > kCullMinPoses) {                       // the culled path's grid (never used by small scenes)
-    obstacle_grid_kernel<<<1, 1024, 0, st>>>(dst.bounds, Mv, nullptr, dst.gbounds, dst.gcell, dst.ghdr);
+    obstacle_grid_kernel<<<1, 1024, 0, st>>>(dst.bounds, Mv, nullptr, dst.gbounds, dst.gcell, sc->d_cnt, dst.ghdr);
     g_launches.fetch_add(1);
   }
   CU_TRY(cudaStreamSynchronize(st));       // the staging vectors die here

@@ -35,7 +35,7 @@ __device__ __forceinline__ int grid_coord(float v, float v0, float s, int G) {
 __global__ void __launch_bounds__(1024) obstacle_grid_kernel(const float4* __restrict__ bounds, int Mv_host,
                                                              const int* __restrict__ totals2,
                                                              float4* __restrict__ gbounds, int* __restrict__ gcell,
-                                                             GridHdr* __restrict__ hdr) {
+                                                             int* __restrict__ gidx, GridHdr* __restrict__ hdr) {
   __shared__ int cnt[kObsGridMax * kObsGridMax + 1];
   __shared__ float red[5][32];
   __shared__ int wsum[32];
@@ -90,28 +90,24 @@ __global__ void __launch_bounds__(1024) obstacle_grid_kernel(const float4* __res
     if (tid == 0) gcell[cells] = Mv;
   }
   __syncthreads();
-  for (int i = tid; i < Mv; i += 1024) {                   // scatter (cnt = cursors)
+  for (int i = tid; i < Mv; i += 1024) {                   // scatter of the indices (cnt = cursors), any order
     const float4 b = bounds[2 * i];
-    const int pos = atomicAdd(&cnt[grid_coord(b.y, y0, sy, G) * G + grid_coord(b.x, x0, sx, G)], 1);
-    gbounds[pos] = b;
-    gbounds[Mv + pos] = bounds[2 * i + 1];
+    gidx[atomicAdd(&cnt[grid_coord(b.y, y0, sy, G) * G + grid_coord(b.x, x0, sx, G)], 1)] = i;
   }
   __syncthreads();
-  // deterministic order inside a cell (by first pair record = packed order): after the scatter
-  // cnt[c] is the END of cell c, its begin is the end of cell c-1
-  for (int c = tid; c < cells; c += 1024) {
+  // deterministic order inside a cell (packed order): entry i goes to its rank among the cell's
+  // indices.  After the scatter cnt[c] is the END of cell c, its begin is the end of cell c-1.
+  // (Work is sum over cells of size^2, spread over the threads: a scene with every obstacle in one
+  // cell still takes Mv^2 / 1024 steps per thread.)
+  for (int q = tid; q < Mv; q += 1024) {
+    const int i = gidx[q];
+    const float4 b = bounds[2 * i];
+    const int c = grid_coord(b.y, y0, sy, G) * G + grid_coord(b.x, x0, sx, G);
     const int b0 = c ? cnt[c - 1] : 0, b1 = cnt[c];
-    for (int i = b0 + 1; i < b1; ++i) {
-      const float4 key = gbounds[i], key2 = gbounds[Mv + i];
-      int j = i - 1;
-      while (j >= b0 && __float_as_int(gbounds[j].w) > __float_as_int(key.w)) {
-        gbounds[j + 1] = gbounds[j];
-        gbounds[Mv + j + 1] = gbounds[Mv + j];
-        --j;
-      }
-      gbounds[j + 1] = key;
-      gbounds[Mv + j + 1] = key2;
-    }
+    int rank = 0;
+    for (int r = b0; r < b1; ++r) rank += gidx[r] < i;
+    gbounds[b0 + rank] = b;
+    gbounds[Mv + b0 + rank] = bounds[2 * i + 1];
   }
   if (tid == 0) {
     GridHdr h;
