@@ -226,3 +226,27 @@ def test_culled_path_stress_cases(env, n_poses, V):
     v_dev, _ = both(s2)
     assert np.array_equal(v_dev, v)
     s2.close()
+
+
+def test_culled_path_degenerate_grid(env):
+    """All obstacle centres coincide (nested polygons): the obstacle grid has zero extent, every
+    obstacle lands in one cell and the seed rectangle has to double ~30 times.  Still exact."""
+    torch, O, psdf = env
+    from paper_2607_04310_b200 import workloads as W
+    rng = np.random.default_rng(77)
+    base = W.rectangle(1.0, 1.0)
+    polys = [W.place(base * (0.2 + 0.02 * i), (5.0, -3.0), 0.0) for i in range(80)]
+    A, B, S = W.pad_scene(rng, polys, 6)
+    footprint = W.rectangle(0.6, 0.4).astype(np.float32)
+    n = 3000
+    poses = np.column_stack([rng.uniform(-10, 20, n), rng.uniform(-18, 12, n), rng.uniform(-np.pi, np.pi, n)]).astype(np.float32)
+    p = torch.from_numpy(poses).cuda()
+    scene = psdf.Scene(footprint, A, B, S, max_poses=n)
+    v, g, _ = scene.eval(p, grad=True)
+    scene.set_culling(True)
+    v1, g1, _ = scene.eval(p, grad=True)
+    torch.cuda.synchronize()
+    assert torch.equal(v1, v) and torch.equal(g1, g)
+    ref = O.evaluate(footprint, A, B, S, poses[:400])
+    compare(ref, v.cpu().numpy()[:400], what="nested obstacles")
+    scene.close()
