@@ -170,6 +170,11 @@ cudaError_t launch_v(const psdf_scene* sc, const EvalParams& p, int mode, bool l
   }
 }
 
+// lane-split kernel: few poses or little work (measured crossover against the tile-scan kernel)
+inline bool lanes_plan(const psdf_scene* sc, int N) {
+  return N <= 128 || (long long)N * (sc->Mv > 0 ? sc->Mv : 1) <= (1 << 17);
+}
+
 // Launch plan: lane-split kernel for MPC-sized batches; otherwise the
 // tile-scan kernel, with the obstacle range cut into chunks when the pose tiles alone
 // would not fill 148 SMs several times over.
@@ -202,9 +207,7 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
   p.rho_theta = rho_theta;
   const int mode = coeff ? kCoeff : ((grad ? kGrad : 0) | (per_obs ? kPerObs : 0));
 
-  const long long pairs = (long long)N * (sc->Mv > 0 ? sc->Mv : 1);
-  // lane-split kernel: few poses or little work (measured crossover against the tile-scan kernel)
-  const bool lanes = N <= 128 || pairs <= (1 << 17) || window != nullptr;
+  const bool lanes = lanes_plan(sc, N) || window != nullptr;
   dim3 grid;
   int bd;
   if (sc->culling && !lanes && N > kCullMinPoses && !per_obs && sc->Mv >= 64) {
@@ -465,12 +468,14 @@ static psdf_status ensure_host_path(psdf_scene* sc, bool per_obs) {
 // kernel instead of through two copy-engine operations, which removes two graph nodes'
 // worth of latency.  Same output layout as the graph path.
 constexpr int kZeroCopyMaxPoses = 512;
-constexpr int kZeroCopyMaxObstacles = 64;
+constexpr int kZeroCopyMaxObstaclesPerObs = 64;
 
-// Measured on B200 (bench.py mpc_latency): the single zero-copy launch beats the 3-node graph
-// by 4-6 us for M <= 64 obstacles and loses 1-2 us at M = 100, hence the obstacle bound.
-static inline bool use_zero_copy(const psdf_scene* sc, int N) {
-  return sc->zero_copy && N <= kZeroCopyMaxPoses && sc->Mv <= kZeroCopyMaxObstacles;
+// Measured on B200 (bench.py mpc_latency, Table-I shapes up to 1000 obstacles): the single launch
+// beats the 3-node graph by 4-7 us whenever the batch is MPC sized; only the [N,M] per-obstacle
+// output of a large scene stays on the copy engine (scattered 4-byte stores over PCIe otherwise).
+static inline bool use_zero_copy(const psdf_scene* sc, int N, bool per_obs) {
+  return sc->zero_copy && N <= kZeroCopyMaxPoses && lanes_plan(sc, N) &&      // (the lane-split kernel reads the staging layout)
+         (!per_obs || sc->Mv <= kZeroCopyMaxObstaclesPerObs);
 }
 
 static psdf_status run_zero_copy(psdf_scene* sc, int N, int mode, float d_min, float rho_p, float rho_theta) {
@@ -488,7 +493,7 @@ static psdf_status run_zero_copy(psdf_scene* sc, int N, int mode, float d_min, f
 
 // Graph replay {H2D poses, kernel, D2H results}; captured once per (N, outputs, MPC constants).
 static psdf_status run_graph(psdf_scene* sc, int N, int mode, float d_min, float rho_p, float rho_theta) {
-  if (use_zero_copy(sc, N)) return run_zero_copy(sc, N, mode, d_min, rho_p, rho_theta);
+  if (use_zero_copy(sc, N, (mode & kPerObs) != 0)) return run_zero_copy(sc, N, mode, d_min, rho_p, rho_theta);
   GraphEntry* hit = nullptr;
   GraphEntry* victim = &sc->graphs[0];
   for (auto& g : sc->graphs) {
@@ -541,8 +546,8 @@ static psdf_status run_graph(psdf_scene* sc, int N, int mode, float d_min, float
   return PSDF_OK;
 }
 
-static void stage_poses(psdf_scene* sc, const float* poses, int N) {
-  if (!use_zero_copy(sc, N)) { std::memcpy(sc->h_in, poses, sizeof(float) * 3 * (size_t)N); return; }
+static void stage_poses(psdf_scene* sc, const float* poses, int N, bool per_obs) {
+  if (!use_zero_copy(sc, N, per_obs)) { std::memcpy(sc->h_in, poses, sizeof(float) * 3 * (size_t)N); return; }
   if (N <= kArgPoses) {
     for (int n = 0; n < N; ++n) sc->h_args.q[n] = make_float4(poses[3 * n], poses[3 * n + 1], poses[3 * n + 2], 0.f);
     return;
@@ -560,11 +565,11 @@ psdf_status psdf_eval_host(psdf_scene* sc, const float* poses, int N, float* val
   if (N == 0) return PSDF_OK;
   psdf_status s = ensure_host_path(sc, per_obstacle != nullptr);
   if (s != PSDF_OK) return s;
-  stage_poses(sc, poses, N);
+  stage_poses(sc, poses, N, per_obstacle != nullptr);
   const int mode = (grad ? kGrad : 0) | (per_obstacle ? kPerObs : 0);
   s = run_graph(sc, N, mode, 0.f, 0.f, 0.f);
   if (s != PSDF_OK) return s;
-  if (use_zero_copy(sc, N)) {
+  if (use_zero_copy(sc, N, per_obstacle != nullptr)) {
     for (int n = 0; n < N; ++n) {
       value[n] = sc->h_out[4 * n];
       if (grad) { grad[3 * n] = sc->h_out[4 * n + 1]; grad[3 * n + 1] = sc->h_out[4 * n + 2]; grad[3 * n + 2] = sc->h_out[4 * n + 3]; }
@@ -618,7 +623,7 @@ psdf_status psdf_mpc_coeffs_host(psdf_scene* sc, const float* poses, int N, floa
   if (N == 0) return PSDF_OK;
   psdf_status s = ensure_host_path(sc, false);
   if (s != PSDF_OK) return s;
-  stage_poses(sc, poses, N);
+  stage_poses(sc, poses, N, false);
   s = run_graph(sc, N, kCoeff, d_min, rho_p, rho_theta);
   if (s != PSDF_OK) return s;
   std::memcpy(coeff, sc->h_out, sizeof(float) * 4 * (size_t)N);
