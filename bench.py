@@ -132,12 +132,16 @@ def mpc_latency(torch, psdf, replays=2000):
     from paper_2607_04310_b200 import workloads as W
     out = {}
 
-    def host_lat(scene, w, n_rep, grad=True, per_obs=False, coeffs=False):
+    def host_lat(scene, w, n_rep, grad=True, per_obs=False, coeffs=False, bound=True):
         value = np.empty(w.N, np.float32)
         g = np.empty((w.N, 3), np.float32) if grad else None
         po = np.empty((w.N, w.M), np.float32) if per_obs else None
-        call = (lambda: scene.mpc_coeffs_host(w.poses, 0.3, 0.05, 0.05)) if coeffs else \
-               (lambda: scene.eval_host_into(w.poses, value, g, po))
+        if coeffs:       # pre-marshalled calls (Scene.bind_*): what an MPC loop with fixed buffers makes
+            call = scene.bind_mpc_coeffs_host(w.poses, np.empty((w.N, 4), np.float32), 0.3, 0.05, 0.05)
+        elif bound:
+            call = scene.bind_eval_host(w.poses, value, g, po)
+        else:            # marshalling on every call (numpy pointer extraction: ~2 us per array)
+            call = lambda: scene.eval_host_into(w.poses, value, g, po)
         for _ in range(50):
             call()
         ts = []
@@ -170,6 +174,7 @@ def mpc_latency(torch, psdf, replays=2000):
              "eval_host_value_grad": host_lat(scene, w, replays),
              "kernel_only_value_grad": kernel_lat(scene, w)}
         if idx == 1:
+            e["eval_host_value_grad_marshalled_per_call"] = host_lat(scene, w, replays, bound=False)
             e["mpc_coeffs_host"] = host_lat(scene, w, replays, coeffs=True)
         else:
             e["eval_host_value_grad_per_obstacle"] = host_lat(scene, w, replays, per_obs=True)
@@ -188,7 +193,8 @@ def mpc_latency(torch, psdf, replays=2000):
                                       "M100_B100": 2.207,
                                       "note": "PAPER.md:417-419 Table I, PSDF rows (PyTorch graph incl. backward, "
                                               "RTX 4090): context only, other hardware"}
-    out["clock"] = "host perf_counter_ns around the Python binding's C-ABI call (ctypes overhead included)"
+    out["clock"] = ("host perf_counter_ns around the Python binding's pre-marshalled C-ABI call (Scene.bind_eval_host / "
+                    "bind_mpc_coeffs_host: the ctypes foreign call is inside, numpy pointer extraction is done once)")
     return out
 
 

@@ -269,6 +269,43 @@ class Scene:
                                     per_obstacle.ctypes.data if per_obstacle is not None else None),
                "psdf_eval_host")
 
+    def bind_eval_host(self, poses, value, grad=None, per_obstacle=None):
+        """psdf_eval_host with the argument marshalling done ONCE: returns a zero-argument
+        callable over caller-owned contiguous float32 numpy arrays (an MPC loop rewrites
+        `poses` in place every control cycle and calls it; numpy's pointer extraction alone
+        costs ~2 us per array per call).  The arrays are kept alive by the callable."""
+        N = int(poses.shape[0])
+        for a in (poses, value, grad, per_obstacle):
+            assert a is None or (a.dtype == np.float32 and a.flags.c_contiguous)
+        assert value.shape[0] == N and (grad is None or grad.shape == (N, 3))
+        assert per_obstacle is None or per_obstacle.shape == (N, self.M)
+        fn, h = lib().psdf_eval_host, self._h
+        args = (h, poses.ctypes.data, N, value.ctypes.data, grad.ctypes.data if grad is not None else None,
+                per_obstacle.ctypes.data if per_obstacle is not None else None)
+        keep = (poses, value, grad, per_obstacle)
+
+        def call(_keep=keep):
+            status = fn(*args)
+            if status != PSDF_OK:
+                raise PsdfError(status, "psdf_eval_host")
+        return call
+
+    def bind_mpc_coeffs_host(self, poses, coeff, d_min, rho_p, rho_theta):
+        """psdf_mpc_coeffs_host, pre-marshalled like bind_eval_host; coeff is [N,4] float32."""
+        N = int(poses.shape[0])
+        for a in (poses, coeff):
+            assert a.dtype == np.float32 and a.flags.c_contiguous
+        assert coeff.shape == (N, 4)
+        fn = lib().psdf_mpc_coeffs_host
+        args = (self._h, poses.ctypes.data, N, float(d_min), float(rho_p), float(rho_theta), coeff.ctypes.data)
+        keep = (poses, coeff)
+
+        def call(_keep=keep):
+            status = fn(*args)
+            if status != PSDF_OK:
+                raise PsdfError(status, "psdf_mpc_coeffs_host")
+        return call
+
     def mpc_coeffs_host(self, poses, d_min, rho_p, rho_theta):
         poses, pp = _host(poses, np.float32)
         N = int(poses.shape[0])

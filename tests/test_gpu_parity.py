@@ -45,6 +45,18 @@ def test_small_configs_device_and_host_paths(env, workloads_cache, cfg):
     for _ in range(2):
         v2, g2, po2 = scene.eval_host(w.poses, grad=True, per_obstacle=True)
         assert np.array_equal(v2, v) and np.array_equal(g2, g) and np.array_equal(po2, po)
+    # pre-marshalled calls: same results, buffers rewritten in place
+    vb, gb = np.zeros(w.N, np.float32), np.zeros((w.N, 3), np.float32)
+    pb = w.poses.copy()
+    call = scene.bind_eval_host(pb, vb, gb)
+    call()
+    assert np.array_equal(vb, v) and np.array_equal(gb, g)
+    pb[:] = w.poses[::-1]
+    call()
+    assert np.array_equal(vb, v[::-1]) and np.array_equal(gb, g[::-1])
+    cb = np.zeros((w.N, 4), np.float32)
+    scene.bind_mpc_coeffs_host(pb, cb, 0.3, 0.05, 0.05)()
+    assert np.array_equal(cb, scene.mpc_coeffs_host(pb, 0.3, 0.05, 0.05))
     v3, g3, po3 = scene.eval_host(w.poses, grad=False)
     assert g3 is None and po3 is None
     compare(ref, v3, what=w.name + " value-only host")
