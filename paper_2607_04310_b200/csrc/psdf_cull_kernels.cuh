@@ -167,7 +167,10 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
   // broad-phase proxies of the posed footprint: its bounding box (centre bx,by; axes (cs,sn),
   // (-sn,cs); half extents fp.bhx, fp.bhy) and the circle of radius fp.rbox around the box centre
   const float bx = fmaf(cs, fp.bcx, fmaf(-sn, fp.bcy, x)), by = fmaf(sn, fp.bcx, fmaf(cs, fp.bcy, y));
-  const float rpad = fp.rbox * 1.0001f + 1e-4f;            // footprint radius + safety for fp32 rounding
+  // safety for fp32 rounding: relative 1e-4 on every bound, 1e-4 m absolute, and 4 ulp of the
+  // coordinates themselves (the posed box centre is a rounded sum: 1 mm at 2e4 m from the origin)
+  const float cpad = 4.8e-7f * fmaxf(fabsf(bx), fabsf(by));
+  const float rpad = fp.rbox * 1.0001f + 1e-4f + cpad;    // footprint radius + safety
   const GridHdr gh = *p.ghdr;
   const int G = gh.G;
   const float4* __restrict__ gcirc = p.gbounds;            // (cx, cy, R, first pair record), grid order
@@ -265,7 +268,7 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
   // ---- main round: everything the seed bound cannot exclude, resumable when the queue fills
   const float ub = active ? bound_now() : -kInf;
   const float need = (ub + gh.rmax) * 1.0001f + rpad;
-  const float ub_pad = fmaf(fabsf(ub), 1e-4f, ub) + 2e-4f;
+  const float ub_pad = fmaf(fabsf(ub), 1e-4f, ub) + 2e-4f + cpad;
   bool done = !active || !(need >= 0.f);
   int cx0 = 0, cx1 = 0, cy1 = -1, row = 0, i = 0, e = 0;
   if (!done) {

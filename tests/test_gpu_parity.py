@@ -262,3 +262,55 @@ def test_culled_path_degenerate_grid(env):
     ref = O.evaluate(footprint, A, B, S, poses[:400])
     compare(ref, v.cpu().numpy()[:400], what="nested obstacles")
     scene.close()
+
+
+def _random_scene(seed):
+    """One case of the randomised culled-vs-dense differential run (same draw order)."""
+    from paper_2607_04310_b200 import workloads as W
+    rng = np.random.default_rng(seed)
+    V = int(rng.integers(3, 17))
+    M = int(rng.choice([64, 70, 200, 700, 2500]))
+    arena = float(rng.choice([3.0, 30.0, 300.0, 3000.0]))
+    off = float(rng.choice([0.0, 0.0, 1000.0, -20000.0]))
+    E = int(rng.choice([6, 8, 12, 16]))
+    rmax = float(rng.choice([0.3, 1.5, 6.0]))
+    polys = []
+    for _ in range(M):
+        if rng.random() < 0.4:
+            poly = W.rectangle(float(rng.uniform(0.3, 3) * rmax), float(rng.uniform(0.1, 1) * rmax))
+        else:
+            rad = float(rng.uniform(0.5, 1.0) * rmax)
+            poly = W.convex_kgon(rng, int(rng.integers(3, min(E, 3 + int(rad * 8)) + 1)), rad)
+        polys.append(W.place(poly, rng.uniform(0, arena, 2) + off, float(rng.uniform(-np.pi, np.pi))))
+    A, B, S = W.pad_scene(rng, polys, E, extra_rows=int(rng.integers(0, 3)))
+    ang = np.sort(rng.uniform(0, 2 * np.pi, V))
+    ang += np.linspace(0, 1e-3, V)
+    gaps = np.diff(np.concatenate([ang, [ang[0] + 2 * np.pi]]))
+    if gaps.min() < 0.15 or gaps.max() > 3.0:
+        ang = np.linspace(0, 2 * np.pi, V, endpoint=False) + 0.05
+    fr = float(rng.choice([0.2, 1.0, 4.0]))
+    footprint = (np.stack([fr * np.cos(ang), 0.5 * fr * np.sin(ang)], 1) + rng.uniform(-0.5, 0.5, 2) * fr).astype(np.float32)
+    N = int(rng.choice([2049, 5000, 33000, 70000]))
+    poses = np.empty((N, 3), np.float32)
+    poses[:, :2] = rng.uniform(-0.3 * arena, 1.3 * arena, (N, 2)) + off
+    poses[:, 2] = rng.uniform(-7, 7, N)
+    return footprint, A, B, S, poses, dict(V=V, M=M, arena=arena, off=off, N=N)
+
+
+@pytest.mark.parametrize("seed", [902050, 900010, 900002])
+def test_culled_path_far_from_the_origin(env, seed):
+    """Scenes 2e4 m from the origin, where one fp32 ulp of a coordinate is 2 mm: the culling
+    bounds must carry a safety term that grows with the coordinates.  A randomised differential
+    run (2839 scenes) found 5, all at this offset, where a fixed 1e-4 m pad dropped the winner;
+    seed 902050 is one of them (2500 obstacles crowded into 3 x 3 m, 70 000 poses)."""
+    torch, O, psdf = env
+    footprint, A, B, S, poses, info = _random_scene(seed)
+    assert info["off"] == -20000.0
+    scene = psdf.Scene(footprint, A, B, S, max_poses=len(poses))
+    p = torch.from_numpy(poses).cuda()
+    v, g, _ = scene.eval(p, grad=True)
+    scene.set_culling(True)
+    v1, g1, _ = scene.eval(p, grad=True)
+    torch.cuda.synchronize()
+    assert torch.equal(v1, v) and torch.equal(g1, g), info
+    scene.close()
