@@ -194,8 +194,9 @@ inline int pack_scene(const float* A, const float* B, const uint8_t* S, int M, i
   return 0;
 }
 
-// Supported compile-time vertex counts (even: the scan kernel packs vertices in pairs); other V are padded with collinear midpoints
-// (splitting an edge changes neither the polygon nor any min/max of eqs.(14)-(22)).
+// Supported compile-time vertex counts (even: the kernels pack vertices in pairs); other V are
+// padded with copies of the last vertex (pack_footprint; changes neither the polygon nor any
+// min/max of eqs.(14)-(22)).
 inline int padded_vertex_count(int V) {
   static const int sizes[] = {4, 6, 8, 10, 12, 16};
   for (int s : sizes)
@@ -219,38 +220,35 @@ inline int pack_footprint(const float* fpv, int V, Footprint& fp, int& Vp) {
     if ((e1x * e2y - e1y * e2x) < -1e-6 * l1 * l2) return -2;      // not convex
   }
   Vp = padded_vertex_count(V);
-  while ((int)x.size() < Vp) {                                     // split the longest edge
-    int best = 0; double bl = -1;
-    const int n = (int)x.size();
-    for (int l = 0; l < n; ++l) {
-      const double d = std::hypot(x[(l + 1) % n] - x[l], y[(l + 1) % n] - y[l]);
-      if (d > bl) { bl = d; best = l; }
-    }
-    const double mx = 0.5 * (x[best] + x[(best + 1) % n]), my = 0.5 * (y[best] + y[(best + 1) % n]);
-    x.insert(x.begin() + best + 1, mx);
-    y.insert(y.begin() + best + 1, my);
-  }
   std::memset(&fp, 0, sizeof(fp));
   double rmax = 0;
+  // The Vp - V padding vertices repeat the LAST vertex: the edges between the copies have zero
+  // length and borrow the tangent of the last-but-one real edge, so they add only duplicates of
+  // candidates and axes that exist already (a vertex distance, a face depth) and no new
+  // vertex-region / edge-region boundary.  (Splitting an edge at its midpoint would: at long range
+  // fp32 cannot tell the two collinear halves apart and the witness snaps to the artificial vertex.)
   for (int l = 0; l < Vp; ++l) {
-    const int b = (l + 1) % Vp;
-    const double dx = x[b] - x[l], dy = y[b] - y[l], L = std::hypot(dx, dy);
-    const double tx = dx / L, ty = dy / L;
-    fp.vx[l] = (float)x[l]; fp.vy[l] = (float)y[l];
+    const int a = l < V ? l : V - 1;                                  // start vertex of edge l
+    const bool closing = l == Vp - 1, zero = l >= V - 1 && !closing;
+    const int ea = zero ? V - 2 : (closing ? V - 1 : l);              // the real edge that lends its tangent
+    const int eb = (ea + 1) % V;
+    const double dx = x[eb] - x[ea], dy = y[eb] - y[ea], L = std::hypot(dx, dy);
+    const double tx = dx / L, ty = dy / L, h = zero ? 0.0 : 0.5 * L;
+    fp.vx[l] = (float)x[a]; fp.vy[l] = (float)y[a];
     fp.tx[l] = (float)tx; fp.ty[l] = (float)ty;
-    fp.h[l] = (float)(0.5 * L);
-    fp.cN[l] = (float)(x[l] * (-ty) + y[l] * tx);
-    fp.cT[l] = (float)(x[l] * tx + y[l] * ty + 0.5 * L);
+    fp.h[l] = (float)h;
+    fp.cN[l] = (float)(x[a] * (-ty) + y[a] * tx);
+    fp.cT[l] = (float)(x[a] * tx + y[a] * ty + h);
     fp.ncN[l] = -fp.cN[l]; fp.ncT[l] = -fp.cT[l]; fp.nh[l] = -fp.h[l];
   }
   for (int l = 0; l < V; ++l) rmax = std::fmax(rmax, std::hypot((double)fpv[2 * l], (double)fpv[2 * l + 1]));
   fp.rmax = (float)rmax;
   // robot-frame bounding box and the circle around its centre (culled path), rounded up
   double x0 = x[0], x1 = x[0], y0 = y[0], y1 = y[0];
-  for (int l = 1; l < Vp; ++l) { x0 = std::fmin(x0, x[l]); x1 = std::fmax(x1, x[l]); y0 = std::fmin(y0, y[l]); y1 = std::fmax(y1, y[l]); }
+  for (int l = 1; l < V; ++l) { x0 = std::fmin(x0, x[l]); x1 = std::fmax(x1, x[l]); y0 = std::fmin(y0, y[l]); y1 = std::fmax(y1, y[l]); }
   fp.bcx = (float)(0.5 * (x0 + x1)); fp.bcy = (float)(0.5 * (y0 + y1));
   double hx = 0, hy = 0, rb = 0;
-  for (int l = 0; l < Vp; ++l) {
+  for (int l = 0; l < V; ++l) {
     hx = std::fmax(hx, std::fabs(x[l] - (double)fp.bcx)); hy = std::fmax(hy, std::fabs(y[l] - (double)fp.bcy));
     rb = std::fmax(rb, std::hypot(x[l] - (double)fp.bcx, y[l] - (double)fp.bcy));
   }

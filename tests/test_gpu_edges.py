@@ -366,3 +366,34 @@ def test_autograd_module(env):
     rel = np.linalg.norm(got[ok] - want[ok], axis=1) / np.linalg.norm(want[ok], axis=1)
     assert rel.max() <= 1e-3 and ok.mean() > 0.5
     mod.scene.close()
+
+
+def test_odd_footprint_padding_adds_no_witness_boundary(env):
+    """A 15-vertex footprint is padded to 16 for the kernels.  Padding by splitting an edge at
+    its midpoint put an artificial vertex-region boundary on that edge: at 18 m range fp32
+    cannot separate the two collinear halves (d^2 differs by one ulp) and the witness snapped to
+    the artificial vertex (gradient off by 6e-3; found by a randomised run against the oracle,
+    this is that case).  Padding with copies of a vertex adds no boundary."""
+    torch, O, psdf, W = env
+    footprint = np.array([[1.1168420314788818, -0.327312171459198], [1.010167121887207, -0.12635846436023712],
+                          [0.7492443323135376, 0.035527586936950684], [0.37918949127197266, 0.13035441935062408],
+                          [-0.03601149469614029, 0.14172562956809998], [-0.4245666563510895, 0.06767500191926956],
+                          [-0.7192912697792053, -0.07899341732263565], [-0.8692247271537781, -0.27291932702064514],
+                          [-0.8484421968460083, -0.4805711805820465], [-0.6605371832847595, -0.6660441160202026],
+                          [-0.33800017833709717, -0.7972680926322937], [0.06339926272630692, -0.8515533804893494],
+                          [0.4742555320262909, -0.8195134997367859], [0.8235278129577637, -0.7066885232925415],
+                          [1.0508238077163696, -0.5325868129730225]], np.float32)
+    poly = np.array([[-92.06255340576172, -74.37434387207031], [-92.02520751953125, -74.52521514892578],
+                     [-91.90606689453125, -74.4957275390625], [-91.94340515136719, -74.34485626220703]], np.float32)
+    A = poly[None].copy()
+    B = np.roll(poly, -1, axis=0)[None].copy()
+    S = np.ones((1, 4), np.uint8)
+    poses = np.array([[-77.1455078125, -85.82178497314453, 0.9523851275444031]], np.float32)
+    ref = O.evaluate(footprint, A, B, S, poses)
+    assert ref.margin[0] > 1e-3                          # a well-separated winner: the comparison is meaningful
+    scene = psdf.Scene(footprint, A, B, S, max_poses=4)
+    v, g, _ = _run(torch, scene, poses, grad=True)
+    compare(ref, v, g, what="15-gon at 18 m")
+    vh, gh, _ = scene.eval_host(poses, grad=True)
+    compare(ref, vh, gh, what="15-gon at 18 m, host path")
+    scene.close()
