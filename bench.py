@@ -142,7 +142,7 @@ def mpc_latency(torch, psdf, replays=2000):
             call = scene.bind_eval_host(w.poses, value, g, po)
         else:            # marshalling on every call (numpy pointer extraction: ~2 us per array)
             call = lambda: scene.eval_host_into(w.poses, value, g, po)
-        for _ in range(50):
+        for _ in range(500):        # ~10 ms: the first calls of a process run ~5 us slower
             call()
         ts = []
         for _ in range(n_rep):
