@@ -2,9 +2,12 @@
 // eq.(17)): padded (A,B,S) -> packed valid-edge records, in
 // double, validated against Assumption 1.
 #pragma once
+#include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
+#include <thread>
 #include <vector>
 
 #include "psdf_device.cuh"
@@ -167,31 +170,54 @@ PSDF_HD ObstacleBound obstacle_bound(const EdgeRec* er, int e, int pair_begin) {
 
 // Host packer.  returns 0 ok, -2 degenerate
 inline int pack_scene(const float* A, const float* B, const uint8_t* S, int M, int E, PackedScene& out) {
-  out.edges.clear();
-  out.pairs.clear();
+  // pass 1: valid-edge counts -> offsets (what the device packer's scan kernel does)
+  out.row_slot.assign((size_t)M + 1, 0);
   out.row_begin.assign(1, 0);
   out.pair_begin.assign(1, 0);
   out.empty_rows.clear();
-  out.bounds.clear();
-  out.row_slot.assign((size_t)M + 1, 0);
-  std::vector<EdgeRec> tmp((size_t)E);
+  std::vector<int> cnt((size_t)M);
   for (int i = 0; i < M; ++i) {
     int e = 0;
-    const int slot = (int)out.row_begin.size() - 1;
-    out.row_slot[i] = slot;
-    if (pack_row(A + (size_t)i * E * 2, B + (size_t)i * E * 2, S + (size_t)i * E, E, i, slot, tmp.data(), &e) != 0)
-      return -2;
+    for (int j = 0; j < E; ++j) e += S[(size_t)i * E + j] ? 1 : 0;
+    cnt[i] = e;
+    out.row_slot[i] = (int)out.row_begin.size() - 1;
     if (e == 0) { out.empty_rows.push_back(i); continue; }
-    out.edges.insert(out.edges.end(), tmp.begin(), tmp.begin() + e);
-    const ObstacleBound ob = obstacle_bound(tmp.data(), e, (int)out.pairs.size());
-    out.bounds.push_back(ob.circ);
-    out.bounds.push_back(ob.obb);
-    for (int k2 = 0; k2 < (e + 1) / 2; ++k2) out.pairs.push_back(make_pair_rec(tmp.data(), e, k2, slot));
-    out.row_begin.push_back((int)out.edges.size());
-    out.pair_begin.push_back((int)out.pairs.size());
+    out.row_begin.push_back(out.row_begin.back() + e);
+    out.pair_begin.push_back(out.pair_begin.back() + (e + 1) / 2);
   }
-  out.row_slot[M] = (int)out.row_begin.size() - 1;
-  return 0;
+  const int Mv = (int)out.row_begin.size() - 1;
+  out.row_slot[M] = Mv;
+  out.edges.assign((size_t)out.row_begin.back(), EdgeRec{});
+  out.pairs.assign((size_t)out.pair_begin.back(), PairRec{});
+  out.bounds.assign(2 * (size_t)Mv, float4{});
+  // pass 2: rows are independent; large scenes are split over a few threads
+  std::atomic<int> status{0};
+  auto work = [&](int i0, int i1) {
+    for (int i = i0; i < i1 && status.load(std::memory_order_relaxed) == 0; ++i) {
+      const int slot = out.row_slot[i];
+      EdgeRec* er = cnt[i] ? out.edges.data() + out.row_begin[slot] : nullptr;
+      int e = 0;
+      if (pack_row(A + (size_t)i * E * 2, B + (size_t)i * E * 2, S + (size_t)i * E, E, i, slot, er, &e) != 0) {
+        status.store(-2);
+        return;
+      }
+      if (e == 0) continue;
+      const int pb = out.pair_begin[slot];
+      const ObstacleBound ob = obstacle_bound(er, e, pb);
+      out.bounds[2 * (size_t)slot] = ob.circ;
+      out.bounds[2 * (size_t)slot + 1] = ob.obb;
+      for (int k2 = 0; k2 < (e + 1) / 2; ++k2) out.pairs[(size_t)pb + k2] = make_pair_rec(er, e, k2, slot);
+    }
+  };
+  const int n_thr = M >= 512 ? (int)std::min<unsigned>(8u, std::max(1u, std::thread::hardware_concurrency())) : 1;
+  if (n_thr == 1) {
+    work(0, M);
+  } else {
+    std::vector<std::thread> pool;
+    for (int t = 0; t < n_thr; ++t) pool.emplace_back(work, (int)((long long)M * t / n_thr), (int)((long long)M * (t + 1) / n_thr));
+    for (auto& th : pool) th.join();
+  }
+  return status.load();
 }
 
 // Supported compile-time vertex counts (even: the kernels pack vertices in pairs); other V are
