@@ -171,7 +171,13 @@ class Scene:
             lib().psdf_destroy_scene(self._h)
             self._h = None
 
-    __del__ = close
+    def __del__(self):
+        # at interpreter shutdown the module globals may already be gone: the process is about
+        # to release the device anyway
+        try:
+            self.close()
+        except Exception:
+            pass
 
     @property
     def num_obstacles(self):
