@@ -3,10 +3,20 @@
 and k-gons, random mask positions, clockwise rows, fully masked rows), poses scattered over and
 next to the obstacles, at offsets from the origin.  Every public path is checked against the
 oracle or against another path that must agree bit for bit.  Need a B200: `pytest -m gpu`."""
+import os
+
 import numpy as np
 import pytest
 
 from tests.parity import compare
+
+# Knobs for the long runs (defaults = the bounded slice the suite runs):
+#   PSDF_RANDOM_SEED_BASE  first scene seed of test_random_scenes_every_path (default 510000)
+#   PSDF_RANDOM_SCENES     scenes per block, four blocks (default 25)
+#   PSDF_RANDOM_CULLED     number of culled-vs-dense scenes (default 12)
+_SEED_BASE = int(os.environ.get("PSDF_RANDOM_SEED_BASE", "510000"))
+_PER_BLOCK = int(os.environ.get("PSDF_RANDOM_SCENES", "25"))
+_N_CULLED = int(os.environ.get("PSDF_RANDOM_CULLED", "12"))
 
 pytestmark = pytest.mark.gpu
 
@@ -64,7 +74,7 @@ def _scene(W, seed):
 @pytest.mark.parametrize("block", range(4))
 def test_random_scenes_every_path(env, block):
     torch, O, psdf, W = env
-    for seed in range(510000 + 25 * block, 510000 + 25 * (block + 1)):
+    for seed in range(_SEED_BASE + _PER_BLOCK * block, _SEED_BASE + _PER_BLOCK * (block + 1)):
         rng, footprint, A, B, S, poses, tag = _scene(W, seed)
         N, Mrows = len(poses), A.shape[0]
         scene = psdf.Scene(footprint, A, B, S, max_poses=max(N, 8))
@@ -110,7 +120,7 @@ def test_random_scenes_every_path(env, block):
         scene.close()
 
 
-@pytest.mark.parametrize("seed", [902050 + 7 * k for k in range(12)])
+@pytest.mark.parametrize("seed", [902050 + 7 * k for k in range(_N_CULLED)])
 def test_random_scenes_culled_equals_dense(env, seed):
     torch, O, psdf, W = env
     from tests.test_gpu_parity import _random_scene
