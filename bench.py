@@ -237,7 +237,8 @@ def main():
     ap.add_argument("--impl", default="psdf", choices=["psdf", "reference"])
     ap.add_argument("--ref-poses", type=int, default=4096)
     ap.add_argument("--ref-seconds", type=float, default=90.0, help="--impl reference: target total run time")
-    ap.add_argument("--cpu-poses", type=int, default=2048)
+    ap.add_argument("--cpu-poses", type=int, default=16384, help="upper limit of the cpu_baseline pose sample")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target oracle time of the cpu_baseline sample")
     ap.add_argument("--no-latency", action="store_true", help="skip the MPC-sized latency section")
     ap.add_argument("--value-only", action="store_true", help="extra run without gradients is always reported; "
                     "this flag makes it the headline")
@@ -370,7 +371,11 @@ def main():
         }
         if world == 1:
             from oracle import psdf_oracle as O          # cpu_baseline leg: the oracle as it stands
-            sub = w.subsample(min(args.cpu_poses, w.N))
+            cal = w.subsample(min(256, w.N))             # size the sample for ~cpu_seconds on THIS host
+            t0 = time.perf_counter()
+            O.evaluate(cal.footprint, cal.A, cal.B, cal.S, cal.poses)
+            rate = cal.N / (time.perf_counter() - t0)
+            sub = w.subsample(int(min(max(args.cpu_seconds * rate, 1024), args.cpu_poses, w.N)))
             t0 = time.perf_counter()
             O.evaluate(sub.footprint, sub.A, sub.B, sub.S, sub.poses)
             dt = time.perf_counter() - t0
