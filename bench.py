@@ -105,14 +105,14 @@ def measured_peaks():
         return {}
 
 
-def ncu_traffic(workload_name: str):
-    """Per-launch DRAM bytes of the dominant kernel from the committed ncu --set full
-    capture (profiles/traffic.csv), or None."""
+def ncu_traffic(workload_name: str, column: int = 1):
+    """Per-launch DRAM bytes (column 1) or executed warp instructions (column 2) of the dominant
+    kernel from the committed ncu --set full capture (profiles/traffic.csv), or None."""
     try:
         for ln in open(os.path.join(ROOT, "profiles", "traffic.csv")).read().splitlines()[1:]:
             f = ln.split(",")
             if f[0] == workload_name:
-                return float(f[1])
+                return float(f[column])
     except (OSError, ValueError, IndexError):
         pass
     return None
@@ -334,6 +334,15 @@ def main():
         peak_nominal = sms * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
         achieved = F / t_kernel / 1e12
         hbm = float(peaks.get("hbm_gbs", 6650.0))
+        # SURVEY.md 8(d) issue-slot view: executed lane-instructions/s against one instruction per
+        # lane and clock (= P_fp32 / 2); the instruction count is the committed ncu capture's.
+        warp_inst = ncu_traffic(w.name, 2)
+        issue_view = None
+        if warp_inst:
+            issue_peak = sms * FP32_LANES_PER_SM * sm_max * 1e6
+            issue_view = {"warp_inst_per_launch": warp_inst, "lane_inst_per_s": warp_inst * 32 / t_kernel,
+                          "peak_lane_inst_per_s": issue_peak, "frac": warp_inst * 32 / t_kernel / issue_peak,
+                          "source": "smsp__inst_executed.sum of the committed ncu --set full capture (profiles/traffic.csv)"}
         out = {
             "metric": METRIC, "value": pairs * world * args.steps / t_dev, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_dev / args.steps * 1e3,
@@ -349,6 +358,7 @@ def main():
                                         "(clocks.max.sm, MEASURED_PEAKS.json); no FP32 figure in MEASURED_PEAKS.json",
                          "flops_per_launch": F, "flop_formula": "32*V*e+6*e+4*V+6 per (pose, obstacle), valid edges only",
                          "kernel_ms": t_kernel * 1e3, "kernel_ms_min": float(np.min(times)),
+                         "kernel_ms_median": float(np.median(times)), "issue_slot_view": issue_view,
                          "peak_measured_ffma": fp32_meas, "frac_of_measured_ffma": achieved / fp32_meas if fp32_meas else None,
                          "hbm_bytes_algorithmic": algorithmic_bytes(w),
                          "hbm_gbs_achieved": algorithmic_bytes(w) / t_kernel / 1e9, "hbm_gbs_peak_measured": hbm},
@@ -383,6 +393,12 @@ def main():
                                    "kind": "oracle", "seconds": dt,
                                    "sample": f"{sub.N} of {w.N} poses (stride subsample) x {w.M} obstacles, "
                                              "value+grad, float64, OpenMP"}
+            one = w.subsample(int(min(max(0.25 * args.cpu_seconds * rate / max(O.max_threads(), 1), 64), w.N)))
+            t0 = time.perf_counter()
+            O.evaluate(one.footprint, one.A, one.B, one.S, one.poses, nthreads=1)
+            dt1 = time.perf_counter() - t0
+            out["cpu_baseline"]["single_thread"] = {"value": one.n_pairs() / dt1, "unit": UNIT, "seconds": dt1,
+                                                    "sample": f"{one.N} of {w.N} poses (stride subsample), 1 thread"}
             if not args.no_latency:
                 out["mpc_latency"] = mpc_latency(torch, psdf)
         print(json.dumps(out), flush=True)
