@@ -34,18 +34,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_ubench() -> str:
-    """Pipe micro-benchmarks behind DESIGN.md section 6.4 (csrc/ubench/pipes.cu)."""
-    out = os.path.join(CSRC, "ubench", "pipes")
-    cmd = [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-o", out,
-           os.path.join(CSRC, "ubench", "pipes.cu")]
-    subprocess.run(cmd, check=True)
-    return out
-
-
 if __name__ == "__main__":
-    import sys
-    if len(sys.argv) > 1 and sys.argv[1] == "ubench":
-        print(build_ubench())
-    else:
-        print(build(force=True, verbose=True))
+    print(build(force=True, verbose=True))
