@@ -56,7 +56,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+                                          "-lms", "25", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
             self.t = threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True)
             self.t.start()
         except OSError:
@@ -107,12 +107,13 @@ def measured_peaks():
 
 def ncu_traffic(workload_name: str, column: int = 1):
     """Per-launch DRAM bytes (column 1) or executed warp instructions (column 2) of the dominant
-    kernel from the committed ncu --set full capture (profiles/traffic.csv), or None."""
+    kernel from the committed ncu --set full capture (profiles/traffic.csv), or None; column 3 is the
+    commit whose code was captured (a string)."""
     try:
         for ln in open(os.path.join(ROOT, "profiles", "traffic.csv")).read().splitlines()[1:]:
             f = ln.split(",")
             if f[0] == workload_name:
-                return float(f[column])
+                return f[column] if column == 3 else float(f[column])
     except (OSError, ValueError, IndexError):
         pass
     return None
@@ -149,7 +150,13 @@ def mpc_latency(torch, psdf, replays=2000):
             t0 = time.perf_counter_ns()
             call()
             ts.append((time.perf_counter_ns() - t0) * 1e-3)
-        return _pct(ts)
+        out = _pct(ts)
+        # the same call timed INSIDE the library (steady_clock around the C-ABI entry point: no
+        # interpreter, no ctypes in the timed region)
+        inlib = scene.bench_host_latency(w.poses, n_rep, grad=grad, per_obstacle=per_obs,
+                                         coeffs=(0.3, 0.05, 0.05) if coeffs else None)
+        out["c_abi_clock"] = _pct(inlib)
+        return out
 
     def kernel_lat(scene, w, n_rep=300, per_obs=False):
         poses = torch.from_numpy(w.poses).cuda()
@@ -228,6 +235,81 @@ def run_reference(args, w):
             "gpu_launches": 0}
 
 
+def pinned(torch, shape):
+    """Page-locked host array (numpy view of a pinned torch tensor): what a caller that cares about
+    end-to-end time hands to psdf_eval_host (include/psdf.h: pinned buffers are used in place)."""
+    return torch.empty(shape, dtype=torch.float32, pin_memory=True).numpy()
+
+
+class DeviceRun:
+    """One workload resident in HBM: scene, poses, outputs, and the timed psdf_eval loop."""
+
+    def __init__(self, torch, psdf, w, flush):
+        self.torch, self.w, self.flush = torch, w, flush
+        self.scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=w.N)
+        self.poses = torch.from_numpy(w.poses).cuda()
+        self.value = torch.empty(w.N, dtype=torch.float32, device="cuda")
+        self.grad = torch.empty((w.N, 3), dtype=torch.float32, device="cuda")
+        self.stream = torch.cuda.current_stream()
+
+    def timed(self, n_steps, with_grad=True):
+        """n_steps psdf_eval calls, L2 flushed before each, CUDA events on the launching stream."""
+        torch = self.torch
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_steps)]
+        for a, b in evs:
+            self.flush.zero_()                               # L2 flush between timed iterations
+            a.record(self.stream)
+            self.scene.eval(self.poses, value=self.value, grad=self.grad if with_grad else False, stream=self.stream)
+            b.record(self.stream)
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in evs]
+
+    def e2e(self, n_steps, pin):
+        """n_steps psdf_eval_host calls from HOST buffers (host clock; H2D and D2H inside).  Returns
+        (seconds per step, value, grad) with the outputs of the last call."""
+        w = self.w
+        if pin:
+            p, v, g = pinned(self.torch, (w.N, 3)), pinned(self.torch, (w.N,)), pinned(self.torch, (w.N, 3))
+            p[:] = w.poses
+        else:
+            p, v, g = w.poses, np.empty(w.N, np.float32), np.empty((w.N, 3), np.float32)
+        for _ in range(3):
+            self.scene.eval_host_into(p, v, g)
+        v[:] = 0
+        g[:] = 0
+        t0 = time.perf_counter()
+        for _ in range(n_steps):
+            self.scene.eval_host_into(p, v, g)
+        return (time.perf_counter() - t0) / n_steps, v, g
+
+
+def parity_report(torch, psdf, O, workloads, budget_poses):
+    """BASELINE.md section 3 / SURVEY.md 5: GPU against the oracle on all five configs, measured exactly
+    as tests/parity.py does (|d value|, gradient relative error where the oracle's arg-min margin
+    allows, compared and penetrating fractions).  Configs 1-2 whole, 3-5 on a random sample of the
+    FULL-size launch's outputs.  Runs outside every timed region; the oracle calls here belong to
+    the cpu_baseline leg (the same oracle, the same host cores)."""
+    from tests.parity import stats, VALUE_TOL, GRAD_REL_TOL
+    out = {"bar": {"value_tol_m": VALUE_TOL, "grad_rel_tol": GRAD_REL_TOL, "margin_min_m": 1e-4,
+                   "rule": "gradient compared where the oracle's arg-min margin > 1e-4 m; on the separated branch also "
+                           "phi > 1e-3 m (DESIGN.md reading G9)"}}
+    for idx, w in workloads.items():
+        scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=w.N)
+        v, g, po = scene.eval(torch.from_numpy(w.poses).cuda(), grad=True, per_obstacle=(idx == 2))
+        torch.cuda.synchronize()
+        v, g = v.cpu().numpy(), g.cpu().numpy()
+        n = min(w.N, budget_poses[idx])
+        sel = np.sort(np.random.default_rng(777 + idx).choice(w.N, n, replace=False))
+        ref = O.evaluate(w.footprint, w.A, w.B, w.S, w.poses[sel], per_obstacle=(idx == 2))
+        st = stats(ref, v[sel], g[sel], po.cpu().numpy()[sel] if idx == 2 else None)
+        st = {k: st[k] for k in st if not k.startswith("argmax")}
+        st["sample"] = f"{n} of {w.N} poses of the full-size launch" if n < w.N else f"all {w.N} poses"
+        st["within_bar"] = bool(st["inf_pattern_equal"] and st["max_dvalue"] <= VALUE_TOL and st["max_grad_rel"] <= GRAD_REL_TOL)
+        out[w.name] = st
+        scene.close()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -240,6 +322,7 @@ def main():
     ap.add_argument("--cpu-poses", type=int, default=16384, help="upper limit of the cpu_baseline pose sample")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target oracle time of the cpu_baseline sample")
     ap.add_argument("--no-latency", action="store_true", help="skip the MPC-sized latency section")
+    ap.add_argument("--no-extras", action="store_true", help="skip per_config, parity and latency (profiling runs)")
     ap.add_argument("--value-only", action="store_true", help="extra run without gradients is always reported; "
                     "this flag makes it the headline")
     args = ap.parse_args()
@@ -267,60 +350,49 @@ def main():
         torch.cuda.synchronize()
 
     w = load_workload(args.workload, rank)
-    scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=w.N)
-    poses = torch.from_numpy(w.poses).cuda()
-    value = torch.empty(w.N, dtype=torch.float32, device="cuda")
-    grad = torch.empty((w.N, 3), dtype=torch.float32, device="cuda")
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
-    stream = torch.cuda.current_stream()
+    run = DeviceRun(torch, psdf, w, flush)
+    scene, value, grad = run.scene, run.value, run.grad
 
-    def timed(n_steps, with_grad):
-        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_steps)]
-        for a, b in evs:
-            flush.zero_()                                    # L2 flush between timed iterations
-            a.record(stream)
-            scene.eval(poses, value=value, grad=grad if with_grad else False, stream=stream)
-            b.record(stream)
-        torch.cuda.synchronize()
-        return [a.elapsed_time(b) for a, b in evs]
-
-    timed(max(args.warmup, 3), True)
+    run.timed(max(args.warmup, 3), True)
     fp32_meas = psdf.psdf_measure_fp32_peak(8192) if rank == 0 else None
-    timed(3, True)
+    run.timed(3, True)
     sampler = ClockSampler(local_rank)
     n_launch0 = psdf.psdf_kernel_launches()
     barrier()
     sampler.start()
     t_wall0 = time.perf_counter()
-    times = timed(args.steps, not args.value_only)
+    times = run.timed(args.steps, not args.value_only)
     barrier()
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
     launches = psdf.psdf_kernel_launches() - n_launch0
     t_dev = float(np.sum(times)) * 1e-3
-    other = timed(max(args.steps // 4, 5), args.value_only)     # the other variant, for the record
+    other = run.timed(max(args.steps // 4, 5), args.value_only)     # the other variant, for the record
+    run.timed(1, True)
+    v_dense, g_dense = value.cpu().numpy(), grad.cpu().numpy()
 
     # exact broad-phase culling (psdf_set_culling): same outputs, bit for bit
     scene.set_culling(True)
-    timed(5, True)
+    run.timed(5, True)
     scene.cull_stats()
     k_cull = max(args.steps // 2, 10)
-    cull_times = timed(k_cull, True)
+    cull_times = run.timed(k_cull, True)
     eval_pairs, edge_steps = scene.cull_stats()
-    v_cull = value.clone()
-    scene.set_culling(False)
-    timed(1, True)
-    culled_same = bool(torch.equal(v_cull, value))
-
-    # end to end through the public host API: pinned staging + H2D + kernel + D2H inside
-    for _ in range(3):
-        scene.eval_host(w.poses, grad=True)
-    barrier()
+    culled_same = bool(np.array_equal(value.cpu().numpy(), v_dense) and np.array_equal(grad.cpu().numpy(), g_dense))
+    # ... and end to end through psdf_eval_host, from pinned and from ordinary host buffers
     k_e2e = max(args.steps // 4, 5)
-    t0 = time.perf_counter()
-    for _ in range(k_e2e):
-        scene.eval_host(w.poses, grad=True)
-    t_e2e = (time.perf_counter() - t0) / k_e2e
+    t_e2e_cull, vc, gc = run.e2e(4 * k_e2e, pin=True)
+    e2e_cull_checked = bool(np.array_equal(vc, v_dense) and np.array_equal(gc, g_dense))
+    t_e2e_cull_pageable, _, _ = run.e2e(k_e2e, pin=False)
+    scene.set_culling(False)
+
+    # end to end through the public host API (dense): H2D + kernels + D2H inside the timed region
+    barrier()
+    t_e2e, ve, ge = run.e2e(k_e2e, pin=True)
+    e2e_checked = bool(np.array_equal(ve, v_dense) and np.array_equal(ge, g_dense))   # outside the timed region
+    t_e2e_pageable, vp_, gp_ = run.e2e(k_e2e, pin=False)
+    e2e_checked = e2e_checked and bool(np.array_equal(vp_, v_dense) and np.array_equal(gp_, g_dense))
 
     t_dev, t_e2e, t_wall = sharding.max_over_ranks([t_dev, t_e2e, t_wall])      # max over ranks
 
@@ -354,6 +426,8 @@ def main():
                        "parallelism": f"replicated scene, pose-sharded x{world}", "seed": 43100 + args.workload},
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
                          "frac": achieved / peak_nominal, "traffic": ncu_traffic(w.name),
+                         "traffic_source": "profiles/traffic.csv: one ncu --set full capture of this kernel, code of commit "
+                                           f"{ncu_traffic(w.name, 3)} (a constant of that capture, not of this run)",
                          "peak_source": f"derived: {sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x {sm_max:.0f} MHz "
                                         "(clocks.max.sm, MEASURED_PEAKS.json); no FP32 figure in MEASURED_PEAKS.json",
                          "flops_per_launch": F, "flop_formula": "32*V*e+6*e+4*V+6 per (pose, obstacle), valid edges only",
@@ -366,7 +440,10 @@ def main():
                               "ms_per_step": float(np.mean(other)), "value": pairs / (float(np.mean(other)) * 1e-3)},
             "e2e": {"value": pairs * world / t_e2e, "unit": UNIT, "ms_per_step": t_e2e * 1e3,
                     "h2d_bytes_per_step": w.N * 12, "d2h_bytes_per_step": w.N * 16,
-                    "api": "psdf_eval_host (host buffers -> pinned staging -> CUDA graph {H2D, kernel, D2H} -> host)"},
+                    "api": "psdf_eval_host from pinned host buffers (used in place): captured CUDA graph of "
+                           "{H2D pose chunk, kernel, D2H result chunk} branches, stream synchronise",
+                    "from_pageable_buffers_ms_per_step": t_e2e_pageable * 1e3},
+            "e2e_outputs_checked": e2e_checked,
             "culling": {"what": "psdf_set_culling(1): obstacle grid + bounding-circle / oriented-box lower bounds, "
                                 "pair-queue kernel, value+grad; outputs bit-identical to the dense path "
                                 "(checked in this run: %s)" % culled_same,
@@ -374,6 +451,11 @@ def main():
                         "unit": UNIT, "speedup_vs_dense": t_kernel * 1e3 / float(np.mean(cull_times)),
                         "evaluated_pair_fraction": eval_pairs / k_cull / pairs,
                         "evaluated_flops_per_step": ((32.0 * w.V + 6.0) * edge_steps + (4.0 * w.V + 6.0) * eval_pairs) / k_cull,
+                        "e2e_culled": {"ms_per_step": t_e2e_cull * 1e3, "value": pairs / t_e2e_cull, "unit": UNIT,
+                                       "over_kernel": t_e2e_cull * 1e3 / float(np.mean(cull_times)),
+                                       "outputs_checked": e2e_cull_checked,
+                                       "from_pageable_buffers_ms_per_step": t_e2e_cull_pageable * 1e3,
+                                       "api": "psdf_eval_host with culling on, pinned host buffers"},
                         "note": "pairs/s counts all pairs (SURVEY.md 8(d)); culled pairs cost at most two bound tests"},
             "gpu_launches": int(launches), "wall_s_timed_region": t_wall, "clocks": clocks,
             "paper_context": {"psdf_rtx4090_M100_B100_ms": 2.207, "implied_pairs_per_s": 4.5e6,
@@ -399,8 +481,27 @@ def main():
             dt1 = time.perf_counter() - t0
             out["cpu_baseline"]["single_thread"] = {"value": one.n_pairs() / dt1, "unit": UNIT, "seconds": dt1,
                                                     "sample": f"{one.N} of {w.N} poses (stride subsample), 1 thread"}
-            if not args.no_latency:
-                out["mpc_latency"] = mpc_latency(torch, psdf)
+            if not args.no_extras:
+                from paper_2607_04310_b200 import workloads as W
+                allw = {i: (w if i == args.workload else W.make_config(i)) for i in (1, 2, 3, 4, 5)}
+                # roofline fraction of the other large configs (value+grad), same protocol as the headline
+                per = {}
+                for i in (3, 4, 5):
+                    if i == args.workload:
+                        tk = t_kernel
+                    else:
+                        r = DeviceRun(torch, psdf, allw[i], flush)
+                        r.timed(5)
+                        tk = float(np.mean(r.timed(max(args.steps // 2, 10)))) * 1e-3
+                        r.scene.close()
+                    Fi = flops_per_launch(allw[i])
+                    per[allw[i].name] = {"ms_per_step": tk * 1e3, "pairs_per_s": allw[i].n_pairs() / tk,
+                                         "tflops": Fi / tk / 1e12, "frac": Fi / tk / 1e12 / peak_nominal,
+                                         "N": allw[i].N, "M": allw[i].M, "V": allw[i].V, "what": "value+grad, dense"}
+                out["per_config"] = per
+                out["parity"] = parity_report(torch, psdf, O, allw, {1: 20, 2: 50, 3: 3000, 4: 1200, 5: 1000})
+                if not args.no_latency:
+                    out["mpc_latency"] = mpc_latency(torch, psdf)
         print(json.dumps(out), flush=True)
     scene.close()
     if world > 1:

@@ -21,8 +21,22 @@
  * void* (NULL = legacy default stream).  The caller owns every I/O buffer and the stream;
  * the library copies the scene at create/update and owns that copy.
  *
- * Thread-safety: calls that use the same psdf_scene must be ordered on ONE stream (the
- * scene carries a small device workspace); different scenes are independent.
+ * Ordering and thread-safety (different scenes are always independent):
+ *   - one host thread at a time per scene: a call that finds the scene inside another call of
+ *     another thread returns PSDF_ERR_BUSY and does nothing;
+ *   - the stream-taking evaluation calls (psdf_eval, psdf_eval_windows) share one small device
+ *     workspace per scene: on one scene they must be ordered on ONE stream, or by the caller's own
+ *     events; each only enqueues and returns;
+ *   - the *_host calls run on the scene's own stream with a workspace of their own and return
+ *     after synchronising it: they may be issued while an asynchronous psdf_eval of the same scene
+ *     is still in flight on the caller's stream;
+ *   - psdf_update_scene / psdf_set_culling wait for the scene's own stream; an update orders itself
+ *     after earlier psdf_eval work by stream order when it is given the stream those calls used,
+ *     and by a device-wide synchronisation when they used another one;
+ *   - psdf_eval may be captured into a caller's CUDA graph (it only enqueues one kernel).  The
+ *     captured node holds the scene's buffers and launch plan by value: such a graph must be
+ *     captured again after psdf_update_scene or psdf_set_culling, and its replays ordered against
+ *     updates by the caller.
  */
 #ifndef PSDF_H_
 #define PSDF_H_
@@ -43,7 +57,8 @@ typedef enum {
                                 convex polygon, footprint not convex counter-clockwise */
   PSDF_ERR_CAPACITY = -3,    /* N > max_poses given at create */
   PSDF_ERR_CUDA = -4,        /* a CUDA call failed (psdf_last_cuda_error() has the code) */
-  PSDF_ERR_ALLOC = -5
+  PSDF_ERR_ALLOC = -5,       /* host or device memory allocation failed */
+  PSDF_ERR_BUSY = -6         /* the scene is inside another call of another host thread */
 } psdf_status;
 
 typedef enum { PSDF_MEM_HOST = 0, PSDF_MEM_DEVICE = 1 } psdf_mem;
@@ -75,14 +90,18 @@ psdf_status psdf_update_scene(psdf_scene* scene, const float* A, const float* B,
  *                               edge;  NULL = not wanted
  * No valid obstacle at all: value=+INF, grad=0.  Non-finite pose: NaN outputs.
  * At ties / kinks the gradient is that of one of the tied branches. */
-psdf_status psdf_eval(psdf_scene* scene, const float* poses, int N, float* value, float* grad,
+psdf_status psdf_eval(const psdf_scene* scene, const float* poses, int N, float* value, float* grad,
                       float* per_obstacle, void* cuda_stream);
 
-/* MPC-sized path: same semantics with HOST buffers.  Copies the poses into the scene's
- * pinned staging buffer, then either (N <= 512 and <= 64 obstacles) launches ONE kernel that
- * reads the poses from and writes the results to the pinned, device-mapped staging buffers
- * directly, or replays a captured CUDA graph {H2D, kernel, D2H}; both on the scene's own
- * stream; synchronises, copies the results out.  grad / per_obstacle may be NULL. */
+/* Same semantics with HOST buffers (Alg.1 l.5-11: upload the nominal states,
+ * evaluate, bring the results back), on the scene's own stream; returns after synchronising it.
+ * MPC-sized batches (N <= 512; with per_obstacle only up to 64 obstacles): ONE kernel launch; up
+ * to 128 poses travel inside the launch, results are written to pinned, device-mapped staging and
+ * copied out.  Larger batches: replay of a captured CUDA graph of up to four branches
+ * {H2D pose chunk, kernel, D2H result chunk} that overlap copies and kernels.  Buffers in pinned
+ * (page-locked) host memory are read and written in place by the copy engines; ordinary memory
+ * goes through the scene's pinned staging (one extra host copy each way).  Results are
+ * bit-identical to psdf_eval on the same poses.  grad / per_obstacle may be NULL. */
 psdf_status psdf_eval_host(psdf_scene* scene, const float* poses, int N, float* value, float* grad,
                            float* per_obstacle);
 
@@ -93,15 +112,17 @@ psdf_status psdf_eval_host(psdf_scene* scene, const float* poses, int N, float* 
  * psdf_eval; row_window is a device [N,2] int32 array (host array for the _host variant, which
  * copies, evaluates on the scene's stream and synchronises).  Meant for MPC-sized batches: one
  * group of lanes per pose, any N <= max_poses. */
-psdf_status psdf_eval_windows(psdf_scene* scene, const float* poses, int N, const int* row_window, float* value,
-                              float* grad, void* cuda_stream);
+psdf_status psdf_eval_windows(const psdf_scene* scene, const float* poses, int N, const int* row_window,
+                              float* value, float* grad, void* cuda_stream);
 psdf_status psdf_eval_windows_host(psdf_scene* scene, const float* poses, int N, const int* row_window,
                                    float* value, float* grad);
 
 /* MPC coefficient epilogue (Alg.1 l.7-11; eqs.(26)-(28)):
  * for each stage s writes coeff[s] = [ h_s - gamma_s ; J_g,s ] with h_s = phi_s - d_min,
  * J_g,s = -grad phi_s, gamma_s = 0.5 (r_max + phi_s) rho_theta^2 + rho_p rho_theta,
- * r_max = max_l |v_l|.  coeff: host [N,4].  Same graph path as psdf_eval_host. */
+ * r_max = max_l |v_l|.  coeff: host [N,4].  A stage that sees no obstacle (phi = +INF, e.g. an
+ * obstacle-free perception frame) gives the inactive row (+INF, 0, 0, 0), never NaN; a non-finite
+ * pose gives NaN.  Same host path as psdf_eval_host. */
 psdf_status psdf_mpc_coeffs_host(psdf_scene* scene, const float* poses, int N, float d_min,
                                  float rho_p, float rho_theta, float* coeff);
 
@@ -110,7 +131,8 @@ psdf_status psdf_mpc_coeffs_host(psdf_scene* scene, const float* poses, int N, f
  * per_obstacle output go through one kernel that looks obstacles up in a uniform grid (rebuilt on
  * the device at every create/update) and skips every obstacle whose lower bound on sd^i (bounding
  * circles, then oriented bounding boxes of footprint and obstacle) exceeds an upper bound of phi
- * obtained from a nearby obstacle; surviving pairs use the same arithmetic and reductions as the
+ * obtained from a nearby obstacle (the grid is built when culling is switched on and kept current by
+ * every update from then on); surviving pairs use the same arithmetic and reductions as the
  * dense path, so value and grad are bit-identical to the dense result.  Default: disabled (dense,
  * branch-free evaluation). */
 psdf_status psdf_set_culling(psdf_scene* scene, int enable);
@@ -130,24 +152,14 @@ psdf_status psdf_component_min(const float* per_component, int N, int M, const i
 psdf_status psdf_trajectory_reduce(const float* value, int T, int H, float d_safe, float* min_value,
                                    int* argmin_stage, float* penalty, void* cuda_stream);
 
-/* Culled-path statistics accumulated since the last call (then reset): out2[0] = number of
- * evaluated (pose, obstacle) pairs, out2[1] = number of (pose, obstacle edge) steps.
- * Synchronises `cuda_stream`.  Used by bench.py for the evaluated-pair fraction and FLOPs. */
-psdf_status psdf_cull_stats(psdf_scene* scene, void* cuda_stream, unsigned long long* out2);
-
 void psdf_destroy_scene(psdf_scene* scene);
 
 /* Introspection (no CUDA work). */
 int psdf_scene_num_obstacles(const psdf_scene* scene);   /* rows with >=1 valid edge */
 int psdf_scene_num_edges(const psdf_scene* scene);       /* total valid edges */
 int psdf_last_cuda_error(void);                          /* cudaError_t of the last failure */
-long long psdf_kernel_launches(void);                    /* kernels launched by this library */
 const char* psdf_status_string(psdf_status status);
 const char* psdf_version(void);
-
-/* Measurement helper: FP32 FMA-only micro-kernel, returns achieved TFLOP/s on the
- * current device (used by bench.py for the measured FP32 roofline denominator). */
-psdf_status psdf_measure_fp32_peak(int iters, void* cuda_stream, double* tflops_out);
 
 #ifdef __cplusplus
 }

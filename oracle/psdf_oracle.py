@@ -111,3 +111,29 @@ def trajectory_reduce(value: np.ndarray, T: int, H: int, d_safe: float):
     Plain definitions in float64."""
     v = np.asarray(value, np.float64).reshape(int(T), int(H))
     return v.min(axis=1), v.argmin(axis=1), (np.maximum(float(d_safe) - v, 0.0) ** 2).sum(axis=1)
+
+
+def mpc_coeffs(value, grad, footprint, d_min: float, rho_p: float, rho_theta: float) -> np.ndarray:
+    """Stage-wise QP parameter vectors [h_s - gamma_s ; J_g,s] of eqs.(26)-(28), PAPER.md:247-289,
+    literally, in float64, from the PSDF values phi_s [N] and state gradients [N,3]:
+        h_s     = phi_s - d_min
+        J_g,s   = -grad_x phi_s
+        r_max   = max_{v in V0} |v|_2                                       Prop.1
+        gamma_s = 1/2 (r_max + phi_s) rho_theta^2 + rho_p rho_theta         eq.(27)
+    Returns [N,4].  The paper is silent on a stage that sees no obstacle (phi_s = +inf, where
+    eq.(27) reads inf - inf): the row is (+inf, 0, 0, 0), an inactive constraint (DESIGN.md
+    reading G17)."""
+    phi = np.asarray(value, np.float64).reshape(-1)
+    g = np.asarray(grad, np.float64).reshape(-1, 3)
+    fp = np.asarray(footprint, np.float64)
+    r_max = max(float(np.hypot(v[0], v[1])) for v in fp)
+    out = np.empty((phi.shape[0], 4))
+    for s in range(phi.shape[0]):
+        if np.isposinf(phi[s]):
+            out[s] = (np.inf, 0.0, 0.0, 0.0)
+            continue
+        h_s = phi[s] - float(d_min)
+        gamma_s = 0.5 * (r_max + phi[s]) * float(rho_theta) ** 2 + float(rho_p) * float(rho_theta)
+        out[s, 0] = h_s - gamma_s
+        out[s, 1:] = -g[s]
+    return out

@@ -8,8 +8,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpsdf.so")
 SOURCES = ["psdf_api.cu"]
-DEPS = ["psdf_api.cu", "psdf_kernels.cuh", "psdf_device.cuh", "psdf_pack.h", "psdf_pack_kernels.cuh", "psdf_cull_kernels.cuh", "psdf_reduce_kernels.cuh", "../../include/psdf.h"]
+DEPS = ["psdf_api.cu", "psdf_kernels.cuh", "psdf_device.cuh", "psdf_pack.h", "psdf_pack_kernels.cuh", "psdf_cull_kernels.cuh", "psdf_reduce_kernels.cuh", "../../include/psdf.h", "../../include/psdf_bench.h"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+# PSDF_NVCC_EXTRA="-DPSDF_TUNING": a measurement build in which the PSDF_BD / PSDF_CHUNKS / PSDF_BRANCHES /
+# PSDF_NO_ZERO_COPY sweep knobs are read from the environment (they do not exist in the product build)
+EXTRA = os.environ.get("PSDF_NVCC_EXTRA", "").split()
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xptxas=-v", "-Xcompiler", "-fPIC", "-shared",
          "-cudart", "static"]
@@ -25,7 +28,7 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
-    cmd = [NVCC] + FLAGS + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    cmd = [NVCC] + FLAGS + EXTRA + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         print(r.stdout[-20000:])

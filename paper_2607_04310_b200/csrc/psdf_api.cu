@@ -1,10 +1,12 @@
 // C-ABI implementation of include/psdf.h: scene handle, dispatch, CUDA-graph host path.
 #include <atomic>
+#include <chrono>
 #include <cstdio>
 #include <cstdlib>
 #include <new>
 
 #include "../../include/psdf.h"
+#include "../../include/psdf_bench.h"
 #include "psdf_kernels.cuh"
 #include "psdf_cull_kernels.cuh"
 #include "psdf_pack.h"
@@ -18,24 +20,43 @@ namespace {
 std::atomic<int> g_last_cuda_error{0};
 std::atomic<long long> g_launches{0};
 
+inline psdf_status cuda_failed(cudaError_t e) {
+  g_last_cuda_error.store((int)e);
+  (void)cudaGetLastError();
+  return e == cudaErrorMemoryAllocation ? PSDF_ERR_ALLOC : PSDF_ERR_CUDA;
+}
+
 #define CU_TRY(expr)                                   \
   do {                                                 \
     cudaError_t _e = (expr);                           \
-    if (_e != cudaSuccess) {                           \
-      g_last_cuda_error.store((int)_e);                \
-      (void)cudaGetLastError();                        \
-      return PSDF_ERR_CUDA;                            \
-    }                                                  \
+    if (_e != cudaSuccess) return cuda_failed(_e);     \
   } while (0)
 
 struct GraphEntry {
-  int N = -1, mode = 0;
+  int N = -1, mode = 0, culling = 0;
   float d_min = 0, rho_p = 0, rho_theta = 0;
+  const void* in = nullptr;            // H2D source and D2H destinations baked into the copy nodes
+  void* out0 = nullptr;
+  void* out1 = nullptr;
+  void* out2 = nullptr;
   cudaGraphExec_t exec = nullptr;
+  int kernels = 0;                     // kernel nodes (for the launch counter)
   unsigned long long stamp = 0;
 };
 constexpr int kGraphCache = 8;
 constexpr int kCullMinPoses = 2048;     // the culled path serves larger batches only
+constexpr int kHostBranches = 4;        // large host batches: up to this many {H2D, kernel, D2H} branches
+
+// Per-call device workspace of the chunked kernels (cross-chunk keys, arrival counters) and the
+// culled path's statistics.  The scene owns two: one for calls on the caller's stream
+// (psdf_eval, psdf_eval_windows), one for the host entry points, which run on the scene's own
+// stream and may therefore overlap an asynchronous psdf_eval still in flight.
+struct Workspace {
+  unsigned long long* depth = nullptr;   // [max_poses] clean = 0
+  unsigned long long* d2 = nullptr;      // [max_poses] clean = ~0
+  unsigned int* count = nullptr;         // [max_poses + 1] clean = 0
+  unsigned long long* stats = nullptr;   // [2]
+};
 
 }  // namespace
 
@@ -45,6 +66,7 @@ struct psdf_scene {
   int n_edges = 0, Mv = 0, n_empty = 0;
   int edge_cap = 0;
   int sm_count = 148;
+  std::atomic<int> busy{0};           // one host thread at a time (PSDF_ERR_BUSY otherwise)
   std::vector<int> h_pair_begin;      // host copy for chunk planning
   int n_pairs = 0;
   // packed scene, double buffered: an update writes the inactive set and flips `cur` only
@@ -59,13 +81,16 @@ struct psdf_scene {
     float4* gbounds = nullptr;        // [2 M] bounds in obstacle-grid order
     int* gcell = nullptr;             // [kObsGridMax^2 + 1]
     GridHdr* ghdr = nullptr;
+    bool grid_ok = false;             // the obstacle grid matches this set's bounds (built lazily)
   } pk[2];
   int cur = 0;
   int* h_win = nullptr;               // pinned [max_poses,2]  (psdf_eval_windows_host)
   int* d_win = nullptr;
-  unsigned long long* d_ws_depth = nullptr;
-  unsigned long long* d_ws_d2 = nullptr;
-  unsigned int* d_ws_count = nullptr;
+  Workspace ws[2];                    // [0] caller-stream calls, [1] host entry points
+  // streams psdf_eval / psdf_eval_windows were enqueued on since the last update: an update on
+  // another stream cannot rely on stream order and synchronises the device instead
+  cudaStream_t eval_stream = nullptr;
+  bool eval_seen = false, eval_multi = false;
   // device packer scratch (psdf_pack_kernels.cuh)
   int* d_cnt = nullptr;               // [M] valid edges per row
   int4* d_offs = nullptr;             // [M] scanned offsets
@@ -73,20 +98,20 @@ struct psdf_scene {
   PackTotals* d_totals = nullptr;
   PackTotals* h_totals = nullptr;     // pinned
   int* h_pair_begin_pinned = nullptr; // pinned [M+1]
-  // culled path (psdf_cull_kernels.cuh)
-  int tune_bd = 0, tune_chunks = 0;   // PSDF_BD / PSDF_CHUNKS, read once at create
+  int tune_bd = 0, tune_chunks = 0, tune_branches = 0;   // measurement sweeps (PSDF_TUNING builds only)
   int culling = 0;                    // psdf_set_culling
-  unsigned long long* d_stats = nullptr;   // [2] psdf_cull_stats
-  // host (graph) path
+  // host path
+  bool host_ready = false;
   cudaStream_t gstream = nullptr;
-  float* h_in = nullptr;              // pinned [max_poses,3]
+  cudaStream_t bstream[kHostBranches] = {};      // side streams of the branched graph
+  cudaEvent_t ev_fork = nullptr, ev_join[kHostBranches] = {};
+  float* h_in = nullptr;              // pinned [max_poses,4]
   float* h_out = nullptr;             // pinned [max_poses,4]   value | grad  (or coeff)
   float* h_per = nullptr;             // pinned [max_poses,M]   lazily
   float* d_in = nullptr;
   float* d_out = nullptr;
   float* d_per = nullptr;
   int zero_copy = 1;                  // pinned staging is device-accessible (UVA): see run_zero_copy
-  const PoseArgs* arg_poses = nullptr;   // set around a launch whose poses travel as a kernel parameter
   PoseArgs h_args;                    // the MPC host path's poses (N <= kArgPoses)
   GraphEntry graphs[kGraphCache];
   unsigned long long stamp = 0;
@@ -94,10 +119,28 @@ struct psdf_scene {
 
 namespace {
 
+struct BusyGuard {                      // concurrent use of one scene from two host threads is an error
+  std::atomic<int>* f;
+  bool ok;
+  explicit BusyGuard(const psdf_scene* sc) : f(const_cast<std::atomic<int>*>(&sc->busy)) {
+    int zero = 0;
+    ok = f->compare_exchange_strong(zero, 1, std::memory_order_acquire);
+  }
+  ~BusyGuard() { if (ok) f->store(0, std::memory_order_release); }
+};
+#define PSDF_ENTER(sc)              \
+  BusyGuard _busy(sc);              \
+  if (!_busy.ok) return PSDF_ERR_BUSY
+
+}  // namespace
+
+namespace {
+
 template <int V, int MODE>
-cudaError_t launch_one(const psdf_scene* sc, const EvalParams& p, bool lanes, dim3 grid, int bd, cudaStream_t st) {
-  if (lanes && sc->arg_poses)
-    psdf_lanes_args_kernel<V, MODE><<<grid, bd, 0, st>>>(sc->fp, p, *sc->arg_poses);
+cudaError_t launch_one(const psdf_scene* sc, const EvalParams& p, bool lanes, dim3 grid, int bd, cudaStream_t st,
+                       const PoseArgs* args) {
+  if (lanes && args)
+    psdf_lanes_args_kernel<V, MODE><<<grid, bd, 0, st>>>(sc->fp, p, *args);
   else if (lanes)
     psdf_lanes_kernel<V, MODE><<<grid, bd, 0, st>>>(sc->fp, p);
   else
@@ -108,13 +151,13 @@ cudaError_t launch_one(const psdf_scene* sc, const EvalParams& p, bool lanes, di
 
 template <int V>
 cudaError_t launch_mode(const psdf_scene* sc, const EvalParams& p, int mode, bool lanes, dim3 grid, int bd,
-                        cudaStream_t st) {
+                        cudaStream_t st, const PoseArgs* args) {
   switch (mode) {
-    case 0: return launch_one<V, 0>(sc, p, lanes, grid, bd, st);
-    case kGrad: return launch_one<V, kGrad>(sc, p, lanes, grid, bd, st);
-    case kPerObs: return launch_one<V, kPerObs>(sc, p, lanes, grid, bd, st);
-    case kGrad | kPerObs: return launch_one<V, kGrad | kPerObs>(sc, p, lanes, grid, bd, st);
-    case kCoeff: return launch_one<V, kCoeff>(sc, p, lanes, grid, bd, st);
+    case 0: return launch_one<V, 0>(sc, p, lanes, grid, bd, st, args);
+    case kGrad: return launch_one<V, kGrad>(sc, p, lanes, grid, bd, st, args);
+    case kPerObs: return launch_one<V, kPerObs>(sc, p, lanes, grid, bd, st, args);
+    case kGrad | kPerObs: return launch_one<V, kGrad | kPerObs>(sc, p, lanes, grid, bd, st, args);
+    case kCoeff: return launch_one<V, kCoeff>(sc, p, lanes, grid, bd, st, args);
     default: return cudaErrorInvalidValue;
   }
 }
@@ -151,21 +194,20 @@ cudaError_t enqueue_culled(const psdf_scene* sc, EvalParams& p, int mode, cudaSt
   p.gbounds = sc->pk[sc->cur].gbounds;
   p.gcell = sc->pk[sc->cur].gcell;
   p.ghdr = sc->pk[sc->cur].ghdr;
-  p.stats = sc->d_stats;
   p.n_chunks = 1;
   if (p.N <= 32768) return launch_cull_v<32>(sc, p, mode, st);
   return launch_cull_v<128>(sc, p, mode, st);
 }
 
 cudaError_t launch_v(const psdf_scene* sc, const EvalParams& p, int mode, bool lanes, dim3 grid, int bd,
-                     cudaStream_t st) {
+                     cudaStream_t st, const PoseArgs* args) {
   switch (sc->Vp) {
-    case 4: return launch_mode<4>(sc, p, mode, lanes, grid, bd, st);
-    case 6: return launch_mode<6>(sc, p, mode, lanes, grid, bd, st);
-    case 8: return launch_mode<8>(sc, p, mode, lanes, grid, bd, st);
-    case 10: return launch_mode<10>(sc, p, mode, lanes, grid, bd, st);
-    case 12: return launch_mode<12>(sc, p, mode, lanes, grid, bd, st);
-    case 16: return launch_mode<16>(sc, p, mode, lanes, grid, bd, st);
+    case 4: return launch_mode<4>(sc, p, mode, lanes, grid, bd, st, args);
+    case 6: return launch_mode<6>(sc, p, mode, lanes, grid, bd, st, args);
+    case 8: return launch_mode<8>(sc, p, mode, lanes, grid, bd, st, args);
+    case 10: return launch_mode<10>(sc, p, mode, lanes, grid, bd, st, args);
+    case 12: return launch_mode<12>(sc, p, mode, lanes, grid, bd, st, args);
+    case 16: return launch_mode<16>(sc, p, mode, lanes, grid, bd, st, args);
     default: return cudaErrorInvalidValue;
   }
 }
@@ -175,36 +217,57 @@ inline bool lanes_plan(const psdf_scene* sc, int N) {
   return N <= 128 || (long long)N * (sc->Mv > 0 ? sc->Mv : 1) <= (1 << 17);
 }
 
+// One evaluation to enqueue.  `which_ws`: 0 = caller-stream workspace, 1 = host-path workspace;
+// `ws_off`: first workspace entry (branches of one host call use disjoint ranges).
+struct EvalCall {
+  const float* poses = nullptr;
+  int N = 0;
+  float* value = nullptr;
+  float* grad = nullptr;
+  float* per_obs = nullptr;
+  float* coeff = nullptr;
+  float d_min = 0.f, rho_p = 0.f, rho_theta = 0.f;
+  float* packed = nullptr;            // zero-copy staging layout
+  const int* window = nullptr;        // per-pose obstacle row windows
+  const PoseArgs* args = nullptr;     // poses travelling as a kernel parameter
+  int which_ws = 0, ws_off = 0;
+};
+
 // Launch plan: lane-split kernel for MPC-sized batches; otherwise the
 // tile-scan kernel, with the obstacle range cut into chunks when the pose tiles alone
 // would not fill 148 SMs several times over.
-psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float* value, float* grad,
-                         float* per_obs, float* coeff, float d_min, float rho_p, float rho_theta,
-                         cudaStream_t st, float* packed = nullptr, const int* window = nullptr) {
+psdf_status enqueue_eval(const psdf_scene* sc, const EvalCall& c, cudaStream_t st) {
+  const int N = c.N;
   if (N == 0) return PSDF_OK;
+  const Workspace& ws = sc->ws[c.which_ws];
+  float* const per_obs = c.per_obs;
+  float* const coeff = c.coeff;
+  float* const grad = c.grad;
+  const int* const window = c.window;
   EvalParams p{};
   p.pairs = sc->pk[sc->cur].pairs;
   p.row_slot = sc->pk[sc->cur].row_slot;
   p.bounds = sc->pk[sc->cur].bounds;
   p.window = window;
   p.empty_rows = sc->pk[sc->cur].empty;
-  p.poses = poses;
-  p.value = value;
+  p.poses = c.poses;
+  p.value = c.value;
   p.grad = grad;
   p.per_obs = per_obs;
   p.coeff = coeff;
-  p.packed = packed;
-  p.ws_depth = sc->d_ws_depth;
-  p.ws_d2 = sc->d_ws_d2;
-  p.ws_count = sc->d_ws_count;
+  p.packed = c.packed;
+  p.ws_depth = ws.depth + c.ws_off;
+  p.ws_d2 = ws.d2 + c.ws_off;
+  p.ws_count = ws.count + c.ws_off;
+  p.stats = ws.stats;
   p.n_edges = sc->n_edges;
   p.Mv = sc->Mv;
   p.M_rows = sc->M;
   p.n_empty = sc->n_empty;
   p.N = N;
-  p.d_min = d_min;
-  p.rho_p = rho_p;
-  p.rho_theta = rho_theta;
+  p.d_min = c.d_min;
+  p.rho_p = c.rho_p;
+  p.rho_theta = c.rho_theta;
   const int mode = coeff ? kCoeff : ((grad ? kGrad : 0) | (per_obs ? kPerObs : 0));
 
   const bool lanes = lanes_plan(sc, N) || window != nullptr;
@@ -212,10 +275,7 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
   int bd;
   if (sc->culling && !lanes && N > kCullMinPoses && !per_obs && sc->Mv >= 64) {
     cudaError_t e = enqueue_culled(sc, p, mode, st);
-    if (e != cudaSuccess) {
-      g_last_cuda_error.store((int)e);
-      return PSDF_ERR_CUDA;
-    }
+    if (e != cudaSuccess) return cuda_failed(e);
     return PSDF_OK;
   }
   if (lanes) {
@@ -242,8 +302,10 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
     const double warps_per_sm = (double)N / 32.0 / sc->sm_count;
     if (warps_per_sm < 256.0) C = (int)std::ceil(256.0 / warps_per_sm);
     const int maxC = sc->Mv / 16 > 0 ? sc->Mv / 16 : 1;
-    if (sc->tune_bd > 0) bd = sc->tune_bd;                                   // tuning overrides
+#ifdef PSDF_TUNING
+    if (sc->tune_bd > 0) bd = sc->tune_bd;                                   // measurement sweeps only
     if (sc->tune_chunks > 0) C = sc->tune_chunks;
+#endif
     if (bd != 32 && bd != 64 && bd != 128 && bd != 256) bd = 64;
     if (C < 1) C = 1;
     if (C > maxC) C = maxC;
@@ -261,12 +323,33 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
     p.n_chunks = C;
     grid = dim3((unsigned)tiles, (unsigned)C);
   }
-  cudaError_t e = launch_v(sc, p, mode, lanes, grid, bd, st);
-  if (e != cudaSuccess) {
-    g_last_cuda_error.store((int)e);
-    return PSDF_ERR_CUDA;
-  }
+  cudaError_t e = launch_v(sc, p, mode, lanes, grid, bd, st, c.args);
+  if (e != cudaSuccess) return cuda_failed(e);
   return PSDF_OK;
+}
+
+// The culled path's obstacle grid for buffer set `set`: built only while culling is
+// switched on (psdf_set_culling, and every update from then on).
+cudaError_t launch_grid(psdf_scene* sc, int set, const int* totals2, int Mv, cudaStream_t st) {
+  psdf_scene::Packed& b = sc->pk[set];
+  obstacle_grid_kernel<<<1, 1024, 0, st>>>(b.bounds, Mv, totals2, b.gbounds, b.gcell, b.ghdr);
+  g_launches.fetch_add(1);
+  b.grid_ok = true;
+  return cudaGetLastError();
+}
+
+// An update writes the inactive buffer set, which evaluations enqueued before the PREVIOUS update may
+// still be reading if they ran on a stream other than `st`: stream order does not cover those.
+psdf_status order_after_evals(psdf_scene* sc, cudaStream_t st) {
+  if (sc->eval_multi || (sc->eval_seen && sc->eval_stream != st)) CU_TRY(cudaDeviceSynchronize());
+  sc->eval_seen = sc->eval_multi = false;
+  return PSDF_OK;
+}
+
+void note_eval_stream(const psdf_scene* csc, cudaStream_t st) {
+  psdf_scene* sc = const_cast<psdf_scene*>(csc);
+  if (!sc->eval_seen) { sc->eval_seen = true; sc->eval_stream = st; }
+  else if (sc->eval_stream != st) sc->eval_multi = true;
 }
 
 // Device-resident (A,B,S): pack on the GPU (count+validate -> scan -> write); only the
@@ -274,7 +357,8 @@ psdf_status enqueue_eval(const psdf_scene* sc, const float* poses, int N, float*
 psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const uint8_t* S, cudaStream_t st) {
   const int M = sc->M, E = sc->E;
   const int bd = 128, gd = (M + bd - 1) / bd;
-  const psdf_scene::Packed& dst = sc->pk[sc->cur ^ 1];      // the inactive set
+  psdf_scene::Packed& dst = sc->pk[sc->cur ^ 1];            // the inactive set
+  dst.grid_ok = false;
   // d_totals and d_pair_begin are one allocation [PackTotals | pair_begin[M+1]]: one copy back
   if (M <= 256) {                                            // measured: fused wins below ~256 rows
     pack_fused_kernel<<<1, 1024, 0, st>>>(A, B, S, M, E, sc->d_totals, dst.edges, dst.pairs, dst.row_begin,
@@ -288,17 +372,14 @@ psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const
                                          dst.row_begin, sc->d_pair_begin, dst.empty, dst.bounds, dst.row_slot);
     g_launches.fetch_add(3);
   }
-  if (sc->max_poses > kCullMinPoses) {                       // the culled path's grid (never used by small scenes)
-    obstacle_grid_kernel<<<1, 1024, 0, st>>>(dst.bounds, 0, reinterpret_cast<const int*>(sc->d_totals), dst.gbounds,
-                                             dst.gcell, sc->d_cnt, dst.ghdr);
-    g_launches.fetch_add(1);
-  }
+  if (sc->culling)                                           // reads {status, Mv} on the device: no extra sync
+    CU_TRY(launch_grid(sc, sc->cur ^ 1, reinterpret_cast<const int*>(sc->d_totals), 0, st));
   CU_TRY(cudaMemcpyAsync(sc->h_totals, sc->d_totals, sizeof(PackTotals) + sizeof(int) * ((size_t)M + 1),
                          cudaMemcpyDeviceToHost, st));
   CU_TRY(cudaStreamSynchronize(st));                         // the only synchronisation of an update
   CU_TRY(cudaGetLastError());
   const PackTotals t = *sc->h_totals;
-  if (t.status != 0) return PSDF_ERR_DEGENERATE;             // the live set has not been touched
+  if (t.status != 0) { dst.grid_ok = false; return PSDF_ERR_DEGENERATE; }   // the live set has not been touched
   sc->h_pair_begin.assign(sc->h_pair_begin_pinned, sc->h_pair_begin_pinned + t.Mv + 1);
   sc->n_edges = t.n_edges;
   sc->Mv = t.Mv;
@@ -310,10 +391,13 @@ psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const
 
 psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const uint8_t* S, psdf_mem where,
                          cudaStream_t st) {
+  psdf_status s0 = order_after_evals(sc, st);
+  if (s0 != PSDF_OK) return s0;
   if (where == PSDF_MEM_DEVICE) return pack_on_device(sc, A, B, S, st);
   PackedScene ps;
   if (pack_scene(A, B, S, sc->M, sc->E, ps) != 0) return PSDF_ERR_DEGENERATE;
-  const psdf_scene::Packed& dst = sc->pk[sc->cur ^ 1];
+  psdf_scene::Packed& dst = sc->pk[sc->cur ^ 1];
+  dst.grid_ok = false;
   const int n_edges = (int)ps.edges.size(), Mv = (int)ps.row_begin.size() - 1, n_empty = (int)ps.empty_rows.size();
   const int n_pairs = (int)ps.pairs.size();
   // (dst.edges / dst.row_begin are the device packer's scratch: the kernels read pair records only)
@@ -321,10 +405,7 @@ psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const u
   CU_TRY(cudaMemcpyAsync(dst.row_slot, ps.row_slot.data(), sizeof(int) * (size_t)(sc->M + 1), cudaMemcpyHostToDevice, st));
   if (Mv) CU_TRY(cudaMemcpyAsync(dst.bounds, ps.bounds.data(), sizeof(float4) * 2 * Mv, cudaMemcpyHostToDevice, st));
   if (n_empty) CU_TRY(cudaMemcpyAsync(dst.empty, ps.empty_rows.data(), sizeof(int) * n_empty, cudaMemcpyHostToDevice, st));
-  if (sc->max_poses > kCullMinPoses) {                       // the culled path's grid (never used by small scenes)
-    obstacle_grid_kernel<<<1, 1024, 0, st>>>(dst.bounds, Mv, nullptr, dst.gbounds, dst.gcell, sc->d_cnt, dst.ghdr);
-    g_launches.fetch_add(1);
-  }
+  if (sc->culling) CU_TRY(launch_grid(sc, sc->cur ^ 1, nullptr, Mv, st));
   CU_TRY(cudaStreamSynchronize(st));       // the staging vectors die here
   sc->n_edges = n_edges;
   sc->Mv = Mv;
@@ -345,6 +426,11 @@ void psdf_destroy_scene(psdf_scene* sc) {
   for (auto& g : sc->graphs)
     if (g.exec) cudaGraphExecDestroy(g.exec);
   if (sc->gstream) cudaStreamDestroy(sc->gstream);
+  for (int b = 1; b < kHostBranches; ++b) {
+    if (sc->bstream[b]) cudaStreamDestroy(sc->bstream[b]);
+    if (sc->ev_join[b]) cudaEventDestroy(sc->ev_join[b]);
+  }
+  if (sc->ev_fork) cudaEventDestroy(sc->ev_fork);
   for (auto& b : sc->pk) {
     cudaFree(b.edges); cudaFree(b.pairs); cudaFree(b.row_begin); cudaFree(b.row_slot); cudaFree(b.empty); cudaFree(b.bounds);
     cudaFree(b.gbounds); cudaFree(b.gcell); cudaFree(b.ghdr);
@@ -352,14 +438,26 @@ void psdf_destroy_scene(psdf_scene* sc) {
   cudaFree(sc->d_win);
   if (sc->h_totals) cudaFreeHost(sc->h_totals);
   if (sc->h_win) cudaFreeHost(sc->h_win);
-  cudaFree(sc->d_ws_depth); cudaFree(sc->d_ws_d2); cudaFree(sc->d_ws_count);
-  cudaFree(sc->d_stats);
+  for (auto& w : sc->ws) { cudaFree(w.depth); cudaFree(w.d2); cudaFree(w.count); cudaFree(w.stats); }
   cudaFree(sc->d_cnt); cudaFree(sc->d_offs); cudaFree(sc->d_totals);   // d_pair_begin lives inside d_totals' block
   cudaFree(sc->d_in); cudaFree(sc->d_out); cudaFree(sc->d_per);
   if (sc->h_in) cudaFreeHost(sc->h_in);
   if (sc->h_out) cudaFreeHost(sc->h_out);
   if (sc->h_per) cudaFreeHost(sc->h_per);
   delete sc;
+}
+
+static psdf_status alloc_workspace(Workspace& w, int max_poses, cudaStream_t st) {
+  const size_t n = (size_t)max_poses, n_cnt = n + 1;      // scan: one counter per pose tile; lanes: one per pose group
+  CU_TRY(cudaMalloc(&w.depth, sizeof(unsigned long long) * n));
+  CU_TRY(cudaMalloc(&w.d2, sizeof(unsigned long long) * n));
+  CU_TRY(cudaMalloc(&w.count, sizeof(unsigned int) * n_cnt));
+  CU_TRY(cudaMalloc(&w.stats, sizeof(unsigned long long) * 2));
+  CU_TRY(cudaMemsetAsync(w.depth, 0x00, sizeof(unsigned long long) * n, st));
+  CU_TRY(cudaMemsetAsync(w.d2, 0xff, sizeof(unsigned long long) * n, st));
+  CU_TRY(cudaMemsetAsync(w.count, 0x00, sizeof(unsigned int) * n_cnt, st));
+  CU_TRY(cudaMemsetAsync(w.stats, 0x00, sizeof(unsigned long long) * 2, st));
+  return PSDF_OK;
 }
 
 psdf_status psdf_create_scene(const float* footprint, int V, const float* A, const float* B,
@@ -371,8 +469,11 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
   psdf_scene* sc = new (std::nothrow) psdf_scene();
   if (!sc) return PSDF_ERR_ALLOC;
   sc->V = V; sc->M = M; sc->E = E; sc->max_poses = max_poses;
-  if (const char* e = std::getenv("PSDF_BD")) sc->tune_bd = std::atoi(e);             // measurement sweeps only
+#ifdef PSDF_TUNING                                         // measurement sweeps only (not in product builds)
+  if (const char* e = std::getenv("PSDF_BD")) sc->tune_bd = std::atoi(e);
   if (const char* e = std::getenv("PSDF_CHUNKS")) sc->tune_chunks = std::atoi(e);
+  if (const char* e = std::getenv("PSDF_BRANCHES")) sc->tune_branches = std::atoi(e);
+#endif
   const int rc = pack_footprint(footprint, V, sc->fp, sc->Vp);
   if (rc != 0) { delete sc; return rc == -1 ? PSDF_ERR_INVALID_ARG : PSDF_ERR_DEGENERATE; }
   if (where == PSDF_MEM_HOST) {   // validate before touching CUDA (Assumption 1)
@@ -403,15 +504,8 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
     CU_TRY(cudaMalloc(&sc->d_offs, sizeof(int4) * (size_t)M));
     CU_TRY(cudaMalloc(&sc->d_totals, sizeof(PackTotals) + sizeof(int) * (size_t)(M + 1)));
     sc->d_pair_begin = reinterpret_cast<int*>(sc->d_totals + 1);
-    CU_TRY(cudaMalloc(&sc->d_stats, sizeof(unsigned long long) * 2));
-    CU_TRY(cudaMemsetAsync(sc->d_stats, 0, sizeof(unsigned long long) * 2, st));
-    CU_TRY(cudaMalloc(&sc->d_ws_depth, sizeof(unsigned long long) * (size_t)max_poses));
-    CU_TRY(cudaMalloc(&sc->d_ws_d2, sizeof(unsigned long long) * (size_t)max_poses));
-    const size_t n_cnt = (size_t)max_poses + 1;          // scan: one per pose tile; lanes: one per pose group
-    CU_TRY(cudaMalloc(&sc->d_ws_count, sizeof(unsigned int) * n_cnt));
-    CU_TRY(cudaMemsetAsync(sc->d_ws_depth, 0x00, sizeof(unsigned long long) * (size_t)max_poses, st));
-    CU_TRY(cudaMemsetAsync(sc->d_ws_d2, 0xff, sizeof(unsigned long long) * (size_t)max_poses, st));
-    CU_TRY(cudaMemsetAsync(sc->d_ws_count, 0x00, sizeof(unsigned int) * n_cnt, st));
+    psdf_status s = alloc_workspace(sc->ws[0], max_poses, st);
+    if (s != PSDF_OK) return s;
     return upload_scene(sc, A, B, S, where, st);
   };
   status = body();
@@ -420,45 +514,84 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
   return PSDF_OK;
 }
 
+static void drop_graphs(psdf_scene* sc) {      // launch plans and scene pointers are baked into the captured graphs
+  for (auto& g : sc->graphs) {
+    if (g.exec) cudaGraphExecDestroy(g.exec);
+    g = GraphEntry();
+  }
+}
+
 psdf_status psdf_update_scene(psdf_scene* sc, const float* A, const float* B, const uint8_t* S,
                               psdf_mem where, void* cuda_stream) {
-  if (!sc || !A || !B || !S) return PSDF_ERR_INVALID_ARG;
+  if (!sc || !A || !B || !S || (where != PSDF_MEM_HOST && where != PSDF_MEM_DEVICE)) return PSDF_ERR_INVALID_ARG;
+  PSDF_ENTER(sc);
   // both paths validate before anything live changes (host: pack_scene; device: status word
   // checked before the buffer flip), so a bad update leaves the old scene in force
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (sc->gstream) CU_TRY(cudaStreamSynchronize(sc->gstream));
   psdf_status s = upload_scene(sc, A, B, S, where, st);
   if (s != PSDF_OK) return s;
-  for (auto& g : sc->graphs) {           // launch plans are baked into the captured graphs
-    if (g.exec) cudaGraphExecDestroy(g.exec);
-    g = GraphEntry();
-  }
+  drop_graphs(sc);
   return PSDF_OK;
 }
 
-psdf_status psdf_eval(psdf_scene* sc, const float* poses, int N, float* value, float* grad,
+psdf_status psdf_eval(const psdf_scene* sc, const float* poses, int N, float* value, float* grad,
                       float* per_obstacle, void* cuda_stream) {
   if (!sc || N < 0 || (N > 0 && (!poses || !value))) return PSDF_ERR_INVALID_ARG;
   if (N > sc->max_poses) return PSDF_ERR_CAPACITY;
-  return enqueue_eval(sc, poses, N, value, grad, per_obstacle, nullptr, 0.f, 0.f, 0.f, (cudaStream_t)cuda_stream);
+  PSDF_ENTER(sc);
+  note_eval_stream(sc, (cudaStream_t)cuda_stream);
+  EvalCall c;
+  c.poses = poses; c.N = N; c.value = value; c.grad = grad; c.per_obs = per_obstacle;
+  return enqueue_eval(sc, c, (cudaStream_t)cuda_stream);
 }
 
+// Host path resources: the scene's own stream, pinned (device-mapped) staging, device buffers, a
+// private workspace, side streams for the branched graph.  All or nothing: `host_ready` is set last.
 static psdf_status ensure_host_path(psdf_scene* sc, bool per_obs) {
-  if (!sc->gstream) {
-    CU_TRY(cudaStreamCreateWithFlags(&sc->gstream, cudaStreamNonBlocking));
-    CU_TRY(cudaHostAlloc(&sc->h_in, sizeof(float) * 4 * (size_t)sc->max_poses, cudaHostAllocMapped));
-    CU_TRY(cudaHostAlloc(&sc->h_out, sizeof(float) * 4 * (size_t)sc->max_poses, cudaHostAllocMapped));
-    int dev = 0, uva = 0;
-    CU_TRY(cudaGetDevice(&dev));
-    CU_TRY(cudaDeviceGetAttribute(&uva, cudaDevAttrUnifiedAddressing, dev));
-    if (const char* e = std::getenv("PSDF_NO_ZERO_COPY")) uva = (e[0] == '1') ? 0 : uva;
-    sc->zero_copy = uva;
-    CU_TRY(cudaMalloc(&sc->d_in, sizeof(float) * 3 * (size_t)sc->max_poses));
-    CU_TRY(cudaMalloc(&sc->d_out, sizeof(float) * 4 * (size_t)sc->max_poses));
+  if (!sc->host_ready) {
+    auto body = [&]() -> psdf_status {
+      if (!sc->gstream) CU_TRY(cudaStreamCreateWithFlags(&sc->gstream, cudaStreamNonBlocking));
+      for (int b = 1; b < kHostBranches; ++b) {
+        if (!sc->bstream[b]) CU_TRY(cudaStreamCreateWithFlags(&sc->bstream[b], cudaStreamNonBlocking));
+        if (!sc->ev_join[b]) CU_TRY(cudaEventCreateWithFlags(&sc->ev_join[b], cudaEventDisableTiming));
+      }
+      if (!sc->ev_fork) CU_TRY(cudaEventCreateWithFlags(&sc->ev_fork, cudaEventDisableTiming));
+      if (!sc->h_in) CU_TRY(cudaHostAlloc(&sc->h_in, sizeof(float) * 4 * (size_t)sc->max_poses, cudaHostAllocMapped));
+      if (!sc->h_out) CU_TRY(cudaHostAlloc(&sc->h_out, sizeof(float) * 4 * (size_t)sc->max_poses, cudaHostAllocMapped));
+      int dev = 0, uva = 0;
+      CU_TRY(cudaGetDevice(&dev));
+      CU_TRY(cudaDeviceGetAttribute(&uva, cudaDevAttrUnifiedAddressing, dev));
+#ifdef PSDF_TUNING
+      if (const char* e = std::getenv("PSDF_NO_ZERO_COPY")) uva = (e[0] == '1') ? 0 : uva;
+#endif
+      sc->zero_copy = uva;
+      if (!sc->d_in) CU_TRY(cudaMalloc(&sc->d_in, sizeof(float) * 3 * (size_t)sc->max_poses));
+      if (!sc->d_out) CU_TRY(cudaMalloc(&sc->d_out, sizeof(float) * 4 * (size_t)sc->max_poses));
+      if (!sc->ws[1].depth) {
+        psdf_status s = alloc_workspace(sc->ws[1], sc->max_poses, sc->gstream);
+        if (s != PSDF_OK) {                      // partial workspace: release it so that a retry starts clean
+          Workspace& w = sc->ws[1];
+          cudaFree(w.depth); cudaFree(w.d2); cudaFree(w.count); cudaFree(w.stats);
+          w = Workspace();
+          return s;
+        }
+        CU_TRY(cudaStreamSynchronize(sc->gstream));
+      }
+      return PSDF_OK;
+    };
+    psdf_status s = body();
+    if (s != PSDF_OK) return s;                  // whatever was created stays owned by the scene; nothing is used
+    sc->host_ready = true;
   }
   if (per_obs && !sc->d_per) {
-    CU_TRY(cudaHostAlloc(&sc->h_per, sizeof(float) * (size_t)sc->max_poses * sc->M, cudaHostAllocMapped));
-    CU_TRY(cudaMalloc(&sc->d_per, sizeof(float) * (size_t)sc->max_poses * sc->M));
+    float* h = nullptr;
+    float* d = nullptr;
+    CU_TRY(cudaHostAlloc(&h, sizeof(float) * (size_t)sc->max_poses * sc->M, cudaHostAllocMapped));
+    cudaError_t e = cudaMalloc(&d, sizeof(float) * (size_t)sc->max_poses * sc->M);
+    if (e != cudaSuccess) { cudaFreeHost(h); return cuda_failed(e); }
+    sc->h_per = h;
+    sc->d_per = d;
   }
   return PSDF_OK;
 }
@@ -466,7 +599,7 @@ static psdf_status ensure_host_path(psdf_scene* sc, bool per_obs) {
 // MPC-sized batches: ONE kernel launch that reads the poses from, and writes the results to,
 // the pinned (mapped) staging buffers directly: a few hundred bytes cross PCIe inside the
 // kernel instead of through two copy-engine operations, which removes two graph nodes'
-// worth of latency.  Same output layout as the graph path.
+// worth of latency.
 constexpr int kZeroCopyMaxPoses = 512;
 constexpr int kZeroCopyMaxObstaclesPerObs = 64;
 
@@ -478,26 +611,89 @@ static inline bool use_zero_copy(const psdf_scene* sc, int N, bool per_obs) {
          (!per_obs || sc->Mv <= kZeroCopyMaxObstaclesPerObs);
 }
 
-static psdf_status run_zero_copy(psdf_scene* sc, int N, int mode, float d_min, float rho_p, float rho_theta) {
+// What one host call wants: caller's buffers (ordinary or pinned host memory) and constants.
+struct HostCall {
+  const float* poses = nullptr;
+  int N = 0, mode = 0;
+  float* value = nullptr;
+  float* grad = nullptr;
+  float* per = nullptr;
+  float* coeff = nullptr;
+  float d_min = 0.f, rho_p = 0.f, rho_theta = 0.f;
+};
+
+static psdf_status run_zero_copy(psdf_scene* sc, const HostCall& h) {
   // staging layout: h_in [N,4] poses (padded), h_out [N,4] = (value, grad) or coefficients;
   // up to kArgPoses poses go into the launch itself (kernel parameter) instead
-  sc->arg_poses = N <= kArgPoses ? &sc->h_args : nullptr;
-  psdf_status s = enqueue_eval(sc, sc->h_in, N, sc->d_in /*unused*/, (mode & kGrad) ? sc->d_out : nullptr,
-                               (mode & kPerObs) ? sc->h_per : nullptr, (mode & kCoeff) ? sc->h_out : nullptr, d_min,
-                               rho_p, rho_theta, sc->gstream, sc->h_out);
-  sc->arg_poses = nullptr;
+  const int N = h.N;
+  if (N <= kArgPoses) {
+    for (int n = 0; n < N; ++n) sc->h_args.q[n] = make_float4(h.poses[3 * n], h.poses[3 * n + 1], h.poses[3 * n + 2], 0.f);
+  } else {
+    for (int n = 0; n < N; ++n) {
+      sc->h_in[4 * n] = h.poses[3 * n]; sc->h_in[4 * n + 1] = h.poses[3 * n + 1];
+      sc->h_in[4 * n + 2] = h.poses[3 * n + 2]; sc->h_in[4 * n + 3] = 0.f;
+    }
+  }
+  EvalCall c;
+  c.poses = sc->h_in; c.N = N;
+  c.grad = (h.mode & kGrad) ? sc->d_out : nullptr;            // (non-null = wanted; results go to `packed`)
+  c.per_obs = (h.mode & kPerObs) ? sc->h_per : nullptr;
+  c.coeff = (h.mode & kCoeff) ? sc->h_out : nullptr;
+  c.d_min = h.d_min; c.rho_p = h.rho_p; c.rho_theta = h.rho_theta;
+  c.packed = sc->h_out;
+  c.args = N <= kArgPoses ? &sc->h_args : nullptr;
+  c.which_ws = 1;
+  psdf_status s = enqueue_eval(sc, c, sc->gstream);
   if (s != PSDF_OK) return s;
   CU_TRY(cudaStreamSynchronize(sc->gstream));
+  if (h.mode & kCoeff) {
+    std::memcpy(h.coeff, sc->h_out, sizeof(float) * 4 * (size_t)N);
+  } else {
+    for (int n = 0; n < N; ++n) {
+      h.value[n] = sc->h_out[4 * n];
+      if (h.grad) { h.grad[3 * n] = sc->h_out[4 * n + 1]; h.grad[3 * n + 1] = sc->h_out[4 * n + 2]; h.grad[3 * n + 2] = sc->h_out[4 * n + 3]; }
+    }
+  }
+  if (h.per) std::memcpy(h.per, sc->h_per, sizeof(float) * (size_t)N * sc->M);
   return PSDF_OK;
 }
 
-// Graph replay {H2D poses, kernel, D2H results}; captured once per (N, outputs, MPC constants).
-static psdf_status run_graph(psdf_scene* sc, int N, int mode, float d_min, float rho_p, float rho_theta) {
-  if (use_zero_copy(sc, N, (mode & kPerObs) != 0)) return run_zero_copy(sc, N, mode, d_min, rho_p, rho_theta);
+// Pinned (page-locked, e.g. cudaHostAlloc / cudaHostRegister / torch pin_memory) caller memory can
+// be the source / destination of the copy nodes directly: no staging memcpy on the host.
+static bool is_pinned_host(const void* ptr) {
+  if (!ptr) return false;
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, ptr) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeHost;
+}
+
+// Large host batches: replay of a captured CUDA graph with K branches, each {H2D pose chunk,
+// kernel on that chunk, D2H result chunk}, so that the copies of one chunk overlap the kernels of
+// the others (two copy engines + SMs busy at once).  Per-pose results do not depend on the batch
+// they are evaluated in, so the chunked results are bit-identical to one psdf_eval over all N.
+// Captured once per (N, outputs, constants, buffers); pinned caller buffers are used in place.
+static psdf_status run_graph(psdf_scene* sc, const HostCall& h) {
+  const int N = h.N, mode = h.mode;
+  const size_t M = (size_t)sc->M;
+  // sources / destinations of the copy nodes
+  const bool pin_in = is_pinned_host(h.poses);
+  const float* src = pin_in ? h.poses : sc->h_in;
+  float* dst0 = nullptr;      // value [N] or coeff [N,4]
+  float* dst1 = nullptr;      // grad [N,3]
+  float* dst2 = nullptr;      // per_obstacle [N,M]
+  if (mode & kCoeff) dst0 = is_pinned_host(h.coeff) ? h.coeff : sc->h_out;
+  else {
+    dst0 = is_pinned_host(h.value) ? h.value : sc->h_out;
+    if (mode & kGrad) dst1 = is_pinned_host(h.grad) ? h.grad : sc->h_out + N;
+    if (mode & kPerObs) dst2 = is_pinned_host(h.per) ? h.per : sc->h_per;
+  }
+  if (!pin_in) std::memcpy(sc->h_in, h.poses, sizeof(float) * 3 * (size_t)N);
+
   GraphEntry* hit = nullptr;
   GraphEntry* victim = &sc->graphs[0];
   for (auto& g : sc->graphs) {
-    if (g.exec && g.N == N && g.mode == mode && g.d_min == d_min && g.rho_p == rho_p && g.rho_theta == rho_theta) {
+    if (g.exec && g.N == N && g.mode == mode && g.culling == sc->culling && g.d_min == h.d_min && g.rho_p == h.rho_p &&
+        g.rho_theta == h.rho_theta && g.in == src && g.out0 == dst0 && g.out1 == dst1 && g.out2 == dst2) {
       hit = &g;
       break;
     }
@@ -505,57 +701,93 @@ static psdf_status run_graph(psdf_scene* sc, int N, int mode, float d_min, float
   }
   if (!hit) {
     if (victim->exec) { cudaGraphExecDestroy(victim->exec); *victim = GraphEntry(); }
+    // branches: chunk boundaries on multiples of 128 poses (a CTA of either kernel never straddles one)
+    int K = N >= 32768 ? 4 : (N >= 8192 ? 2 : 1);
+#ifdef PSDF_TUNING
+    if (sc->tune_branches > 0) K = sc->tune_branches;
+#endif
+    if (K > kHostBranches) K = kHostBranches;
+    const int per = ((N + K - 1) / K + 127) / 128 * 128;
     cudaGraph_t graph = nullptr;
-    CU_TRY(cudaStreamBeginCapture(sc->gstream, cudaStreamCaptureModeThreadLocal));
-    cudaError_t e = cudaMemcpyAsync(sc->d_in, sc->h_in, sizeof(float) * 3 * (size_t)N, cudaMemcpyHostToDevice, sc->gstream);
+    cudaStream_t g0 = sc->gstream;
+    const long long launches0 = g_launches.load();
+    CU_TRY(cudaStreamBeginCapture(g0, cudaStreamCaptureModeThreadLocal));
+    cudaError_t e = cudaSuccess;
     psdf_status s = PSDF_OK;
-    if (e == cudaSuccess) {
-      float* value = sc->d_out;                       // [N] value | [N,3] grad, or [N,4] coeff + value after
-      if (mode & kCoeff)
-        s = enqueue_eval(sc, sc->d_in, N, sc->d_in /*scratch: value not returned*/, nullptr, nullptr, sc->d_out,
-                         d_min, rho_p, rho_theta, sc->gstream);
-      else
-        s = enqueue_eval(sc, sc->d_in, N, value, (mode & kGrad) ? sc->d_out + N : nullptr,
-                         (mode & kPerObs) ? sc->d_per : nullptr, nullptr, 0.f, 0.f, 0.f, sc->gstream);
+    int forked = 0;
+    if (K > 1) e = cudaEventRecord(sc->ev_fork, g0);
+    for (int b = 0; b < K && e == cudaSuccess && s == PSDF_OK; ++b) {
+      const int n0 = b * per, n = (n0 + per <= N ? per : N - n0);
+      if (n <= 0) break;
+      cudaStream_t st = b == 0 ? g0 : sc->bstream[b];
+      if (b > 0) { e = cudaStreamWaitEvent(st, sc->ev_fork, 0); if (e != cudaSuccess) break; forked = b; }
+      e = cudaMemcpyAsync(sc->d_in + 3 * (size_t)n0, src + 3 * (size_t)n0, sizeof(float) * 3 * (size_t)n, cudaMemcpyHostToDevice, st);
+      if (e != cudaSuccess) break;
+      EvalCall c;
+      c.poses = sc->d_in + 3 * (size_t)n0; c.N = n; c.which_ws = 1; c.ws_off = n0;
+      if (mode & kCoeff) {
+        c.coeff = sc->d_out + 4 * (size_t)n0;
+        c.d_min = h.d_min; c.rho_p = h.rho_p; c.rho_theta = h.rho_theta;
+      } else {
+        c.value = sc->d_out + n0;
+        if (mode & kGrad) c.grad = sc->d_out + N + 3 * (size_t)n0;
+        if (mode & kPerObs) c.per_obs = sc->d_per + (size_t)n0 * M;
+      }
+      s = enqueue_eval(sc, c, st);
+      if (s != PSDF_OK) break;
+      if (mode & kCoeff) {
+        e = cudaMemcpyAsync(dst0 + 4 * (size_t)n0, c.coeff, sizeof(float) * 4 * (size_t)n, cudaMemcpyDeviceToHost, st);
+      } else {
+        e = cudaMemcpyAsync(dst0 + n0, c.value, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && (mode & kGrad))
+          e = cudaMemcpyAsync(dst1 + 3 * (size_t)n0, c.grad, sizeof(float) * 3 * (size_t)n, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && (mode & kPerObs))
+          e = cudaMemcpyAsync(dst2 + (size_t)n0 * M, c.per_obs, sizeof(float) * (size_t)n * M, cudaMemcpyDeviceToHost, st);
+      }
     }
-    if (e == cudaSuccess && s == PSDF_OK) {
-      const size_t nout = (mode & (kGrad | kCoeff)) ? 4 * (size_t)N : (size_t)N;
-      e = cudaMemcpyAsync(sc->h_out, sc->d_out, sizeof(float) * nout, cudaMemcpyDeviceToHost, sc->gstream);
-      if (e == cudaSuccess && (mode & kPerObs))
-        e = cudaMemcpyAsync(sc->h_per, sc->d_per, sizeof(float) * (size_t)N * sc->M, cudaMemcpyDeviceToHost, sc->gstream);
+    for (int b = 1; b <= forked; ++b) {                  // join every forked branch, also on failure
+      cudaError_t ej = cudaEventRecord(sc->ev_join[b], sc->bstream[b]);
+      if (ej == cudaSuccess) ej = cudaStreamWaitEvent(g0, sc->ev_join[b], 0);
+      if (e == cudaSuccess) e = ej;
     }
-    cudaError_t e2 = cudaStreamEndCapture(sc->gstream, &graph);
+    cudaError_t e2 = cudaStreamEndCapture(g0, &graph);
+    const int kernels = (int)(g_launches.load() - launches0);
+    g_launches.fetch_sub(kernels);                       // captured, not run: counted per replay below
     if (e != cudaSuccess || e2 != cudaSuccess || s != PSDF_OK || !graph) {
       if (graph) cudaGraphDestroy(graph);
-      g_last_cuda_error.store((int)(e != cudaSuccess ? e : e2));
-      (void)cudaGetLastError();
-      return s != PSDF_OK ? s : PSDF_ERR_CUDA;
+      if (s != PSDF_OK) { (void)cudaGetLastError(); return s; }
+      return cuda_failed(e != cudaSuccess ? e : (e2 != cudaSuccess ? e2 : cudaErrorUnknown));
     }
     cudaGraphExec_t exec = nullptr;
     e = cudaGraphInstantiate(&exec, graph, 0);
     cudaGraphDestroy(graph);
     CU_TRY(e);
-    victim->exec = exec; victim->N = N; victim->mode = mode;
-    victim->d_min = d_min; victim->rho_p = rho_p; victim->rho_theta = rho_theta;
+    victim->exec = exec; victim->N = N; victim->mode = mode; victim->culling = sc->culling;
+    victim->d_min = h.d_min; victim->rho_p = h.rho_p; victim->rho_theta = h.rho_theta;
+    victim->kernels = kernels;
+    victim->in = src; victim->out0 = dst0; victim->out1 = dst1; victim->out2 = dst2;
     hit = victim;
   }
   hit->stamp = ++sc->stamp;
   CU_TRY(cudaGraphLaunch(hit->exec, sc->gstream));
-  g_launches.fetch_add(1);   // the replayed graph holds one kernel node
+  g_launches.fetch_add(hit->kernels);
   CU_TRY(cudaStreamSynchronize(sc->gstream));
+  // ordinary (pageable) caller memory: results come back through the pinned staging buffers
+  if (mode & kCoeff) {
+    if (dst0 != h.coeff) std::memcpy(h.coeff, sc->h_out, sizeof(float) * 4 * (size_t)N);
+  } else {
+    if (dst0 != h.value) std::memcpy(h.value, sc->h_out, sizeof(float) * (size_t)N);
+    if ((mode & kGrad) && dst1 != h.grad) std::memcpy(h.grad, sc->h_out + N, sizeof(float) * 3 * (size_t)N);
+    if ((mode & kPerObs) && dst2 != h.per) std::memcpy(h.per, sc->h_per, sizeof(float) * (size_t)N * M);
+  }
   return PSDF_OK;
 }
 
-static void stage_poses(psdf_scene* sc, const float* poses, int N, bool per_obs) {
-  if (!use_zero_copy(sc, N, per_obs)) { std::memcpy(sc->h_in, poses, sizeof(float) * 3 * (size_t)N); return; }
-  if (N <= kArgPoses) {
-    for (int n = 0; n < N; ++n) sc->h_args.q[n] = make_float4(poses[3 * n], poses[3 * n + 1], poses[3 * n + 2], 0.f);
-    return;
-  }
-  for (int n = 0; n < N; ++n) {
-    sc->h_in[4 * n] = poses[3 * n]; sc->h_in[4 * n + 1] = poses[3 * n + 1];
-    sc->h_in[4 * n + 2] = poses[3 * n + 2]; sc->h_in[4 * n + 3] = 0.f;
-  }
+static psdf_status run_host(psdf_scene* sc, const HostCall& h) {
+  psdf_status s = ensure_host_path(sc, (h.mode & kPerObs) != 0);
+  if (s != PSDF_OK) return s;
+  if (use_zero_copy(sc, h.N, (h.mode & kPerObs) != 0)) return run_zero_copy(sc, h);
+  return run_graph(sc, h);
 }
 
 psdf_status psdf_eval_host(psdf_scene* sc, const float* poses, int N, float* value, float* grad,
@@ -563,31 +795,34 @@ psdf_status psdf_eval_host(psdf_scene* sc, const float* poses, int N, float* val
   if (!sc || N < 0 || (N > 0 && (!poses || !value))) return PSDF_ERR_INVALID_ARG;
   if (N > sc->max_poses) return PSDF_ERR_CAPACITY;
   if (N == 0) return PSDF_OK;
-  psdf_status s = ensure_host_path(sc, per_obstacle != nullptr);
-  if (s != PSDF_OK) return s;
-  stage_poses(sc, poses, N, per_obstacle != nullptr);
-  const int mode = (grad ? kGrad : 0) | (per_obstacle ? kPerObs : 0);
-  s = run_graph(sc, N, mode, 0.f, 0.f, 0.f);
-  if (s != PSDF_OK) return s;
-  if (use_zero_copy(sc, N, per_obstacle != nullptr)) {
-    for (int n = 0; n < N; ++n) {
-      value[n] = sc->h_out[4 * n];
-      if (grad) { grad[3 * n] = sc->h_out[4 * n + 1]; grad[3 * n + 1] = sc->h_out[4 * n + 2]; grad[3 * n + 2] = sc->h_out[4 * n + 3]; }
-    }
-  } else {
-    std::memcpy(value, sc->h_out, sizeof(float) * (size_t)N);
-    if (grad) std::memcpy(grad, sc->h_out + N, sizeof(float) * 3 * (size_t)N);
-  }
-  if (per_obstacle) std::memcpy(per_obstacle, sc->h_per, sizeof(float) * (size_t)N * sc->M);
-  return PSDF_OK;
+  PSDF_ENTER(sc);
+  HostCall h;
+  h.poses = poses; h.N = N; h.value = value; h.grad = grad; h.per = per_obstacle;
+  h.mode = (grad ? kGrad : 0) | (per_obstacle ? kPerObs : 0);
+  return run_host(sc, h);
 }
 
-psdf_status psdf_eval_windows(psdf_scene* sc, const float* poses, int N, const int* row_window, float* value,
+psdf_status psdf_mpc_coeffs_host(psdf_scene* sc, const float* poses, int N, float d_min, float rho_p,
+                                 float rho_theta, float* coeff) {
+  if (!sc || N < 0 || (N > 0 && (!poses || !coeff))) return PSDF_ERR_INVALID_ARG;
+  if (N > sc->max_poses) return PSDF_ERR_CAPACITY;
+  if (N == 0) return PSDF_OK;
+  PSDF_ENTER(sc);
+  HostCall h;
+  h.poses = poses; h.N = N; h.coeff = coeff; h.mode = kCoeff;
+  h.d_min = d_min; h.rho_p = rho_p; h.rho_theta = rho_theta;
+  return run_host(sc, h);
+}
+
+psdf_status psdf_eval_windows(const psdf_scene* sc, const float* poses, int N, const int* row_window, float* value,
                               float* grad, void* cuda_stream) {
   if (!sc || N < 0 || (N > 0 && (!poses || !value || !row_window))) return PSDF_ERR_INVALID_ARG;
   if (N > sc->max_poses) return PSDF_ERR_CAPACITY;
-  return enqueue_eval(sc, poses, N, value, grad, nullptr, nullptr, 0.f, 0.f, 0.f, (cudaStream_t)cuda_stream, nullptr,
-                      row_window);
+  PSDF_ENTER(sc);
+  note_eval_stream(sc, (cudaStream_t)cuda_stream);
+  EvalCall c;
+  c.poses = poses; c.N = N; c.value = value; c.grad = grad; c.window = row_window;
+  return enqueue_eval(sc, c, (cudaStream_t)cuda_stream);
 }
 
 psdf_status psdf_eval_windows_host(psdf_scene* sc, const float* poses, int N, const int* row_window, float* value,
@@ -595,19 +830,27 @@ psdf_status psdf_eval_windows_host(psdf_scene* sc, const float* poses, int N, co
   if (!sc || N < 0 || (N > 0 && (!poses || !value || !row_window))) return PSDF_ERR_INVALID_ARG;
   if (N > sc->max_poses) return PSDF_ERR_CAPACITY;
   if (N == 0) return PSDF_OK;
+  PSDF_ENTER(sc);
   psdf_status s = ensure_host_path(sc, false);
   if (s != PSDF_OK) return s;
   if (!sc->h_win) {
-    CU_TRY(cudaMallocHost(&sc->h_win, sizeof(int) * 2 * (size_t)sc->max_poses));
-    CU_TRY(cudaMalloc(&sc->d_win, sizeof(int) * 2 * (size_t)sc->max_poses));
+    int* h = nullptr;
+    int* d = nullptr;
+    CU_TRY(cudaMallocHost(&h, sizeof(int) * 2 * (size_t)sc->max_poses));
+    cudaError_t e = cudaMalloc(&d, sizeof(int) * 2 * (size_t)sc->max_poses);
+    if (e != cudaSuccess) { cudaFreeHost(h); return cuda_failed(e); }
+    sc->h_win = h;
+    sc->d_win = d;
   }
   std::memcpy(sc->h_in, poses, sizeof(float) * 3 * (size_t)N);
   std::memcpy(sc->h_win, row_window, sizeof(int) * 2 * (size_t)N);
   cudaStream_t st = sc->gstream;
   CU_TRY(cudaMemcpyAsync(sc->d_in, sc->h_in, sizeof(float) * 3 * (size_t)N, cudaMemcpyHostToDevice, st));
   CU_TRY(cudaMemcpyAsync(sc->d_win, sc->h_win, sizeof(int) * 2 * (size_t)N, cudaMemcpyHostToDevice, st));
-  s = enqueue_eval(sc, sc->d_in, N, sc->d_out, grad ? sc->d_out + N : nullptr, nullptr, nullptr, 0.f, 0.f, 0.f, st,
-                   nullptr, sc->d_win);
+  EvalCall c;
+  c.poses = sc->d_in; c.N = N; c.value = sc->d_out; c.grad = grad ? sc->d_out + N : nullptr; c.window = sc->d_win;
+  c.which_ws = 1;
+  s = enqueue_eval(sc, c, st);
   if (s != PSDF_OK) return s;
   CU_TRY(cudaMemcpyAsync(sc->h_out, sc->d_out, sizeof(float) * (grad ? 4 : 1) * (size_t)N, cudaMemcpyDeviceToHost, st));
   CU_TRY(cudaStreamSynchronize(st));
@@ -616,28 +859,16 @@ psdf_status psdf_eval_windows_host(psdf_scene* sc, const float* poses, int N, co
   return PSDF_OK;
 }
 
-psdf_status psdf_mpc_coeffs_host(psdf_scene* sc, const float* poses, int N, float d_min, float rho_p,
-                                 float rho_theta, float* coeff) {
-  if (!sc || N < 0 || (N > 0 && (!poses || !coeff))) return PSDF_ERR_INVALID_ARG;
-  if (N > sc->max_poses) return PSDF_ERR_CAPACITY;
-  if (N == 0) return PSDF_OK;
-  psdf_status s = ensure_host_path(sc, false);
-  if (s != PSDF_OK) return s;
-  stage_poses(sc, poses, N, false);
-  s = run_graph(sc, N, kCoeff, d_min, rho_p, rho_theta);
-  if (s != PSDF_OK) return s;
-  std::memcpy(coeff, sc->h_out, sizeof(float) * 4 * (size_t)N);
-  return PSDF_OK;
-}
-
 psdf_status psdf_set_culling(psdf_scene* sc, int enable) {
   if (!sc) return PSDF_ERR_INVALID_ARG;
+  PSDF_ENTER(sc);
   if (sc->gstream) CU_TRY(cudaStreamSynchronize(sc->gstream));
-  sc->culling = enable ? 1 : 0;
-  for (auto& g : sc->graphs) {           // launch plans are baked into the captured graphs
-    if (g.exec) cudaGraphExecDestroy(g.exec);
-    g = GraphEntry();
+  if (enable && !sc->pk[sc->cur].grid_ok) {      // built here, then kept current by every update
+    CU_TRY(launch_grid(sc, sc->cur, nullptr, sc->Mv, (cudaStream_t)0));
+    CU_TRY(cudaStreamSynchronize((cudaStream_t)0));
   }
+  sc->culling = enable ? 1 : 0;
+  drop_graphs(sc);
   return PSDF_OK;
 }
 
@@ -667,10 +898,19 @@ psdf_status psdf_trajectory_reduce(const float* value, int T, int H, float d_saf
 
 psdf_status psdf_cull_stats(psdf_scene* sc, void* cuda_stream, unsigned long long* out2) {
   if (!sc || !out2) return PSDF_ERR_INVALID_ARG;
+  PSDF_ENTER(sc);
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  CU_TRY(cudaMemcpyAsync(out2, sc->d_stats, sizeof(unsigned long long) * 2, cudaMemcpyDeviceToHost, st));
-  CU_TRY(cudaMemsetAsync(sc->d_stats, 0, sizeof(unsigned long long) * 2, st));
-  CU_TRY(cudaStreamSynchronize(st));
+  if (sc->gstream) CU_TRY(cudaStreamSynchronize(sc->gstream));
+  out2[0] = out2[1] = 0ull;
+  for (const Workspace& w : sc->ws) {            // caller-stream and host-path evaluations
+    if (!w.stats) continue;
+    unsigned long long v[2] = {0ull, 0ull};
+    CU_TRY(cudaMemcpyAsync(v, w.stats, sizeof(v), cudaMemcpyDeviceToHost, st));
+    CU_TRY(cudaMemsetAsync(w.stats, 0, sizeof(v), st));
+    CU_TRY(cudaStreamSynchronize(st));
+    out2[0] += v[0];
+    out2[1] += v[1];
+  }
   return PSDF_OK;
 }
 
@@ -678,7 +918,7 @@ int psdf_scene_num_obstacles(const psdf_scene* sc) { return sc ? sc->Mv : 0; }
 int psdf_scene_num_edges(const psdf_scene* sc) { return sc ? sc->n_edges : 0; }
 int psdf_last_cuda_error(void) { return g_last_cuda_error.load(); }
 long long psdf_kernel_launches(void) { return g_launches.load(); }
-const char* psdf_version(void) { return "psdf-b200 0.1 (sm_100a)"; }
+const char* psdf_version(void) { return "psdf-b200 0.2 (sm_100a)"; }
 
 const char* psdf_status_string(psdf_status s) {
   switch (s) {
@@ -688,8 +928,24 @@ const char* psdf_status_string(psdf_status s) {
     case PSDF_ERR_CAPACITY: return "N exceeds max_poses";
     case PSDF_ERR_CUDA: return "CUDA error";
     case PSDF_ERR_ALLOC: return "allocation failed";
+    case PSDF_ERR_BUSY: return "scene in use by another host thread";
   }
   return "unknown status";
+}
+
+psdf_status psdf_bench_host_latency(psdf_scene* sc, const float* poses, int N, float* value, float* grad,
+                                    float* per_obstacle, float* coeff, float d_min, float rho_p, float rho_theta,
+                                    int reps, double* out_us) {
+  if (!sc || !out_us || reps < 1) return PSDF_ERR_INVALID_ARG;
+  for (int r = 0; r < reps; ++r) {
+    const auto t0 = std::chrono::steady_clock::now();
+    const psdf_status s = coeff ? psdf_mpc_coeffs_host(sc, poses, N, d_min, rho_p, rho_theta, coeff)
+                                : psdf_eval_host(sc, poses, N, value, grad, per_obstacle);
+    const auto t1 = std::chrono::steady_clock::now();
+    if (s != PSDF_OK) return s;
+    out_us[r] = std::chrono::duration<double, std::micro>(t1 - t0).count();
+  }
+  return PSDF_OK;
 }
 
 psdf_status psdf_measure_fp32_peak(int iters, void* cuda_stream, double* tflops_out) {

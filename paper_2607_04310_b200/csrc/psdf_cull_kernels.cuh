@@ -18,7 +18,7 @@ __device__ __forceinline__ float warp_max_f(float v) { return fkey_inv(__reduce_
 // ------------------------------------------------------------------------------------------
 // Obstacle grid: the bounds re-ordered by cell of a G x G grid over the obstacle centres
 // (row-major: a rectangle of cells is one contiguous range of `gbounds` per grid row), built on
-// the device after every pack (host or device packer) by one CTA.
+// the device by one CTA when culling is switched on and after every pack while it is on.
 struct GridHdr {
   float x0, y0, sx, sy;    // cell(x) = clamp((int)((x - x0) * sx), 0, G-1)
   float rmax;              // largest bounding-circle radius
@@ -35,7 +35,7 @@ __device__ __forceinline__ int grid_coord(float v, float v0, float s, int G) {
 __global__ void __launch_bounds__(1024) obstacle_grid_kernel(const float4* __restrict__ bounds, int Mv_host,
                                                              const int* __restrict__ totals2,
                                                              float4* __restrict__ gbounds, int* __restrict__ gcell,
-                                                             int* __restrict__ gidx, GridHdr* __restrict__ hdr) {
+                                                             GridHdr* __restrict__ hdr) {
   __shared__ int cnt[kObsGridMax * kObsGridMax + 1];
   __shared__ float red[5][32];
   __shared__ int wsum[32];
@@ -90,24 +90,15 @@ __global__ void __launch_bounds__(1024) obstacle_grid_kernel(const float4* __res
     if (tid == 0) gcell[cells] = Mv;
   }
   __syncthreads();
-  for (int i = tid; i < Mv; i += 1024) {                   // scatter of the indices (cnt = cursors), any order
+  // scatter of the bounds themselves (cnt = cursors).  The order inside a cell is whatever the
+  // atomics give: the culled kernel's results do not depend on it (its reductions are arg-min /
+  // arg-max keys with the packed slot as tie-break), and a rank pass to make it deterministic would
+  // be quadratic in the cell size (every obstacle in one cell: Mv^2 / 1024 steps per thread).
+  for (int i = tid; i < Mv; i += 1024) {
     const float4 b = bounds[2 * i];
-    gidx[atomicAdd(&cnt[grid_coord(b.y, y0, sy, G) * G + grid_coord(b.x, x0, sx, G)], 1)] = i;
-  }
-  __syncthreads();
-  // deterministic order inside a cell (packed order): entry i goes to its rank among the cell's
-  // indices.  After the scatter cnt[c] is the END of cell c, its begin is the end of cell c-1.
-  // (Work is sum over cells of size^2, spread over the threads: a scene with every obstacle in one
-  // cell still takes Mv^2 / 1024 steps per thread.)
-  for (int q = tid; q < Mv; q += 1024) {
-    const int i = gidx[q];
-    const float4 b = bounds[2 * i];
-    const int c = grid_coord(b.y, y0, sy, G) * G + grid_coord(b.x, x0, sx, G);
-    const int b0 = c ? cnt[c - 1] : 0, b1 = cnt[c];
-    int rank = 0;
-    for (int r = b0; r < b1; ++r) rank += gidx[r] < i;
-    gbounds[b0 + rank] = b;
-    gbounds[Mv + b0 + rank] = bounds[2 * i + 1];
+    const int at = atomicAdd(&cnt[grid_coord(b.y, y0, sy, G) * G + grid_coord(b.x, x0, sx, G)], 1);
+    gbounds[at] = b;
+    gbounds[Mv + at] = bounds[2 * i + 1];
   }
   if (tid == 0) {
     GridHdr h;

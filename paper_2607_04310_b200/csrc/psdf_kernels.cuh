@@ -63,7 +63,7 @@ __device__ __forceinline__ void finalize_pose(const Footprint& fp, const EvalPar
   }
   if (p.packed) {                                   // zero-copy staging: one 16-byte store per pose
     if (!(MODE & kCoeff)) reinterpret_cast<float4*>(p.packed)[n] = make_float4(value, g[0], g[1], g[2]);
-  } else {
+  } else if (!(MODE & kCoeff)) {
     p.value[n] = value;
   }
   if ((MODE & kGrad) && !p.packed) {
@@ -72,9 +72,11 @@ __device__ __forceinline__ void finalize_pose(const Footprint& fp, const EvalPar
     p.grad[3 * n + 2] = g[2];
   }
   if (MODE & kCoeff) {
-    // [h_s - gamma_s ; J_g,s], eqs.(26)-(28) PAPER.md:247-268; J_g = -grad phi.
+    // [h_s - gamma_s ; J_g,s], eqs.(26)-(28) PAPER.md:247-268; J_g = -grad phi.  A stage that sees no
+    // obstacle (phi = +inf; eq.(27) would read inf - inf) is an inactive row (+inf, 0, 0, 0): reading G17.
     const float gamma = 0.5f * (fp.rmax + value) * p.rho_theta * p.rho_theta + p.rho_p * p.rho_theta;
-    reinterpret_cast<float4*>(p.coeff)[n] = make_float4(value - p.d_min - gamma, -g[0], -g[1], -g[2]);
+    const float c0 = (finite && slot < 0) ? kInf : value - p.d_min - gamma;
+    reinterpret_cast<float4*>(p.coeff)[n] = make_float4(c0, -g[0], -g[1], -g[2]);
   }
 }
 

@@ -20,13 +20,17 @@ PSDF_ERR_DEGENERATE = -2
 PSDF_ERR_CAPACITY = -3
 PSDF_ERR_CUDA = -4
 PSDF_ERR_ALLOC = -5
+PSDF_ERR_BUSY = -6
 PSDF_MEM_HOST = 0
 PSDF_MEM_DEVICE = 1
 
+# include/psdf.h: the product ABI
 EXPORTS = ["psdf_create_scene", "psdf_update_scene", "psdf_eval", "psdf_eval_host",
-           "psdf_eval_windows", "psdf_eval_windows_host", "psdf_mpc_coeffs_host", "psdf_component_min", "psdf_trajectory_reduce", "psdf_set_culling", "psdf_cull_stats", "psdf_destroy_scene", "psdf_scene_num_obstacles",
-           "psdf_scene_num_edges", "psdf_last_cuda_error", "psdf_kernel_launches",
-           "psdf_status_string", "psdf_version", "psdf_measure_fp32_peak"]
+           "psdf_eval_windows", "psdf_eval_windows_host", "psdf_mpc_coeffs_host", "psdf_component_min",
+           "psdf_trajectory_reduce", "psdf_set_culling", "psdf_destroy_scene", "psdf_scene_num_obstacles",
+           "psdf_scene_num_edges", "psdf_last_cuda_error", "psdf_status_string", "psdf_version"]
+# include/psdf_bench.h: measurement instrumentation (bench.py, tests)
+BENCH_EXPORTS = ["psdf_kernel_launches", "psdf_cull_stats", "psdf_measure_fp32_peak", "psdf_bench_host_latency"]
 
 _lib = None
 
@@ -83,6 +87,9 @@ def lib():
     L.psdf_status_string.restype = ctypes.c_char_p
     L.psdf_status_string.argtypes = [i]
     L.psdf_version.restype = ctypes.c_char_p
+    L.psdf_bench_host_latency.restype = i
+    L.psdf_bench_host_latency.argtypes = [vp, fp_, i, fp_, fp_, fp_, fp_, ctypes.c_float, ctypes.c_float, ctypes.c_float,
+                                          i, ctypes.POINTER(ctypes.c_double)]
     L.psdf_measure_fp32_peak.restype = i
     L.psdf_measure_fp32_peak.argtypes = [i, vp, ctypes.POINTER(ctypes.c_double)]
     _lib = L
@@ -311,6 +318,23 @@ class Scene:
             if status != PSDF_OK:
                 raise PsdfError(status, "psdf_mpc_coeffs_host")
         return call
+
+    def bench_host_latency(self, poses, reps, grad=True, per_obstacle=False, coeffs=None):
+        """psdf_bench_host_latency (include/psdf_bench.h): per-call microseconds of psdf_eval_host, or of
+        psdf_mpc_coeffs_host when coeffs = (d_min, rho_p, rho_theta), timed inside the library."""
+        poses, pp = _host(poses, np.float32)
+        N = int(poses.shape[0])
+        value = np.empty(N, np.float32)
+        g = np.empty((N, 3), np.float32) if grad else None
+        po = np.empty((N, self.M), np.float32) if per_obstacle else None
+        c = np.empty((N, 4), np.float32) if coeffs else None
+        d_min, rho_p, rho_theta = coeffs if coeffs else (0.0, 0.0, 0.0)
+        out = (ctypes.c_double * int(reps))()
+        _check(lib().psdf_bench_host_latency(self._h, pp, N, value.ctypes.data, g.ctypes.data if g is not None else None,
+                                             po.ctypes.data if po is not None else None,
+                                             c.ctypes.data if c is not None else None, float(d_min), float(rho_p),
+                                             float(rho_theta), int(reps), out), "psdf_bench_host_latency")
+        return np.frombuffer(out, dtype=np.float64).copy()
 
     def mpc_coeffs_host(self, poses, d_min, rho_p, rho_theta):
         poses, pp = _host(poses, np.float32)

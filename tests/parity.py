@@ -1,41 +1,77 @@
 """Shared GPU-vs-oracle comparison (the bar of BASELINE.json.north_star):
-|d value| <= 1e-5 m everywhere; gradient relative error <= 1e-3 where the oracle's
-arg-min margin exceeds 1e-4 m and |phi| > 1e-3 m (reading G9)."""
+|d value| <= 1e-5 m everywhere; gradient relative error <= 1e-3 where the oracle's arg-min
+margin exceeds 1e-4 m (reading G9).  On the SEPARATED branch only, poses with
+phi <= 1e-3 m are also left out of the gradient comparison: there n = (w - Q)/d is the
+normalisation of a vector of length d and fp32's ~3e-7 m absolute error in it is a relative
+1e-3 at d = 3e-4 m (SURVEY.md H-d, G9); the penetrating branch takes a face normal and is
+compared right up to contact.  `stats` only measures (bench.py prints it as its `parity`
+object), `compare` asserts the bar on top."""
 import numpy as np
 
 VALUE_TOL = 1e-5
 GRAD_REL_TOL = 1e-3
 MARGIN_MIN = 1e-4
-PHI_MIN = 1e-3
+PHI_MIN = 1e-3          # separated branch only
 
 
-def compare(ref, value, grad=None, per_obstacle=None, what=""):
+def grad_mask(ref):
+    """Poses whose gradient is compared (reading G9)."""
+    fin = np.isfinite(ref.value)
+    near_contact_separated = (ref.value > 0.0) & (ref.value <= PHI_MIN)
+    return fin & (ref.margin > MARGIN_MIN) & ~near_contact_separated
+
+
+def stats(ref, value, grad=None, per_obstacle=None):
+    """Error figures of one comparison; nothing is asserted."""
     value = np.asarray(value, np.float64)
     fin = np.isfinite(ref.value)
-    assert np.array_equal(np.isinf(value), ~fin), what
     dv = np.abs(value[fin] - ref.value[fin])
-    stats = {"max_dvalue": float(dv.max()) if dv.size else 0.0}
-    assert stats["max_dvalue"] <= VALUE_TOL, (what, stats, int(np.argmax(dv)))
+    out = {"n": int(ref.value.size), "inf_pattern_equal": bool(np.array_equal(np.isposinf(value), ~fin)),
+           "max_dvalue": float(dv.max()) if dv.size else 0.0,
+           "penetrating_frac": float((ref.value[fin] < 0).mean()) if fin.any() else 0.0}
+    if dv.size:
+        out["argmax_dvalue"] = int(np.nonzero(fin)[0][int(np.argmax(dv))])
     if grad is not None:
         grad = np.asarray(grad, np.float64)
-        ok = fin & (ref.margin > MARGIN_MIN) & (np.abs(ref.value) > PHI_MIN)
+        ok = grad_mask(ref)
         den = np.linalg.norm(ref.grad[ok], axis=1)
         rel = np.linalg.norm(grad[ok] - ref.grad[ok], axis=1) / den
-        stats["grad_compared"] = float(ok.mean()) if ok.size else 0.0
-        stats["max_grad_rel"] = float(rel.max()) if rel.size else 0.0
+        pen = fin & (ref.value < 0)
+        out["grad_compared"] = float(ok.mean()) if ok.size else 0.0
+        out["grad_compared_penetrating"] = float(ok[pen].mean()) if pen.any() else None
+        out["grad_excluded_by_margin"] = int((fin & ~(ref.margin > MARGIN_MIN)).sum())
+        out["grad_excluded_near_contact_separated"] = int((fin & (ref.margin > MARGIN_MIN) & ~ok).sum())
+        out["max_grad_rel"] = float(rel.max()) if rel.size else 0.0
+        out["grad_finite"] = bool(np.isfinite(grad[fin]).all())
         if rel.size:
-            k = int(np.argmax(rel))
-            assert stats["max_grad_rel"] <= GRAD_REL_TOL, (what, stats, np.nonzero(ok)[0][k],
-                                                          grad[ok][k], ref.grad[ok][k])
-        assert np.isfinite(grad[fin]).all()
+            out["argmax_grad_rel"] = int(np.nonzero(ok)[0][int(np.argmax(rel))])
     if per_obstacle is not None:
         po = np.asarray(per_obstacle, np.float64)
         pf = np.isfinite(ref.per_obstacle)
-        assert np.array_equal(np.isposinf(po), ~pf), what
         dpo = np.abs(po[pf] - ref.per_obstacle[pf])
-        stats["max_dper_obstacle"] = float(dpo.max()) if dpo.size else 0.0
-        # far obstacles: fp32 cannot hold 1e-5 m at tens of metres (ulp(32 m) = 3.8e-6), so the
-        # per-obstacle bar is 1e-5 m + 4 ulp_fp32(|sd|); phi itself stays at 1e-5.
+        out["per_obstacle_inf_pattern_equal"] = bool(np.array_equal(np.isposinf(po), ~pf))
+        out["max_dper_obstacle"] = float(dpo.max()) if dpo.size else 0.0
+        # far obstacles: fp32 cannot hold 1e-5 m at tens of metres (ulp(32 m) = 3.8e-6), so the general
+        # per-obstacle bar is 1e-5 m + 4 ulp_fp32(|sd|) (reading G16); phi itself stays at 1e-5
         tol = VALUE_TOL + 4.0 * np.abs(ref.per_obstacle[pf]) * 2.0 ** -23
-        assert (dpo <= tol).all(), (what, stats)
-    return stats
+        out["per_obstacle_within_ulp_bar"] = bool((dpo <= tol).all())
+    return out
+
+
+def compare(ref, value, grad=None, per_obstacle=None, what="", per_obstacle_plain_tol=False):
+    """Asserts the bar.  per_obstacle_plain_tol: the per-obstacle values must hold the plain
+    1e-5 m as well (BASELINE config 2, the config that asks for them)."""
+    st = stats(ref, value, grad, per_obstacle)
+    assert st["inf_pattern_equal"], what
+    assert st["max_dvalue"] <= VALUE_TOL, (what, st)
+    if grad is not None:
+        if "argmax_grad_rel" in st:
+            k = st["argmax_grad_rel"]
+            assert st["max_grad_rel"] <= GRAD_REL_TOL, (what, st, np.asarray(grad)[k], ref.grad[k])
+        assert st["grad_finite"], what
+    if per_obstacle is not None:
+        assert st["per_obstacle_inf_pattern_equal"], what
+        assert st["per_obstacle_within_ulp_bar"], (what, st)
+        if per_obstacle_plain_tol:
+            assert st["max_dper_obstacle"] <= VALUE_TOL, (what, st)
+    return st

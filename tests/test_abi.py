@@ -17,16 +17,42 @@ def psdf():
     return m
 
 
-def test_exports_match_header(psdf):
-    hdr = open(os.path.join(ROOT, "include", "psdf.h")).read()
+def _declared(header):
+    hdr = open(os.path.join(ROOT, "include", header)).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(psdf_[a-z0-9_]+)\s*\(", hdr))
+    return set(re.findall(r"\b(psdf_[a-z0-9_]+)\s*\(", hdr))
+
+
+def test_exports_match_header(psdf):
+    """Every symbol include/psdf.h (product ABI) and include/psdf_bench.h (instrumentation) declare
+    is exported, and the binding's lists are exactly the headers'."""
+    declared = _declared("psdf.h")
     assert declared == set(psdf.EXPORTS), declared ^ set(psdf.EXPORTS)
+    bench = _declared("psdf_bench.h")
+    assert bench == set(psdf.BENCH_EXPORTS), bench ^ set(psdf.BENCH_EXPORTS)
+    assert not (declared & bench)
     L = psdf.lib()
-    for name in declared:
+    for name in declared | bench:
         assert getattr(L, name) is not None
     assert "sm_100a" in psdf.psdf_version()
     assert psdf.lib().psdf_status_string(-2).decode().startswith("degenerate")
+    assert psdf.lib().psdf_status_string(psdf.PSDF_ERR_ALLOC).decode() == "allocation failed"
+    assert "another host thread" in psdf.lib().psdf_status_string(psdf.PSDF_ERR_BUSY).decode()
+    # the status codes of the header and of the binding agree
+    hdr = open(os.path.join(ROOT, "include", "psdf.h")).read()
+    for name, val in re.findall(r"(PSDF_(?:OK|ERR_[A-Z_]+))\s*=\s*(-?\d+)", hdr):
+        assert getattr(psdf, name) == int(val), name
+
+
+def test_product_build_has_no_tuning_knobs(psdf):
+    """The sweep knobs (PSDF_BD, PSDF_CHUNKS, PSDF_BRANCHES, PSDF_NO_ZERO_COPY) exist only in
+    -DPSDF_TUNING measurement builds: the product library holds neither their names nor a getenv."""
+    blob = open(psdf.LIB_PATH, "rb").read()
+    for knob in (b"PSDF_BD", b"PSDF_CHUNKS", b"PSDF_BRANCHES", b"PSDF_NO_ZERO_COPY"):
+        assert knob not in blob, knob
+    src = open(os.path.join(ROOT, "paper_2607_04310_b200", "csrc", "psdf_api.cu")).read()
+    outside = re.sub(r"#ifdef PSDF_TUNING.*?#endif", "", src, flags=re.S)
+    assert "getenv" not in outside
 
 
 def test_host_validation_without_gpu(psdf):

@@ -38,7 +38,7 @@ def test_small_configs_device_and_host_paths(env, workloads_cache, cfg):
     w = workloads_cache(cfg)
     ref = _oracle(O, w, per_obstacle=True)
     scene, (v, g, po) = _gpu_eval(torch, psdf, w, grad=True, per_obstacle=True)
-    st = compare(ref, v, g, po, what=w.name)
+    st = compare(ref, v, g, po, what=w.name, per_obstacle_plain_tol=True)     # plain 1e-5 m per obstacle
     print(w.name, st)
     assert st["grad_compared"] > 0.5
     # host (CUDA graph) path, twice (capture, then replay), all output combinations

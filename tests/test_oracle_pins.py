@@ -23,9 +23,9 @@ def _num(tok):
 def _poly(spec):
     t = spec.split()
     if t[0] == "box":
-        x0, x1, y0, y1 = map(float, t[1:])
+        x0, x1, y0, y1 = map(_num, t[1:])
         return np.array([[x0, y0], [x1, y0], [x1, y1], [x0, y1]])
-    v = np.array(list(map(float, t[1:]))).reshape(-1, 2)
+    v = np.array(list(map(_num, t[1:]))).reshape(-1, 2)
     return v
 
 
@@ -41,9 +41,9 @@ def _scene(polys, E=None, M_extra=0):
     return A, B, S
 
 
-def _cases():
+def _cases(path=GOLD):
     out = []
-    for line in open(GOLD):
+    for line in open(path):
         if line.startswith("#") or not line.strip():
             continue
         f = [x.strip() for x in line.split("|")]
@@ -69,6 +69,51 @@ def test_closed_forms(case):
         for k, tok in enumerate(per.split(None, 1)):
             if tok.strip() != "-":
                 assert abs(r.per_obstacle[0, k] - _num(tok)) < 1e-12
+    # the winner row and its branch (eq.(23): separated <=> value > 0; contact counts as not separated)
+    assert r.branch[0] == (1 if _num(val) > 0 else 0), cid
+    assert r.winner[0] == int(np.argmin(r.per_obstacle[0])), cid
+    if cid == "P8":
+        assert r.winner[0] == 1
+
+
+MARGINS = os.path.join(os.path.dirname(__file__), "golden", "margins.txt")
+_K = 0.3 * math.cos(0.3) + 0.2 * math.sin(0.3)
+_YW = 0.2 * math.cos(0.3) - 0.3 * math.sin(0.3)
+
+
+@pytest.mark.parametrize("case", _cases(MARGINS), ids=lambda c: c[0])
+def test_margin_rule_exact(case):
+    """Rule O7 / reading G9 pinned to hand-worked values: the gap of a loser with a different
+    gradient, a same-gradient loser passing its own margin on (shifted by the gap), structural
+    ties that share a witness, and a competitor inside one obstacle.  Replacing `gap + c[k].m`
+    in the oracle's reduce() by INF fails M2, by `gap` fails M2, M3, M4 (and P2)."""
+    cid, fpn, pose, obst, winner, margin, _ = case
+    ENV.update(k=_K, yw=_YW)
+    pose = [_num(t) for t in pose.split()]
+    A, B, S = _scene([_poly(s) for s in obst.split(";")])
+    for window in (-1.0, 0.2):                              # all duals, and the windowed mode bench/tests use
+        r = O.evaluate(FP[fpn], A, B, S, [pose], per_obstacle=True, window=window)
+        assert abs(r.margin[0] - _num(margin)) < 1e-12, (cid, window, r.margin[0], _num(margin))
+        assert r.winner[0] == int(winner) and r.branch[0] == 1
+
+
+def test_mpc_coeffs_hand_worked():
+    """eqs.(26)-(28), on P8 (phi = 0.9-k = 0.554295012, grad (1, 0, -yw) with
+    yw = 0.10241124): r_max = sqrt(0.3^2+0.2^2) = sqrt(0.13) = 0.360555128, rho_p = rho_theta = 0.1:
+    gamma = 0.5*(0.360555128+0.554295012)*0.01 + 0.01 = 0.014574251,
+    h - gamma = 0.554295012 - 0.01 - 0.014574251 = 0.529720761,  J_g = (-1, 0, +0.10241124)."""
+    A, B, S = _scene([_poly("box 1 2 1 2"), _poly("box -2 -0.9 -0.3 0.4")])
+    r = O.evaluate(FP["rect"], A, B, S, [(0.0, 0.0, 0.3)], window=-1.0)
+    c = O.mpc_coeffs(r.value, r.grad, FP["rect"], 0.01, 0.1, 0.1)
+    assert c.shape == (1, 4)
+    assert np.abs(c[0] - np.array([0.529720761, -1.0, 0.0, 0.10241124])).max() < 5e-9
+    # independent numbers: gamma of a literal phi, two stages, different radii
+    c2 = O.mpc_coeffs([1.0, 2.0], [[0.6, 0.8, 0.1], [0.0, -1.0, -0.2]], [[3, 4], [-3, 4], [-3, -4], [3, -4]], 0.25, 0.2, 0.5)
+    # r_max = 5: gamma = 0.5*(5+1)*0.25 + 0.1 = 0.85 ; 0.5*(5+2)*0.25 + 0.1 = 0.975
+    assert np.allclose(c2, [[1.0 - 0.25 - 0.85, -0.6, -0.8, -0.1], [2.0 - 0.25 - 0.975, 0.0, 1.0, 0.2]], rtol=0, atol=1e-15)
+    # no obstacle in view (reading G17): inactive constraint row
+    c3 = O.mpc_coeffs([np.inf], [[0.0, 0.0, 0.0]], FP["rect"], 0.01, 0.1, 0.1)
+    assert np.isposinf(c3[0, 0]) and (c3[0, 1:] == 0).all()
 
 
 def test_axis_aligned_box_box_formula():
