@@ -183,7 +183,7 @@ cudaError_t launch_cull_v(const psdf_scene* sc, const EvalParams& p, int mode, c
     case 8: return launch_cull_mode<8, NP>(sc, p, mode, st);
     case 10: return launch_cull_mode<10, NP>(sc, p, mode, st);
     case 12: return launch_cull_mode<12, NP>(sc, p, mode, st);
-    case 16: return launch_cull_mode<16, NP>(sc, p, mode, st);
+    case 16: return launch_cull_mode<16, (NP > 64 ? 64 : NP)>(sc, p, mode, st);   // (shared-memory budget)
     default: return cudaErrorInvalidValue;
   }
 }

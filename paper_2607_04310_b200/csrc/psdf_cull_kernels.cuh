@@ -111,36 +111,69 @@ __global__ void __launch_bounds__(1024) obstacle_grid_kernel(const float4* __res
 
 
 // ------------------------------------------------------------------------------------------
-// Culled evaluation over the obstacle grid, pair-queue formulation.  CTA = NP poses, one per
-// thread.  Every thread walks the grid cells around ITS pose and pushes the
-// obstacles that pass the bounding-circle test as (pose, obstacle) pairs into a shared-memory
-// queue; the CTA then evaluates the queued pairs one per lane, whatever pose they belong to
-// (the posed footprints sit in shared memory), with the dense kernel's arithmetic (edge_step2),
-// and folds each result into its pose's 64-bit arg-max / arg-min keys with shared-memory
-// atomics (same keys as the dense kernel: lowest slot on ties).  Two rounds: a seed round (one
-// near obstacle per pose) gives every pose a finite upper bound, the main round queues whatever
-// that bound cannot exclude.  The last step is the dense kernel's tail (finalize_pose).
+// Culled evaluation over the obstacle grid.  CTA = NP poses.  The work of a pose is irregular (its
+// upper bound decides how many grid cells it has to look at, its neighbourhood how many obstacles
+// survive), so every stage hands its output to the WHOLE CTA through shared memory and the next
+// stage runs one item per lane, whatever pose it belongs to:
+//   seed     thread per pose: the nearest bounding circle in a small rectangle of cells -> pair queue
+//   drain    lane per queued (pose, obstacle) pair: the dense kernel's arithmetic (edge_step2), result
+//            folded into the pose's 64-bit arg-max / arg-min keys with shared-memory atomics (the
+//            dense kernel's keys: lowest slot on ties); every pose now has a finite upper bound ub
+//   rows     thread per pose: the grid rows within ub + R_max + r_R of the pose go into a segment
+//            list, one (pose, row) per entry: a row of the cell rectangle is one contiguous range of
+//            the grid-ordered bounds
+//   circles  lane per segment: bounding-circle test of its entries against the segment's pose ->
+//            queue 1 of (pose, entry)
+//   boxes    lane per queue-1 item: oriented-box separating-axis bound -> pair queue
+//   drain    as above
+//   tail     value; separated poses take their witness gradient in place, the few penetrating ones are
+//            compacted into the first lanes (their branch would otherwise run in every warp for two or
+//            three lanes); stores as in the dense kernel (finalize_store).
+// Queues and the segment list have fixed sizes: a stage that finds its output full stops, the
+// stages behind it run, and it resumes where it stopped.
 template <int V>
 struct __align__(16) PosedSlot {      // one posed footprint in shared memory
   float2 rx[V / 2], ry[V / 2], Tx[V / 2], Ty[V / 2];
-  float px, py, ub, pad;
+  float px, py, pad0, pad1;
 };
 
-// NP = poses (= threads) per CTA; NP = 32 makes every warp an independent unit (no block barriers)
+struct __align__(16) WalkPose {       // what the shared stages need to know about a pose
+  float bx, by, cs, sn;               // posed bounding-box centre, rotation
+  float ub, ub_pad, rpad;             // upper bound of phi, padded copies for the two tests
+  int seed_rec;                       // the seed obstacle (already evaluated)
+  int cx0, cx1, pad0, pad1;           // columns of the cell rectangle
+};
+
+template <int V, int NP>
+struct CullShape {
+  // queue entries: as many as fit next to the posed footprints in 48 KB of static shared memory
+  static constexpr int kFixed = NP * ((int)sizeof(PosedSlot<V>) + (int)sizeof(WalkPose) + 16 + 12 + 2) + NP * 8 * 2 + 64;
+  static constexpr int kQueue = (kFixed + NP * 8 * 16 <= 48 * 1024 - 256) ? NP * 8 : NP * 4;
+  static constexpr int kSeg = NP * 8;
+  static_assert(kFixed + kQueue * 16 <= 48 * 1024 - 256, "culled kernel: static shared memory budget");
+};
+
+// NP = poses (= threads) per CTA; NP = 32 makes every warp an independent unit
 template <int V, int MODE, int NP>
 __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ Footprint fp,
                                                         const __grid_constant__ EvalParams p) {
-  constexpr int kCullQueue = (NP * 16 * (int)sizeof(int2) + NP * (int)sizeof(PosedSlot<V>) > 44 * 1024) ? NP * 8 : NP * 16;
+  constexpr int kQueue = CullShape<V, NP>::kQueue, kSeg = CullShape<V, NP>::kSeg;
   __shared__ PosedSlot<V> s_pose[NP];
+  __shared__ WalkPose s_walk[NP];
   __shared__ unsigned long long s_kd[NP], s_k2[NP];
-  __shared__ int2 s_queue[kCullQueue];
-  __shared__ int s_count;
+  __shared__ int2 s_q1[kQueue];          // circle survivors: (pose, grid entry)
+  __shared__ int2 s_q2[kQueue];          // pairs to evaluate: (pose, first pair record)
+  __shared__ unsigned short s_seg[kSeg]; // (pose << 6) | grid row
+  __shared__ float s_g[NP][3];           // gradients of the compacted penetrating poses
+  __shared__ unsigned short s_pen[NP];
+  __shared__ int s_n1, s_n2, s_nseg, s_npen;
   __shared__ unsigned int s_stat[2];
   const int tid = threadIdx.x;
   const int k = blockIdx.x * NP + tid;
   const int n = min(k, p.N - 1);                           // tail threads recompute the last pose
   const float x = __ldg(p.poses + 3 * n), y = __ldg(p.poses + 3 * n + 1), th = __ldg(p.poses + 3 * n + 2);
-  const bool active = k < p.N && isfinite(x) && isfinite(y) && isfinite(th);
+  const bool finite = isfinite(x) && isfinite(y) && isfinite(th);
+  const bool active = k < p.N && finite;
   float sn, cs;
   sincosf(th, &sn, &cs);
   {
@@ -153,7 +186,7 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
   }
   s_kd[tid] = 0ull;
   s_k2[tid] = ~0ull;
-  if (tid == 0) { s_count = 0; s_stat[0] = 0u; s_stat[1] = 0u; }
+  if (tid == 0) { s_n1 = 0; s_n2 = 0; s_nseg = 0; s_npen = 0; s_stat[0] = 0u; s_stat[1] = 0u; }
   __syncthreads();
   // broad-phase proxies of the posed footprint: its bounding box (centre bx,by; axes (cs,sn),
   // (-sn,cs); half extents fp.bhx, fp.bhy) and the circle of radius fp.rbox around the box centre
@@ -173,7 +206,7 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
   // evaluates the first nq queued pairs, one per lane
   auto drain = [&](int nq) {
     for (int j = tid; j < nq; j += NP) {
-      const int2 pr = s_queue[j];
+      const int2 pr = s_q2[j];
       const PosedSlot<V>& sp = s_pose[pr.x];
       Posed2<V> P;
 #pragma unroll
@@ -205,15 +238,8 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
       atomicMin(&s_k2[pr.x], ((unsigned long long)__float_as_uint(minD2) << 32) | (unsigned)slot);
     }
   };
-  // this pose's upper bound of phi from its keys
-  auto bound_now = [&]() {
-    const unsigned long long kd = s_kd[tid], k2 = s_k2[tid];
-    const float depth = kd ? fkey_inv((uint32_t)(kd >> 32)) : -kInf;
-    const float d2 = (k2 != ~0ull) ? __uint_as_float((uint32_t)(k2 >> 32)) : kInf;
-    return depth >= 0.f ? -depth : sqrtf(d2);
-  };
 
-  // ---- seed round: the entry with the smallest (d^2 - R^2) in a growing rectangle of cells
+  // ---- seed: the entry with the smallest (d^2 - R^2) in a growing rectangle of cells
   int seed_rec = -1;
   if (active) {
     float ext = rpad + 0.5f * gh.cell;
@@ -249,64 +275,123 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
       ext *= 2.f;
     }
   }
-  if (seed_rec >= 0) s_queue[atomicAdd(&s_count, 1)] = make_int2(tid, seed_rec);
+  if (seed_rec >= 0) s_q2[atomicAdd(&s_n2, 1)] = make_int2(tid, seed_rec);
   __syncthreads();
-  drain(s_count);
-  __syncthreads();
-  if (tid == 0) s_count = 0;
+  drain(s_n2);
   __syncthreads();
 
-  // ---- main round: everything the seed bound cannot exclude, resumable when the queue fills
-  const float ub = active ? bound_now() : -kInf;
-  const float need = (ub + gh.rmax) * 1.0001f + rpad;
-  const float ub_pad = fmaf(fabsf(ub), 1e-4f, ub) + 2e-4f + cpad;
-  bool done = !active || !(need >= 0.f);
-  int cx0 = 0, cx1 = 0, cy1 = -1, row = 0, i = 0, e = 0;
-  if (!done) {
-    cx0 = grid_coord(bx - need, gh.x0, gh.sx, G); cx1 = grid_coord(bx + need, gh.x0, gh.sx, G);
-    row = grid_coord(by - need, gh.y0, gh.sy, G) - 1; cy1 = grid_coord(by + need, gh.y0, gh.sy, G);
+  // ---- rows: the cell rectangle the seed bound cannot exclude
+  int row_next = 0, n_rows = 0;
+  {
+    float ub = -kInf;
+    if (active) {
+      const unsigned long long kd = s_kd[tid], k2 = s_k2[tid];
+      const float depth = kd ? fkey_inv((uint32_t)(kd >> 32)) : -kInf;
+      const float d2 = (k2 != ~0ull) ? __uint_as_float((uint32_t)(k2 >> 32)) : kInf;
+      ub = depth >= 0.f ? -depth : sqrtf(d2);
+    }
+    const float need = (ub + gh.rmax) * 1.0001f + rpad;
+    WalkPose wp;
+    wp.bx = bx; wp.by = by; wp.cs = cs; wp.sn = sn;
+    wp.ub = ub; wp.ub_pad = fmaf(fabsf(ub), 1e-4f, ub) + 2e-4f + cpad; wp.rpad = rpad;
+    wp.seed_rec = seed_rec;
+    wp.cx0 = wp.cx1 = wp.pad0 = wp.pad1 = 0;
+    if (active && need >= 0.f) {
+      wp.cx0 = grid_coord(bx - need, gh.x0, gh.sx, G); wp.cx1 = grid_coord(bx + need, gh.x0, gh.sx, G);
+      row_next = grid_coord(by - need, gh.y0, gh.sy, G);
+      n_rows = grid_coord(by + need, gh.y0, gh.sy, G) - row_next + 1;
+    }
+    s_walk[tid] = wp;
   }
+  if (tid == 0) s_n2 = 0;
+
   while (true) {
-    while (!done) {
-      if (i >= e) {
-        if (++row > cy1) { done = true; break; }
-        i = __ldg(gcell + row * G + cx0);
-        e = __ldg(gcell + row * G + cx1 + 1);
-        continue;
+    __syncthreads();                                       // (s_nseg = 0 and the previous round's reads are done)
+    // every pose appends as many of its remaining rows as fit into the segment list
+    if (n_rows > 0) {
+      const int base = atomicAdd(&s_nseg, n_rows);
+      const int take = min(n_rows, max(kSeg - base, 0));
+      for (int r = 0; r < take; ++r) s_seg[base + r] = (unsigned short)((tid << 6) | (row_next + r));
+      row_next += take;
+      n_rows -= take;
+    }
+    __syncthreads();
+    const int n_seg = min(s_nseg, kSeg);
+    // ---- circles: lane per segment, resumable when queue 1 fills
+    int seg = tid, i = 0, e = 0, pose = 0;
+    float wbx = 0.f, wby = 0.f, wub = 0.f, wrpad = 0.f;
+    int wseed = -1;
+    bool cdone = false;
+    while (true) {
+      while (!cdone) {
+        if (i >= e) {
+          if (seg >= n_seg) { cdone = true; break; }
+          const int sv = s_seg[seg];
+          seg += NP;
+          pose = sv >> 6;
+          const WalkPose& wp = s_walk[pose];
+          const int row = sv & 63;
+          i = __ldg(gcell + row * G + wp.cx0);
+          e = __ldg(gcell + row * G + wp.cx1 + 1);
+          wbx = wp.bx; wby = wp.by; wub = wp.ub; wrpad = wp.rpad; wseed = wp.seed_rec;
+          continue;
+        }
+        float4 b[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) b[u] = __ldg(gcirc + min(i + u, e - 1));   // four independent loads in flight
+        unsigned hit = 0u;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const float dx = b[u].x - wbx, dy = b[u].y - wby;
+          const float t = (wub + b[u].z) * 1.0001f + wrpad;
+          const bool ok = (i + u < e) && !(t < 0.f) && !(fmaf(dx, dx, dy * dy) > t * t) && (__float_as_int(b[u].w) != wseed);
+          hit |= ok ? (1u << u) : 0u;
+        }
+        if (hit) {
+          const int cnt = __popc(hit);
+          const int at = atomicAdd(&s_n1, cnt);
+          if (at + cnt > kQueue) {                         // queue 1 full: these four entries again next round
+            for (int w = at; w < kQueue; ++w) s_q1[w] = make_int2(0, -1);   // reserved, not filled
+            break;
+          }
+          int w = at;
+#pragma unroll
+          for (int u = 0; u < 4; ++u)
+            if (hit & (1u << u)) s_q1[w++] = make_int2(pose, i + u);
+        }
+        i += 4;
       }
-      float4 b[4];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) b[u] = __ldg(gcirc + min(i + u, e - 1));   // four independent loads in flight
-      bool full = false;
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        if (full || i + u >= e) continue;
-        const float dx = b[u].x - bx, dy = b[u].y - by;
-        const float t = (ub + b[u].z) * 1.0001f + rpad;
-        if ((t < 0.f) || (fmaf(dx, dx, dy * dy) > t * t) || __float_as_int(b[u].w) == seed_rec) continue;
+      __syncthreads();
+      // (after the first failed reservation the counter is past the end, so every later one fails
+      // too: valid entries, then the failed reservation's blanked slots up to the end)
+      const int n1 = min(s_n1, kQueue);
+      // ---- boxes: lane per circle survivor
+      for (int j = tid; j < n1; j += NP) {
+        const int2 it = s_q1[j];
+        if (it.y < 0) continue;                            // slot reserved by a failed push
+        const WalkPose& wp = s_walk[it.x];
+        const float4 c = __ldg(gcirc + it.y);
+        const float4 o = __ldg(gobb + it.y);               // (ux, uy, hx, hy)
+        const float dx = c.x - wp.bx, dy = c.y - wp.by, pcs = wp.cs, psn = wp.sn;
         // box-box separating-axis bound: sd(boxes) = max over the four box axes of the gap of the
         // projections (exact when they overlap, a lower bound of the distance otherwise), and
         // sd(footprint, obstacle) >= sd(boxes) because each polygon lies inside its box
-        const float4 o = __ldg(gobb + i + u);              // (ux, uy, hx, hy)
-        const float a1 = fabsf(fmaf(o.x, cs, o.y * sn)), a2 = fabsf(fmaf(o.y, cs, -o.x * sn));
+        const float a1 = fabsf(fmaf(o.x, pcs, o.y * psn)), a2 = fabsf(fmaf(o.y, pcs, -o.x * psn));
         const float g0 = fabsf(fmaf(dx, o.x, dy * o.y)) - (o.z + fmaf(fp.bhx, a1, fp.bhy * a2));
         const float g1 = fabsf(fmaf(dy, o.x, -dx * o.y)) - (o.w + fmaf(fp.bhx, a2, fp.bhy * a1));
-        const float g2 = fabsf(fmaf(dx, cs, dy * sn)) - (fp.bhx + fmaf(o.z, a1, o.w * a2));
-        const float g3 = fabsf(fmaf(dy, cs, -dx * sn)) - (fp.bhy + fmaf(o.z, a2, o.w * a1));
-        if (fmaxf(fmaxf(g0, g1), fmaxf(g2, g3)) > ub_pad) continue;
-        const int at = atomicAdd(&s_count, 1);
-        if (at >= kCullQueue) { full = true; i += u; continue; }   // queue full: retry this entry next round
-        s_queue[at] = make_int2(tid, __float_as_int(b[u].w));
+        const float g2 = fabsf(fmaf(dx, pcs, dy * psn)) - (fp.bhx + fmaf(o.z, a1, o.w * a2));
+        const float g3 = fabsf(fmaf(dy, pcs, -dx * psn)) - (fp.bhy + fmaf(o.z, a2, o.w * a1));
+        if (fmaxf(fmaxf(g0, g1), fmaxf(g2, g3)) > wp.ub_pad) continue;
+        s_q2[atomicAdd(&s_n2, 1)] = make_int2(it.x, __float_as_int(c.w));   // (never more than n1 <= kQueue)
       }
-      if (full) break;
-      i += 4;
+      __syncthreads();
+      drain(s_n2);
+      __syncthreads();
+      if (tid == 0) { s_n1 = 0; s_n2 = 0; }
+      if (__syncthreads_and(cdone)) break;
     }
-    __syncthreads();
-    const int nq = min(s_count, kCullQueue);
-    drain(nq);
-    __syncthreads();
-    if (tid == 0) s_count = 0;
-    if (__syncthreads_and(done)) break;
+    if (tid == 0) s_nseg = 0;
+    if (__syncthreads_and(n_rows == 0)) break;
   }
 
   if (p.stats) {
@@ -318,7 +403,7 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
       atomicAdd(p.stats + 1, (unsigned long long)s_stat[1]);
     }
   }
-  if (k >= p.N) return;
+  // ---- tail: value, witness gradient (penetrating poses compacted into the first lanes), stores
   const unsigned long long kd = s_kd[tid], k2 = s_k2[tid];
   const float maxDepth = kd ? fkey_inv((uint32_t)(kd >> 32)) : -kInf;
   const int idDepth = kd ? (int)(0xffffffffu - (uint32_t)kd) : -1;
@@ -326,17 +411,42 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
   const int idD2 = (k2 != ~0ull) ? (int)(uint32_t)k2 : -1;
   const bool separated = !(maxDepth >= 0.f);
   const float value = separated ? sqrtf(minD2) : -maxDepth;
-  Posed<V> Ps;
-  {
-    const PosedSlot<V>& sp = s_pose[tid];
-    Ps.px = x; Ps.py = y;
+  const int slot = separated ? idD2 : idDepth;
+  auto posed_of = [&](int q, Posed<V>& Ps) {
+    const PosedSlot<V>& sp = s_pose[q];
+    Ps.px = sp.px; Ps.py = sp.py;
 #pragma unroll
     for (int l = 0; l < V / 2; ++l) {
       Ps.rx[2 * l] = sp.rx[l].x; Ps.rx[2 * l + 1] = sp.rx[l].y; Ps.ry[2 * l] = sp.ry[l].x; Ps.ry[2 * l + 1] = sp.ry[l].y;
       Ps.Tx[2 * l] = sp.Tx[l].x; Ps.Tx[2 * l + 1] = sp.Tx[l].y; Ps.Ty[2 * l] = sp.Ty[l].x; Ps.Ty[2 * l + 1] = sp.Ty[l].y;
     }
+  };
+  float g[3] = {0.f, 0.f, 0.f};
+  if (MODE & (kGrad | kCoeff)) {
+    const bool want = active && slot >= 0;
+    if (want && !separated) {                              // queue this pose for the compacted pass
+      s_pen[atomicAdd(&s_npen, 1)] = (unsigned short)tid;
+      s_walk[tid].seed_rec = __float_as_int(__ldg(&p.bounds[2 * slot].w));   // (the walk is over: reuse the field)
+    }
+    if (want && separated) {
+      Posed<V> Ps;
+      posed_of(tid, Ps);
+      witness_separated<V>(fp, Ps, recs, __float_as_int(__ldg(&p.bounds[2 * slot].w)), g);
+    }
+    __syncthreads();
+    if (tid < s_npen) {
+      const int q = s_pen[tid];
+      Posed<V> Ps;
+      posed_of(q, Ps);
+      float gp[3];
+      witness_penetrating<V>(fp, Ps, recs, s_walk[q].seed_rec, gp);
+      s_g[q][0] = gp[0]; s_g[q][1] = gp[1]; s_g[q][2] = gp[2];
+    }
+    __syncthreads();
+    if (want && !separated) { g[0] = s_g[tid][0]; g[1] = s_g[tid][1]; g[2] = s_g[tid][2]; }
   }
-  finalize_pose<V, MODE>(fp, p, Ps, n, th, value, separated ? idD2 : idDepth, separated);
+  if (k >= p.N) return;
+  finalize_store<MODE>(fp, p, n, finite, value, slot, g);
 }
 
 }  // namespace psdf

@@ -239,12 +239,11 @@ __device__ __forceinline__ float fkey_inv(uint32_t k) {
 // candidates overlap in the pipe; loads run one edge ahead), pass 2 recomputes that one
 // candidate with its witness points.  Ties go to the first candidate in (edge, vertex, pool)
 // order.
+// The winner's pair records (two edges each: q0, q1 = (A, t), q2 = (h0, h1, last, slot)) are read
+// again: the evaluation pass of this CTA has just pulled them into L1.
 template <int V>
-__device__ __forceinline__ void witness_gradient(const Footprint& fp, const Posed<V>& P,
-                                                 const float4* __restrict__ recs, int rec_begin,
-                                                 bool separated, float* g) {
-  // The winner's pair records (two edges each: q0, q1 = (A, t), q2 = (h0, h1, last, slot))
-  // are read again: the evaluation pass of this CTA has just pulled them into L1.
+__device__ __forceinline__ void witness_separated(const Footprint& fp, const Posed<V>& P,
+                                                  const float4* __restrict__ recs, int rec_begin, float* g) {
   float nx = 0.f, ny = 0.f, cx = 0.f, cy = 0.f;
   const float4* __restrict__ src = recs + 3 * (size_t)rec_begin;
   // edge `j` of the obstacle (j = 2 * record + half), whichever half it is
@@ -254,138 +253,161 @@ __device__ __forceinline__ void witness_gradient(const Footprint& fp, const Pose
     const float4 q2 = __ldg(r + 2);
     h = (j & 1) ? q2.y : q2.x;
   };
-  if (separated) {
-    float best = kInf;
-    int idx = 0;                                           // (j * V + l) * 2 + pool
-    int base = 0;
-    for (const float4* r = src;; r += 3) {
-      const float4 c0 = __ldg(r), c1 = __ldg(r + 1), q2 = __ldg(r + 2);
-      const float h0 = q2.x, h1 = q2.y;
-      const bool more = __float_as_int(q2.z) < 0;
+  float best = kInf;
+  int idx = 0;                                           // (j * V + l) * 2 + pool
+  int base = 0;
+  for (const float4* r = src;; r += 3) {
+    const float4 c0 = __ldg(r), c1 = __ldg(r + 1), q2 = __ldg(r + 2);
+    const float h0 = q2.x, h1 = q2.y;
+    const bool more = __float_as_int(q2.z) < 0;
 #pragma unroll
-      for (int half = 0; half < 2; ++half) {
-        const float4 e0 = half ? c1 : c0;
-        const float h = half ? h1 : h0;
-        if (half && !(h1 >= 0.f)) break;                   // odd edge count: second half unused
-        const float ax = e0.x - P.px, ay = e0.y - P.py, tx = e0.z, ty = e0.w;
-#pragma unroll
-        for (int l = 0; l < V; ++l) {
-          const float dx = P.rx[l] - ax, dy = P.ry[l] - ay;
-          // pool 1: robot vertex l -> obstacle edge j
-          const float sig = dy * tx - dx * ty;
-          const float tm = fmaf(dx, tx, dy * ty) - h;
-          const float ex = fmaxf(fabsf(tm), h) - h;
-          const float d1 = fmaf(ex, ex, sig * sig);
-          // pool 2: obstacle vertex a_j -> robot edge l
-          const float Tx = P.Tx[l], Ty = P.Ty[l];
-          const float sigp = -(dy * Tx - dx * Ty);
-          const float tmp = -fmaf(dx, Tx, dy * Ty) - fp.h[l];
-          const float exp_ = fmaxf(fabsf(tmp), fp.h[l]) - fp.h[l];
-          const float d2 = fmaf(exp_, exp_, sigp * sigp);
-          const bool p1 = d1 < best;
-          best = p1 ? d1 : best;
-          idx = p1 ? base + 2 * l : idx;
-          const bool p2 = d2 < best;
-          best = p2 ? d2 : best;
-          idx = p2 ? base + 2 * l + 1 : idx;
-        }
-        base += 2 * V;
-      }
-      if (!more) break;
-    }
-    // pass 2: the winning candidate again, with its witness
-    const int j = idx / (2 * V), l = (idx / 2) % V;
-    float4 e0;
-    float h;
-    edge_at(j, e0, h);
-    const float ax = e0.x - P.px, ay = e0.y - P.py;
-    float rx = 0.f, ry = 0.f, Tx = 0.f, Ty = 0.f, hl = 0.f;
-#pragma unroll
-    for (int q = 0; q < V; ++q)
-      if (q == l) { rx = P.rx[q]; ry = P.ry[q]; Tx = P.Tx[q]; Ty = P.Ty[q]; hl = fp.h[q]; }
-    const float dx = rx - ax, dy = ry - ay;
-    if (!(idx & 1)) {                                      // (w - Q) = sig n + ex t
-      const float tx = e0.z, ty = e0.w;
-      const float sig = dy * tx - dx * ty;
-      const float tm = fmaf(dx, tx, dy * ty) - h;
-      const float ex = copysignf(fmaxf(fabsf(tm), h) - h, tm);
-      const float inv = rsqrtf(fmaxf(fmaf(ex, ex, sig * sig), 1e-30f));
-      nx = (ex * tx - sig * ty) * inv;
-      ny = (ex * ty + sig * tx) * inv;
-      cx = rx;
-      cy = ry;
-    } else {                                               // (a - Q) = sig' N + ex' T
-      const float sig = -(dy * Tx - dx * Ty);
-      const float tm = -fmaf(dx, Tx, dy * Ty) - hl;
-      const float ex = copysignf(fmaxf(fabsf(tm), hl) - hl, tm);
-      const float inv = rsqrtf(fmaxf(fmaf(ex, ex, sig * sig), 1e-30f));
-      const float ux = (ex * Tx - sig * Ty), uy = (ex * Ty + sig * Tx);      // a - Q
-      nx = -ux * inv;
-      ny = -uy * inv;
-      cx = ax - ux;
-      cy = ay - uy;
-    }
-  } else {
-    float bestO = kInf;                                    // minimum obstacle-face depth and its edge
-    int jO = 0;
-    float gR[V];                                           // robot-face depths and the edge whose start is deepest
-    int jR[V];
-#pragma unroll
-    for (int l = 0; l < V; ++l) { gR[l] = -kInf; jR[l] = 0; }
-    int j = 0;
-    for (const float4* r = src;; r += 3) {
-      const float4 c0 = __ldg(r), c1 = __ldg(r + 1), q2 = __ldg(r + 2);
-      const float h1 = q2.y;
-      const bool more = __float_as_int(q2.z) < 0;
-#pragma unroll
-      for (int half = 0; half < 2; ++half) {
-        if (half && !(h1 >= 0.f)) break;
-        const float4 e0 = half ? c1 : c0;
-        const float ax = e0.x - P.px, ay = e0.y - P.py, tx = e0.z, ty = e0.w;
-        float gj = -kInf;
-#pragma unroll
-        for (int l = 0; l < V; ++l) {
-          const float dx = P.rx[l] - ax, dy = P.ry[l] - ay;
-          gj = fmaxf(gj, dy * tx - dx * ty);
-          const float sigp = -(dy * P.Tx[l] - dx * P.Ty[l]);
-          const bool pr = sigp > gR[l];
-          gR[l] = pr ? sigp : gR[l];
-          jR[l] = pr ? j : jR[l];
-        }
-        const bool po = gj < bestO;
-        bestO = po ? gj : bestO;
-        jO = po ? j : jO;
-        ++j;
-      }
-      if (!more) break;
-    }
-    float best = bestO;
-    int face = -1, jF = jO;                                // -1: obstacle face jO, else robot face
-#pragma unroll
-    for (int l = 0; l < V; ++l)
-      if (gR[l] < best) { best = gR[l]; face = l; jF = jR[l]; nx = -P.Ty[l]; ny = P.Tx[l]; }
-    float4 e0;
-    float h;
-    edge_at(jF, e0, h);
-    const float ax = e0.x - P.px, ay = e0.y - P.py;
-    if (face < 0) {                                        // n = -n_in of edge jO, c = its deepest robot vertex
-      const float tx = e0.z, ty = e0.w;
-      float gj = -kInf;
+    for (int half = 0; half < 2; ++half) {
+      const float4 e0 = half ? c1 : c0;
+      const float h = half ? h1 : h0;
+      if (half && !(h1 >= 0.f)) break;                   // odd edge count: second half unused
+      const float ax = e0.x - P.px, ay = e0.y - P.py, tx = e0.z, ty = e0.w;
 #pragma unroll
       for (int l = 0; l < V; ++l) {
-        const float sig = (P.ry[l] - ay) * tx - (P.rx[l] - ax) * ty;
-        if (sig > gj) { gj = sig; cx = P.rx[l]; cy = P.ry[l]; }
+        const float dx = P.rx[l] - ax, dy = P.ry[l] - ay;
+        // pool 1: robot vertex l -> obstacle edge j
+        const float sig = dy * tx - dx * ty;
+        const float tm = fmaf(dx, tx, dy * ty) - h;
+        const float ex = fmaxf(fabsf(tm), h) - h;
+        const float d1 = fmaf(ex, ex, sig * sig);
+        // pool 2: obstacle vertex a_j -> robot edge l
+        const float Tx = P.Tx[l], Ty = P.Ty[l];
+        const float sigp = -(dy * Tx - dx * Ty);
+        const float tmp = -fmaf(dx, Tx, dy * Ty) - fp.h[l];
+        const float exp_ = fmaxf(fabsf(tmp), fp.h[l]) - fp.h[l];
+        const float d2 = fmaf(exp_, exp_, sigp * sigp);
+        const bool p1 = d1 < best;
+        best = p1 ? d1 : best;
+        idx = p1 ? base + 2 * l : idx;
+        const bool p2 = d2 < best;
+        best = p2 ? d2 : best;
+        idx = p2 ? base + 2 * l + 1 : idx;
       }
-      nx = ty;
-      ny = -tx;
-    } else {                                               // c = the obstacle vertex deepest behind robot face `face`
-      cx = ax;
-      cy = ay;
+      base += 2 * V;
     }
+    if (!more) break;
+  }
+  // pass 2: the winning candidate again, with its witness
+  const int j = idx / (2 * V), l = (idx / 2) % V;
+  float4 e0;
+  float h;
+  edge_at(j, e0, h);
+  const float ax = e0.x - P.px, ay = e0.y - P.py;
+  float rx = 0.f, ry = 0.f, Tx = 0.f, Ty = 0.f, hl = 0.f;
+#pragma unroll
+  for (int q = 0; q < V; ++q)
+    if (q == l) { rx = P.rx[q]; ry = P.ry[q]; Tx = P.Tx[q]; Ty = P.Ty[q]; hl = fp.h[q]; }
+  const float dx = rx - ax, dy = ry - ay;
+  if (!(idx & 1)) {                                      // (w - Q) = sig n + ex t
+    const float tx = e0.z, ty = e0.w;
+    const float sig = dy * tx - dx * ty;
+    const float tm = fmaf(dx, tx, dy * ty) - h;
+    const float ex = copysignf(fmaxf(fabsf(tm), h) - h, tm);
+    const float inv = rsqrtf(fmaxf(fmaf(ex, ex, sig * sig), 1e-30f));
+    nx = (ex * tx - sig * ty) * inv;
+    ny = (ex * ty + sig * tx) * inv;
+    cx = rx;
+    cy = ry;
+  } else {                                               // (a - Q) = sig' N + ex' T
+    const float sig = -(dy * Tx - dx * Ty);
+    const float tm = -fmaf(dx, Tx, dy * Ty) - hl;
+    const float ex = copysignf(fmaxf(fabsf(tm), hl) - hl, tm);
+    const float inv = rsqrtf(fmaxf(fmaf(ex, ex, sig * sig), 1e-30f));
+    const float ux = (ex * Tx - sig * Ty), uy = (ex * Ty + sig * Tx);      // a - Q
+    nx = -ux * inv;
+    ny = -uy * inv;
+    cx = ax - ux;
+    cy = ay - uy;
   }
   g[0] = nx;
   g[1] = ny;
   g[2] = cx * ny - cy * nx;
 }
+
+template <int V>
+__device__ __forceinline__ void witness_penetrating(const Footprint& fp, const Posed<V>& P,
+                                                    const float4* __restrict__ recs, int rec_begin, float* g) {
+  float nx = 0.f, ny = 0.f, cx = 0.f, cy = 0.f;
+  const float4* __restrict__ src = recs + 3 * (size_t)rec_begin;
+  // edge `j` of the obstacle (j = 2 * record + half), whichever half it is
+  auto edge_at = [&](int j, float4& e0, float& h) {
+    const float4* r = src + 3 * (j >> 1);
+    e0 = __ldg(r + (j & 1));
+    const float4 q2 = __ldg(r + 2);
+    h = (j & 1) ? q2.y : q2.x;
+  };
+  float bestO = kInf;                                    // minimum obstacle-face depth and its edge
+  int jO = 0;
+  float gR[V];                                           // robot-face depths and the edge whose start is deepest
+  int jR[V];
+#pragma unroll
+  for (int l = 0; l < V; ++l) { gR[l] = -kInf; jR[l] = 0; }
+  int j = 0;
+  for (const float4* r = src;; r += 3) {
+    const float4 c0 = __ldg(r), c1 = __ldg(r + 1), q2 = __ldg(r + 2);
+    const float h1 = q2.y;
+    const bool more = __float_as_int(q2.z) < 0;
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+      if (half && !(h1 >= 0.f)) break;
+      const float4 e0 = half ? c1 : c0;
+      const float ax = e0.x - P.px, ay = e0.y - P.py, tx = e0.z, ty = e0.w;
+      float gj = -kInf;
+#pragma unroll
+      for (int l = 0; l < V; ++l) {
+        const float dx = P.rx[l] - ax, dy = P.ry[l] - ay;
+        gj = fmaxf(gj, dy * tx - dx * ty);
+        const float sigp = -(dy * P.Tx[l] - dx * P.Ty[l]);
+        const bool pr = sigp > gR[l];
+        gR[l] = pr ? sigp : gR[l];
+        jR[l] = pr ? j : jR[l];
+      }
+      const bool po = gj < bestO;
+      bestO = po ? gj : bestO;
+      jO = po ? j : jO;
+      ++j;
+    }
+    if (!more) break;
+  }
+  float best = bestO;
+  int face = -1, jF = jO;                                // -1: obstacle face jO, else robot face
+#pragma unroll
+  for (int l = 0; l < V; ++l)
+    if (gR[l] < best) { best = gR[l]; face = l; jF = jR[l]; nx = -P.Ty[l]; ny = P.Tx[l]; }
+  float4 e0;
+  float h;
+  edge_at(jF, e0, h);
+  const float ax = e0.x - P.px, ay = e0.y - P.py;
+  if (face < 0) {                                        // n = -n_in of edge jO, c = its deepest robot vertex
+    const float tx = e0.z, ty = e0.w;
+    float gj = -kInf;
+#pragma unroll
+    for (int l = 0; l < V; ++l) {
+      const float sig = (P.ry[l] - ay) * tx - (P.rx[l] - ax) * ty;
+      if (sig > gj) { gj = sig; cx = P.rx[l]; cy = P.ry[l]; }
+    }
+    nx = ty;
+    ny = -tx;
+  } else {                                               // c = the obstacle vertex deepest behind robot face `face`
+    cx = ax;
+    cy = ay;
+  }
+  g[0] = nx;
+  g[1] = ny;
+  g[2] = cx * ny - cy * nx;
+}
+
+template <int V>
+__device__ __forceinline__ void witness_gradient(const Footprint& fp, const Posed<V>& P,
+                                                 const float4* __restrict__ recs, int rec_begin,
+                                                 bool separated, float* g) {
+  if (separated) witness_separated<V>(fp, P, recs, rec_begin, g);
+  else witness_penetrating<V>(fp, P, recs, rec_begin, g);
+}
+
 
 }  // namespace psdf

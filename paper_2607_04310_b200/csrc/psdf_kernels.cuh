@@ -46,11 +46,11 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N_>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N_)); }
 
-// H6-H8 tail shared by both kernels: value, gradient (or MPC coefficients), stores.
-template <int V, int MODE>
-__device__ __forceinline__ void finalize_pose(const Footprint& fp, const EvalParams& p, const Posed<V>& P,
-                                              int n, float th, float value, int slot, bool separated) {
-  const bool finite = isfinite(P.px) && isfinite(P.py) && isfinite(th);
+// H6-H8 tail shared by all kernels: stores of value and gradient (or MPC coefficients).  `g` is the
+// witness gradient of a finite pose that sees an obstacle, zero otherwise.
+template <int MODE>
+__device__ __forceinline__ void finalize_store(const Footprint& fp, const EvalParams& p, int n, bool finite,
+                                               float value, int slot, const float* gw) {
   float g[3] = {0.f, 0.f, 0.f};
   if (!finite) {
     value = __int_as_float(0x7fc00000);
@@ -58,8 +58,7 @@ __device__ __forceinline__ void finalize_pose(const Footprint& fp, const EvalPar
   } else if (slot < 0) {
     value = kInf;                                  // no valid obstacle at all
   } else if (MODE & (kGrad | kCoeff)) {
-    witness_gradient<V>(fp, P, reinterpret_cast<const float4*>(p.pairs), __float_as_int(__ldg(&p.bounds[2 * slot].w)),
-                        separated, g);
+    g[0] = gw[0]; g[1] = gw[1]; g[2] = gw[2];
   }
   if (p.packed) {                                   // zero-copy staging: one 16-byte store per pose
     if (!(MODE & kCoeff)) reinterpret_cast<float4*>(p.packed)[n] = make_float4(value, g[0], g[1], g[2]);
@@ -78,6 +77,17 @@ __device__ __forceinline__ void finalize_pose(const Footprint& fp, const EvalPar
     const float c0 = (finite && slot < 0) ? kInf : value - p.d_min - gamma;
     reinterpret_cast<float4*>(p.coeff)[n] = make_float4(c0, -g[0], -g[1], -g[2]);
   }
+}
+
+template <int V, int MODE>
+__device__ __forceinline__ void finalize_pose(const Footprint& fp, const EvalParams& p, const Posed<V>& P,
+                                              int n, float th, float value, int slot, bool separated) {
+  const bool finite = isfinite(P.px) && isfinite(P.py) && isfinite(th);
+  float g[3] = {0.f, 0.f, 0.f};
+  if (finite && slot >= 0 && (MODE & (kGrad | kCoeff)))
+    witness_gradient<V>(fp, P, reinterpret_cast<const float4*>(p.pairs), __float_as_int(__ldg(&p.bounds[2 * slot].w)),
+                        separated, g);
+  finalize_store<MODE>(fp, p, n, finite, value, slot, g);
 }
 
 // ------------------------------------------------------------------------------------------
