@@ -350,6 +350,8 @@ def main():
         torch.cuda.synchronize()
 
     w = load_workload(args.workload, rank)
+    if os.environ.get("PSDF_BENCH_SHUFFLE"):                  # diagnostic: destroys the spatial coherence of trajectory batches
+        w.poses = w.poses[np.random.default_rng(1).permutation(w.N)].copy()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
     run = DeviceRun(torch, psdf, w, flush)
     scene, value, grad = run.scene, run.value, run.grad

@@ -81,6 +81,7 @@ struct psdf_scene {
     float4* gbounds = nullptr;        // [2 M] bounds in obstacle-grid order
     int* gcell = nullptr;             // [kObsGridMax^2 + 1]
     GridHdr* ghdr = nullptr;
+    GridHdr grid{};                   // host copy of *ghdr (travels in the launch parameters)
     bool grid_ok = false;             // the obstacle grid matches this set's bounds (built lazily)
   } pk[2];
   int cur = 0;
@@ -97,8 +98,10 @@ struct psdf_scene {
   int* d_pair_begin = nullptr;        // [M+1]
   PackTotals* d_totals = nullptr;
   PackTotals* h_totals = nullptr;     // pinned
+  GridHdr* h_ghdr = nullptr;          // pinned: read-back of a freshly built grid header
   int* h_pair_begin_pinned = nullptr; // pinned [M+1]
-  int tune_bd = 0, tune_chunks = 0, tune_branches = 0;   // measurement sweeps (PSDF_TUNING builds only)
+  int tune_bd = 0, tune_chunks = 0, tune_branches = 0, tune_cull_np = 0;   // measurement sweeps (PSDF_TUNING builds only)
+  float grid_per_cell = 2.f;          // obstacles per cell of the culled path's grid (measured: DESIGN.md 6.7)
   int culling = 0;                    // psdf_set_culling
   // host path
   bool host_ready = false;
@@ -162,17 +165,29 @@ cudaError_t launch_mode(const psdf_scene* sc, const EvalParams& p, int mode, boo
   }
 }
 
-template <int V, int NP>
-cudaError_t launch_cull_mode(const psdf_scene* sc, const EvalParams& p, int mode, cudaStream_t st) {
-  const dim3 grid((unsigned)((p.N + NP - 1) / NP));
-  switch (mode) {
-    case 0: psdf_cull_kernel<V, 0, NP><<<grid, NP, 0, st>>>(sc->fp, p); break;
-    case kGrad: psdf_cull_kernel<V, kGrad, NP><<<grid, NP, 0, st>>>(sc->fp, p); break;
-    case kCoeff: psdf_cull_kernel<V, kCoeff, NP><<<grid, NP, 0, st>>>(sc->fp, p); break;
-    default: return cudaErrorInvalidValue;
+template <int V, int MODE, int NP>
+cudaError_t launch_cull_one(const psdf_scene* sc, const EvalParams& p, cudaStream_t st) {
+  constexpr int bytes = CullShape<V, NP>::kBytes;
+  static bool opted_in = false;                  // > 48 KB of dynamic shared memory is opt-in, once per kernel
+  if (!opted_in && bytes > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(psdf_cull_kernel<V, MODE, NP>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return e;
+    opted_in = true;
   }
+  const dim3 grid((unsigned)((p.N + NP - 1) / NP));
+  psdf_cull_kernel<V, MODE, NP><<<grid, NP, bytes, st>>>(sc->fp, p);
   g_launches.fetch_add(1);
   return cudaGetLastError();
+}
+
+template <int V, int NP>
+cudaError_t launch_cull_mode(const psdf_scene* sc, const EvalParams& p, int mode, cudaStream_t st) {
+  switch (mode) {
+    case 0: return launch_cull_one<V, 0, NP>(sc, p, st);
+    case kGrad: return launch_cull_one<V, kGrad, NP>(sc, p, st);
+    case kCoeff: return launch_cull_one<V, kCoeff, NP>(sc, p, st);
+    default: return cudaErrorInvalidValue;
+  }
 }
 
 template <int NP>
@@ -193,8 +208,13 @@ cudaError_t launch_cull_v(const psdf_scene* sc, const EvalParams& p, int mode, c
 cudaError_t enqueue_culled(const psdf_scene* sc, EvalParams& p, int mode, cudaStream_t st) {
   p.gbounds = sc->pk[sc->cur].gbounds;
   p.gcell = sc->pk[sc->cur].gcell;
-  p.ghdr = sc->pk[sc->cur].ghdr;
+  p.grid = sc->pk[sc->cur].grid;
   p.n_chunks = 1;
+#ifdef PSDF_TUNING
+  if (sc->tune_cull_np == 32) return launch_cull_v<32>(sc, p, mode, st);
+  if (sc->tune_cull_np == 64) return launch_cull_v<64>(sc, p, mode, st);
+  if (sc->tune_cull_np == 128) return launch_cull_v<128>(sc, p, mode, st);
+#endif
   if (p.N <= 32768) return launch_cull_v<32>(sc, p, mode, st);
   return launch_cull_v<128>(sc, p, mode, st);
 }
@@ -273,7 +293,8 @@ psdf_status enqueue_eval(const psdf_scene* sc, const EvalCall& c, cudaStream_t s
   const bool lanes = lanes_plan(sc, N) || window != nullptr;
   dim3 grid;
   int bd;
-  if (sc->culling && !lanes && N > kCullMinPoses && !per_obs && sc->Mv >= 64) {
+  // (the culled kernel packs a grid entry / pair record index into 24 bits next to the pose)
+  if (sc->culling && !lanes && N > kCullMinPoses && !per_obs && sc->Mv >= 64 && sc->n_pairs < (1 << 24)) {
     cudaError_t e = enqueue_culled(sc, p, mode, st);
     if (e != cudaSuccess) return cuda_failed(e);
     return PSDF_OK;
@@ -330,12 +351,18 @@ psdf_status enqueue_eval(const psdf_scene* sc, const EvalCall& c, cudaStream_t s
 
 // The culled path's obstacle grid for buffer set `set`: built only while culling is
 // switched on (psdf_set_culling, and every update from then on).
-cudaError_t launch_grid(psdf_scene* sc, int set, const int* totals2, int Mv, cudaStream_t st) {
+cudaError_t launch_grid(psdf_scene* sc, int set, const int* totals2, int Mv, int n_pairs, cudaStream_t st) {
   psdf_scene::Packed& b = sc->pk[set];
-  obstacle_grid_kernel<<<1, 1024, 0, st>>>(b.bounds, Mv, totals2, b.gbounds, b.gcell, b.ghdr);
+  obstacle_grid_kernel<<<1, 1024, 0, st>>>(b.bounds, Mv, n_pairs, totals2, b.gbounds, b.gcell, b.ghdr, sc->grid_per_cell);
   g_launches.fetch_add(1);
-  b.grid_ok = true;
-  return cudaGetLastError();
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaMemcpyAsync(sc->h_ghdr, b.ghdr, sizeof(GridHdr), cudaMemcpyDeviceToHost, st);
+  return e;                             // the caller synchronises `st`, then calls grid_built()
+}
+
+void grid_built(psdf_scene* sc, int set) {
+  sc->pk[set].grid = *sc->h_ghdr;
+  sc->pk[set].grid_ok = true;
 }
 
 // An update writes the inactive buffer set, which evaluations enqueued before the PREVIOUS update may
@@ -373,13 +400,14 @@ psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const
     g_launches.fetch_add(3);
   }
   if (sc->culling)                                           // reads {status, Mv} on the device: no extra sync
-    CU_TRY(launch_grid(sc, sc->cur ^ 1, reinterpret_cast<const int*>(sc->d_totals), 0, st));
+    CU_TRY(launch_grid(sc, sc->cur ^ 1, reinterpret_cast<const int*>(sc->d_totals), 0, 0, st));
   CU_TRY(cudaMemcpyAsync(sc->h_totals, sc->d_totals, sizeof(PackTotals) + sizeof(int) * ((size_t)M + 1),
                          cudaMemcpyDeviceToHost, st));
   CU_TRY(cudaStreamSynchronize(st));                         // the only synchronisation of an update
   CU_TRY(cudaGetLastError());
   const PackTotals t = *sc->h_totals;
-  if (t.status != 0) { dst.grid_ok = false; return PSDF_ERR_DEGENERATE; }   // the live set has not been touched
+  if (t.status != 0) return PSDF_ERR_DEGENERATE;             // the live set has not been touched
+  if (sc->culling) grid_built(sc, sc->cur ^ 1);
   sc->h_pair_begin.assign(sc->h_pair_begin_pinned, sc->h_pair_begin_pinned + t.Mv + 1);
   sc->n_edges = t.n_edges;
   sc->Mv = t.Mv;
@@ -405,8 +433,9 @@ psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const u
   CU_TRY(cudaMemcpyAsync(dst.row_slot, ps.row_slot.data(), sizeof(int) * (size_t)(sc->M + 1), cudaMemcpyHostToDevice, st));
   if (Mv) CU_TRY(cudaMemcpyAsync(dst.bounds, ps.bounds.data(), sizeof(float4) * 2 * Mv, cudaMemcpyHostToDevice, st));
   if (n_empty) CU_TRY(cudaMemcpyAsync(dst.empty, ps.empty_rows.data(), sizeof(int) * n_empty, cudaMemcpyHostToDevice, st));
-  if (sc->culling) CU_TRY(launch_grid(sc, sc->cur ^ 1, nullptr, Mv, st));
+  if (sc->culling) CU_TRY(launch_grid(sc, sc->cur ^ 1, nullptr, Mv, n_pairs, st));
   CU_TRY(cudaStreamSynchronize(st));       // the staging vectors die here
+  if (sc->culling) grid_built(sc, sc->cur ^ 1);
   sc->n_edges = n_edges;
   sc->Mv = Mv;
   sc->n_empty = n_empty;
@@ -437,6 +466,7 @@ void psdf_destroy_scene(psdf_scene* sc) {
   }
   cudaFree(sc->d_win);
   if (sc->h_totals) cudaFreeHost(sc->h_totals);
+  if (sc->h_ghdr) cudaFreeHost(sc->h_ghdr);
   if (sc->h_win) cudaFreeHost(sc->h_win);
   for (auto& w : sc->ws) { cudaFree(w.depth); cudaFree(w.d2); cudaFree(w.count); cudaFree(w.stats); }
   cudaFree(sc->d_cnt); cudaFree(sc->d_offs); cudaFree(sc->d_totals);   // d_pair_begin lives inside d_totals' block
@@ -473,6 +503,8 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
   if (const char* e = std::getenv("PSDF_BD")) sc->tune_bd = std::atoi(e);
   if (const char* e = std::getenv("PSDF_CHUNKS")) sc->tune_chunks = std::atoi(e);
   if (const char* e = std::getenv("PSDF_BRANCHES")) sc->tune_branches = std::atoi(e);
+  if (const char* e = std::getenv("PSDF_CULL_NP")) sc->tune_cull_np = std::atoi(e);
+  if (const char* e = std::getenv("PSDF_GRID_PER_CELL")) sc->grid_per_cell = (float)std::atof(e);
 #endif
   const int rc = pack_footprint(footprint, V, sc->fp, sc->Vp);
   if (rc != 0) { delete sc; return rc == -1 ? PSDF_ERR_INVALID_ARG : PSDF_ERR_DEGENERATE; }
@@ -499,6 +531,7 @@ psdf_status psdf_create_scene(const float* footprint, int V, const float* A, con
       CU_TRY(cudaMalloc(&b.ghdr, sizeof(GridHdr)));
     }
     CU_TRY(cudaMallocHost(&sc->h_totals, sizeof(PackTotals) + sizeof(int) * (size_t)(M + 1)));
+    CU_TRY(cudaMallocHost(&sc->h_ghdr, sizeof(GridHdr)));
     sc->h_pair_begin_pinned = reinterpret_cast<int*>(sc->h_totals + 1);
     CU_TRY(cudaMalloc(&sc->d_cnt, sizeof(int) * (size_t)M));
     CU_TRY(cudaMalloc(&sc->d_offs, sizeof(int4) * (size_t)M));
@@ -864,8 +897,9 @@ psdf_status psdf_set_culling(psdf_scene* sc, int enable) {
   PSDF_ENTER(sc);
   if (sc->gstream) CU_TRY(cudaStreamSynchronize(sc->gstream));
   if (enable && !sc->pk[sc->cur].grid_ok) {      // built here, then kept current by every update
-    CU_TRY(launch_grid(sc, sc->cur, nullptr, sc->Mv, (cudaStream_t)0));
+    CU_TRY(launch_grid(sc, sc->cur, nullptr, sc->Mv, sc->n_pairs, (cudaStream_t)0));
     CU_TRY(cudaStreamSynchronize((cudaStream_t)0));
+    grid_built(sc, sc->cur);
   }
   sc->culling = enable ? 1 : 0;
   drop_graphs(sc);

@@ -19,28 +19,24 @@ __device__ __forceinline__ float warp_max_f(float v) { return fkey_inv(__reduce_
 // Obstacle grid: the bounds re-ordered by cell of a G x G grid over the obstacle centres
 // (row-major: a rectangle of cells is one contiguous range of `gbounds` per grid row), built on
 // the device by one CTA when culling is switched on and after every pack while it is on.
-struct GridHdr {
-  float x0, y0, sx, sy;    // cell(x) = clamp((int)((x - x0) * sx), 0, G-1)
-  float rmax;              // largest bounding-circle radius
-  float cell;              // larger cell edge [m]
-  int G, Mv;
-};
 constexpr int kObsGridMax = 64;
+constexpr int kShortRecords = 3;       // culled kernel: obstacles of up to this many pair records count as short
 
 __device__ __forceinline__ int grid_coord(float v, float v0, float s, int G) {
   return min(max((int)((v - v0) * s), 0), G - 1);      // monotone non-decreasing in v
 }
 
-// totals2 = {status, Mv} written by the device packer (or null: Mv_host is used)
+// totals2 = {status, Mv, n_edges, n_pairs} written by the device packer (or null: the host values are used)
 __global__ void __launch_bounds__(1024) obstacle_grid_kernel(const float4* __restrict__ bounds, int Mv_host,
-                                                             const int* __restrict__ totals2,
+                                                             int n_pairs_host, const int* __restrict__ totals2,
                                                              float4* __restrict__ gbounds, int* __restrict__ gcell,
-                                                             GridHdr* __restrict__ hdr) {
+                                                             GridHdr* __restrict__ hdr, float per_cell) {
   __shared__ int cnt[kObsGridMax * kObsGridMax + 1];
   __shared__ float red[5][32];
   __shared__ int wsum[32];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int Mv = totals2 ? (totals2[0] == 0 ? totals2[1] : 0) : Mv_host;
+  const int n_pairs = totals2 ? totals2[3] : n_pairs_host;
   float x0 = kInf, y0 = kInf, x1 = -kInf, y1 = -kInf, rm = 0.f;
   for (int i = tid; i < Mv; i += 1024) {
     const float4 b = bounds[2 * i];
@@ -51,7 +47,7 @@ __global__ void __launch_bounds__(1024) obstacle_grid_kernel(const float4* __res
   __syncthreads();
   x0 = warp_min_f(red[0][lane]); y0 = warp_min_f(red[1][lane]);
   x1 = warp_max_f(red[2][lane]); y1 = warp_max_f(red[3][lane]); rm = warp_max_f(red[4][lane]);
-  int G = (int)sqrtf(0.5f * (float)Mv);
+  int G = (int)sqrtf((float)Mv / per_cell);                // ~per_cell obstacles in a cell
   G = G < 1 ? 1 : (G > kObsGridMax ? kObsGridMax : G);
   const float wx = fmaxf(x1 - x0, 1e-6f), wy = fmaxf(y1 - y0, 1e-6f);
   const float sx = (float)G / wx, sy = (float)G / wy;
@@ -95,8 +91,12 @@ __global__ void __launch_bounds__(1024) obstacle_grid_kernel(const float4* __res
   // arg-max keys with the packed slot as tie-break), and a rank pass to make it deterministic would
   // be quadratic in the cell size (every obstacle in one cell: Mv^2 / 1024 steps per thread).
   for (int i = tid; i < Mv; i += 1024) {
-    const float4 b = bounds[2 * i];
+    float4 b = bounds[2 * i];
     const int at = atomicAdd(&cnt[grid_coord(b.y, y0, sy, G) * G + grid_coord(b.x, x0, sx, G)], 1);
+    // grid-ordered copy: w = first pair record (24 bits) | min(number of pair records, 127) << 24
+    const int rec = __float_as_int(b.w);
+    const int rec_end = i + 1 < Mv ? __float_as_int(bounds[2 * (i + 1)].w) : n_pairs;
+    b.w = __int_as_float(rec | (min(rec_end - rec, 127) << 24));
     gbounds[at] = b;
     gbounds[Mv + at] = bounds[2 * i + 1];
   }
@@ -119,18 +119,17 @@ __global__ void __launch_bounds__(1024) obstacle_grid_kernel(const float4* __res
 //   drain    lane per queued (pose, obstacle) pair: the dense kernel's arithmetic (edge_step2), result
 //            folded into the pose's 64-bit arg-max / arg-min keys with shared-memory atomics (the
 //            dense kernel's keys: lowest slot on ties); every pose now has a finite upper bound ub
-//   rows     thread per pose: the grid rows within ub + R_max + r_R of the pose go into a segment
-//            list, one (pose, row) per entry: a row of the cell rectangle is one contiguous range of
-//            the grid-ordered bounds
-//   circles  lane per segment: bounding-circle test of its entries against the segment's pose ->
-//            queue 1 of (pose, entry)
+//   pieces   thread per pose: the grid rows within ub + R_max + r_R of the pose (a row of the cell
+//            rectangle is one contiguous range of the grid-ordered bounds) are cut into pieces of at
+//            most eight entries: (pose, first entry, count)
+//   circles  lane per piece: bounding-circle test against the piece's pose -> queue 1 of (pose, entry)
 //   boxes    lane per queue-1 item: oriented-box separating-axis bound -> pair queue
 //   drain    as above
 //   tail     value; separated poses take their witness gradient in place, the few penetrating ones are
 //            compacted into the first lanes (their branch would otherwise run in every warp for two or
 //            three lanes); stores as in the dense kernel (finalize_store).
-// Queues and the segment list have fixed sizes: a stage that finds its output full stops, the
-// stages behind it run, and it resumes where it stopped.
+// Piece list and queues have fixed sizes: a stage that finds its output full stops, the stages
+// behind it run, and it resumes where it stopped.
 template <int V>
 struct __align__(16) PosedSlot {      // one posed footprint in shared memory
   float2 rx[V / 2], ry[V / 2], Tx[V / 2], Ty[V / 2];
@@ -141,32 +140,48 @@ struct __align__(16) WalkPose {       // what the shared stages need to know abo
   float bx, by, cs, sn;               // posed bounding-box centre, rotation
   float ub, ub_pad, rpad;             // upper bound of phi, padded copies for the two tests
   int seed_rec;                       // the seed obstacle (already evaluated)
-  int cx0, cx1, pad0, pad1;           // columns of the cell rectangle
 };
 
+// Dynamic shared memory of one CTA: 440 bytes per pose (four CTAs of 128 poses per SM), what the
+// posed footprints leave goes to the piece list and the two queues.
 template <int V, int NP>
 struct CullShape {
-  // queue entries: as many as fit next to the posed footprints in 48 KB of static shared memory
-  static constexpr int kFixed = NP * ((int)sizeof(PosedSlot<V>) + (int)sizeof(WalkPose) + 16 + 12 + 2) + NP * 8 * 2 + 64;
-  static constexpr int kQueue = (kFixed + NP * 8 * 16 <= 48 * 1024 - 256) ? NP * 8 : NP * 4;
-  static constexpr int kSeg = NP * 8;
-  static_assert(kFixed + kQueue * 16 <= 48 * 1024 - 256, "culled kernel: static shared memory budget");
+  static constexpr int kPerPose = (int)sizeof(PosedSlot<V>) + (int)sizeof(WalkPose) + 16 + 12 + 4;
+  static constexpr int kRest = 440 - kPerPose;
+  static constexpr int kPieceMul = kRest >= 192 ? 12 : (kRest >= 96 ? 6 : 4);
+  static constexpr int kQ1Mul = kRest >= 192 ? 16 : 8;
+  static constexpr int kQ2Mul = kRest >= 192 ? 8 : 4;
+  static_assert(kPieceMul * 8 + kQ1Mul * 4 + kQ2Mul * 4 <= kRest, "culled kernel: shared memory budget");
+  static constexpr int kPiece = NP * kPieceMul, kQ1 = NP * kQ1Mul, kQ2 = NP * kQ2Mul;
+  static constexpr int oPose = 0;
+  static constexpr int oWalk = oPose + NP * (int)sizeof(PosedSlot<V>);
+  static constexpr int oKd = oWalk + NP * (int)sizeof(WalkPose);
+  static constexpr int oK2 = oKd + NP * 8;
+  static constexpr int oPiece = oK2 + NP * 8;
+  static constexpr int oQ1 = oPiece + kPiece * 8;
+  static constexpr int oQ2 = oQ1 + kQ1 * 4;
+  static constexpr int oG = oQ2 + kQ2 * 4;
+  static constexpr int oPen = oG + NP * 12;
+  static constexpr int kBytes = oPen + NP * 4;
 };
 
 // NP = poses (= threads) per CTA; NP = 32 makes every warp an independent unit
 template <int V, int MODE, int NP>
 __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ Footprint fp,
                                                         const __grid_constant__ EvalParams p) {
-  constexpr int kQueue = CullShape<V, NP>::kQueue, kSeg = CullShape<V, NP>::kSeg;
-  __shared__ PosedSlot<V> s_pose[NP];
-  __shared__ WalkPose s_walk[NP];
-  __shared__ unsigned long long s_kd[NP], s_k2[NP];
-  __shared__ int2 s_q1[kQueue];          // circle survivors: (pose, grid entry)
-  __shared__ int2 s_q2[kQueue];          // pairs to evaluate: (pose, first pair record)
-  __shared__ unsigned short s_seg[kSeg]; // (pose << 6) | grid row
-  __shared__ float s_g[NP][3];           // gradients of the compacted penetrating poses
-  __shared__ unsigned short s_pen[NP];
-  __shared__ int s_n1, s_n2, s_nseg, s_npen;
+  using Sh = CullShape<V, NP>;
+  constexpr int kPiece = Sh::kPiece, kQ1 = Sh::kQ1, kQ2 = Sh::kQ2;
+  extern __shared__ __align__(16) unsigned char smem[];
+  PosedSlot<V>* s_pose = reinterpret_cast<PosedSlot<V>*>(smem + Sh::oPose);
+  WalkPose* s_walk = reinterpret_cast<WalkPose*>(smem + Sh::oWalk);
+  unsigned long long* s_kd = reinterpret_cast<unsigned long long*>(smem + Sh::oKd);
+  unsigned long long* s_k2 = reinterpret_cast<unsigned long long*>(smem + Sh::oK2);
+  int2* s_piece = reinterpret_cast<int2*>(smem + Sh::oPiece);   // (first grid entry, pose << 8 | count)
+  int* s_q1 = reinterpret_cast<int*>(smem + Sh::oQ1);          // circle survivors: (pose << 24) | grid entry
+  int* s_q2 = reinterpret_cast<int*>(smem + Sh::oQ2);          // pairs to evaluate: (pose << 24) | first pair record
+  float* s_g = reinterpret_cast<float*>(smem + Sh::oG);        // [NP][3] gradients of the compacted penetrating poses
+  int* s_pen = reinterpret_cast<int*>(smem + Sh::oPen);
+  __shared__ int s_n1, s_n2[2], s_nl[2], s_npiece, s_npen;  // (two sets of pair-queue counters, used alternately)
   __shared__ unsigned int s_stat[2];
   const int tid = threadIdx.x;
   const int k = blockIdx.x * NP + tid;
@@ -186,7 +201,7 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
   }
   s_kd[tid] = 0ull;
   s_k2[tid] = ~0ull;
-  if (tid == 0) { s_n1 = 0; s_n2 = 0; s_nseg = 0; s_npen = 0; s_stat[0] = 0u; s_stat[1] = 0u; }
+  if (tid == 0) { s_n1 = 0; s_n2[0] = 0; s_n2[1] = 0; s_nl[0] = 0; s_nl[1] = 0; s_npiece = 0; s_npen = 0; s_stat[0] = 0u; s_stat[1] = 0u; }
   __syncthreads();
   // broad-phase proxies of the posed footprint: its bounding box (centre bx,by; axes (cs,sn),
   // (-sn,cs); half extents fp.bhx, fp.bhy) and the circle of radius fp.rbox around the box centre
@@ -195,7 +210,7 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
   // coordinates themselves (the posed box centre is a rounded sum: 1 mm at 2e4 m from the origin)
   const float cpad = 4.8e-7f * fmaxf(fabsf(bx), fabsf(by));
   const float rpad = fp.rbox * 1.0001f + 1e-4f + cpad;    // footprint radius + safety
-  const GridHdr gh = *p.ghdr;
+  const GridHdr& gh = p.grid;                              // by value in the launch parameters (read back at pack time)
   const int G = gh.G;
   const float4* __restrict__ gcirc = p.gbounds;            // (cx, cy, R, first pair record), grid order
   const float4* __restrict__ gobb = p.gbounds + gh.Mv;     // (ux, uy, hx, hy), grid order
@@ -203,11 +218,14 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
   const float4* __restrict__ recs = reinterpret_cast<const float4*>(p.pairs);
   unsigned n_pair = 0, n_edge = 0;
 
-  // evaluates the first nq queued pairs, one per lane
-  auto drain = [&](int nq) {
-    for (int j = tid; j < nq; j += NP) {
-      const int2 pr = s_q2[j];
-      const PosedSlot<V>& sp = s_pose[pr.x];
+  // evaluates the queued pairs, one per lane: `ns` obstacles of few pair records queued from the front
+  // of the pair queue, `nl` longer ones from its back, so that the lanes of a warp mostly run loops of
+  // similar length
+  auto drain = [&](int ns, int nl) {
+    for (int j = tid; j < ns + nl; j += NP) {
+      const int pr = s_q2[j < ns ? j : kQ2 - 1 - (j - ns)];
+      const int q = (int)((unsigned)pr >> 24);
+      const PosedSlot<V>& sp = s_pose[q];
       Posed2<V> P;
 #pragma unroll
       for (int l = 0; l < V / 2; ++l) { P.rx[l] = sp.rx[l]; P.ry[l] = sp.ry[l]; P.Tx[l] = sp.Tx[l]; P.Ty[l] = sp.Ty[l]; }
@@ -215,7 +233,7 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
       ObstacleAcc<V> acc;
       acc.reset();
       float minD2 = kInf;
-      const float4* src = recs + 3 * (size_t)pr.y;
+      const float4* src = recs + 3 * (size_t)(pr & 0xffffff);
       float4 q0 = __ldg(src), q1 = __ldg(src + 1), q2 = __ldg(src + 2);
       int last, slot;
       while (true) {
@@ -234,8 +252,8 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
       }
       ++n_pair;
       const float depth = acc.depth();
-      atomicMax(&s_kd[pr.x], ((unsigned long long)fkey(depth) << 32) | (0xffffffffu - (unsigned)slot));
-      atomicMin(&s_k2[pr.x], ((unsigned long long)__float_as_uint(minD2) << 32) | (unsigned)slot);
+      atomicMax(&s_kd[q], ((unsigned long long)fkey(depth) << 32) | (0xffffffffu - (unsigned)slot));
+      atomicMin(&s_k2[q], ((unsigned long long)__float_as_uint(minD2) << 32) | (unsigned)slot);
     }
   };
 
@@ -258,7 +276,40 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
         }
       }
     };
-    while (true) {
+    {
+      // first rectangle (it almost always holds an obstacle): the cell ranges of up to four rows are
+      // loaded together, then the first four entries of each, so that one pose costs two dependent
+      // round trips to L2 here instead of two per row
+      const int cx0 = grid_coord(bx - ext, gh.x0, gh.sx, G), cx1 = grid_coord(bx + ext, gh.x0, gh.sx, G);
+      const int cy0 = grid_coord(by - ext, gh.y0, gh.sy, G), cy1 = grid_coord(by + ext, gh.y0, gh.sy, G);
+      int rs[4], re[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int r = min(cy0 + u, cy1);
+        rs[u] = __ldg(gcell + r * G + cx0);
+        re[u] = (cy0 + u <= cy1) ? __ldg(gcell + r * G + cx1 + 1) : rs[u];
+      }
+      float4 b[4][4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int v = 0; v < 4; ++v) b[u][v] = __ldg(gcirc + max(min(rs[u] + v, re[u] - 1), 0));
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          const float dx = b[u][v].x - bx, dy = b[u][v].y - by;
+          const float key = fmaf(dx, dx, fmaf(dy, dy, -b[u][v].z * b[u][v].z));
+          if (rs[u] + v < re[u] && key < best) { best = key; seed_rec = __float_as_int(b[u][v].w); }   // (record | count << 24)
+        }
+        scan(rs[u] + 4, re[u]);                            // (rows with more than four entries)
+      }
+      for (int row = cy0 + 4; row <= cy1; ++row) scan(__ldg(gcell + row * G + cx0), __ldg(gcell + row * G + cx1 + 1));
+      px0 = cx0; px1 = cx1; py0 = cy0; py1 = cy1;
+      ext *= 2.f;
+      if (cx0 == 0 && cy0 == 0 && cx1 == G - 1 && cy1 == G - 1) ext = -1.f;    // the whole grid already
+    }
+    while (seed_rec < 0 && ext > 0.f) {                    // rare: nothing near, the rectangle doubles
       const int cx0 = grid_coord(bx - ext, gh.x0, gh.sx, G), cx1 = grid_coord(bx + ext, gh.x0, gh.sx, G);
       const int cy0 = grid_coord(by - ext, gh.y0, gh.sy, G), cy1 = grid_coord(by + ext, gh.y0, gh.sy, G);
       for (int row = cy0; row <= cy1; ++row) {
@@ -270,18 +321,28 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
           scan(s, e);
         }
       }
-      if (seed_rec >= 0 || (cx0 == 0 && cy0 == 0 && cx1 == G - 1 && cy1 == G - 1)) break;
+      if (cx0 == 0 && cy0 == 0 && cx1 == G - 1 && cy1 == G - 1) break;
       px0 = cx0; px1 = cx1; py0 = cy0; py1 = cy1;
       ext *= 2.f;
     }
   }
-  if (seed_rec >= 0) s_q2[atomicAdd(&s_n2, 1)] = make_int2(tid, seed_rec);
+  auto push_pair = [&](int q, int w, int set) {            // w = first pair record | count << 24
+    const int at = (w >> 24) <= kShortRecords ? atomicAdd(&s_n2[set], 1) : kQ2 - 1 - atomicAdd(&s_nl[set], 1);
+    s_q2[at] = (q << 24) | (w & 0xffffff);
+  };
+  if (seed_rec >= 0) push_pair(tid, seed_rec, 0);
+  seed_rec &= seed_rec >= 0 ? 0xffffff : -1;               // from here on: the record index alone
   __syncthreads();
-  drain(s_n2);
+  drain(s_n2[0], s_nl[0]);
   __syncthreads();
+  // the pair-queue counter of one round is reset after its drain and used again two rounds later, with
+  // barriers in between: no barrier is spent on the reset itself
+  if (tid == 0) { s_n2[0] = 0; s_nl[0] = 0; }
+  int par = 1;
 
-  // ---- rows: the cell rectangle the seed bound cannot exclude
-  int row_next = 0, n_rows = 0;
+  // ---- the cell rectangle the seed bound cannot exclude: rows [row, row_end), columns [cx0, cx1]
+  int row = 0, row_end = 0, cx0 = 0, cx1 = 0;
+  int pi = 0, pe = 0;                                      // entries of the current row not yet cut into pieces
   {
     float ub = -kInf;
     if (active) {
@@ -295,103 +356,122 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
     wp.bx = bx; wp.by = by; wp.cs = cs; wp.sn = sn;
     wp.ub = ub; wp.ub_pad = fmaf(fabsf(ub), 1e-4f, ub) + 2e-4f + cpad; wp.rpad = rpad;
     wp.seed_rec = seed_rec;
-    wp.cx0 = wp.cx1 = wp.pad0 = wp.pad1 = 0;
     if (active && need >= 0.f) {
-      wp.cx0 = grid_coord(bx - need, gh.x0, gh.sx, G); wp.cx1 = grid_coord(bx + need, gh.x0, gh.sx, G);
-      row_next = grid_coord(by - need, gh.y0, gh.sy, G);
-      n_rows = grid_coord(by + need, gh.y0, gh.sy, G) - row_next + 1;
+      cx0 = grid_coord(bx - need, gh.x0, gh.sx, G); cx1 = grid_coord(bx + need, gh.x0, gh.sx, G);
+      row = grid_coord(by - need, gh.y0, gh.sy, G);
+      row_end = grid_coord(by + need, gh.y0, gh.sy, G) + 1;
     }
     s_walk[tid] = wp;
   }
-  if (tid == 0) s_n2 = 0;
 
   while (true) {
-    __syncthreads();                                       // (s_nseg = 0 and the previous round's reads are done)
-    // every pose appends as many of its remaining rows as fit into the segment list
-    if (n_rows > 0) {
-      const int base = atomicAdd(&s_nseg, n_rows);
-      const int take = min(n_rows, max(kSeg - base, 0));
-      for (int r = 0; r < take; ++r) s_seg[base + r] = (unsigned short)((tid << 6) | (row_next + r));
-      row_next += take;
-      n_rows -= take;
+    __syncthreads();                                       // (counters reset, the previous round's reads done)
+    // ---- pieces: every pose cuts its remaining rows into pieces of <= 8 entries until the list is full
+    bool room = true;
+    auto cut = [&]() {                                     // cuts [pi, pe) into pieces; false when the list is full
+      if (pi >= pe) return true;
+      const int np_ = (pe - pi + 7) >> 3;
+      const int base = atomicAdd(&s_npiece, np_);
+      const int take = min(np_, max(kPiece - base, 0));
+      for (int r = 0; r < take; ++r) s_piece[base + r] = make_int2(pi + 8 * r, (tid << 8) | min(8, pe - pi - 8 * r));
+      pi += 8 * take;
+      return take == np_;
+    };
+    room = cut();                                          // (the remainder of a row that did not fit last round)
+    while (room && row < row_end) {
+      int rs[4], re[4];                                    // the cell ranges of four rows, loaded together
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int r = min(row + u, row_end - 1);
+        rs[u] = __ldg(gcell + r * G + cx0);
+        re[u] = __ldg(gcell + r * G + cx1 + 1);
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (room && row < row_end) {
+          pi = rs[u]; pe = re[u];
+          ++row;
+          room = cut();
+        }
+      }
     }
+    const bool pdone = !(row < row_end || pi < pe);
     __syncthreads();
-    const int n_seg = min(s_nseg, kSeg);
-    // ---- circles: lane per segment, resumable when queue 1 fills
-    int seg = tid, i = 0, e = 0, pose = 0;
-    float wbx = 0.f, wby = 0.f, wub = 0.f, wrpad = 0.f;
-    int wseed = -1;
+    const int n_piece = min(s_npiece, kPiece);
+    // ---- circles: lane per piece (two steps of four entries, loads issued together); resumable when
+    // queue 1 fills
+    int pc = tid;
     bool cdone = false;
     while (true) {
-      while (!cdone) {
-        if (i >= e) {
-          if (seg >= n_seg) { cdone = true; break; }
-          const int sv = s_seg[seg];
-          seg += NP;
-          pose = sv >> 6;
-          const WalkPose& wp = s_walk[pose];
-          const int row = sv & 63;
-          i = __ldg(gcell + row * G + wp.cx0);
-          e = __ldg(gcell + row * G + wp.cx1 + 1);
-          wbx = wp.bx; wby = wp.by; wub = wp.ub; wrpad = wp.rpad; wseed = wp.seed_rec;
-          continue;
-        }
-        float4 b[4];
+      for (; pc < n_piece; pc += NP) {
+        const int2 pcx = s_piece[pc];
+        const int i0 = pcx.x, cnt = pcx.y & 0xff, pose = pcx.y >> 8;
+        const WalkPose& wp = s_walk[pose];
+        const float wbx = wp.bx, wby = wp.by, wub = wp.ub, wrpad = wp.rpad;
+        const int wseed = wp.seed_rec;
+        float4 b[8];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) b[u] = __ldg(gcirc + min(i + u, e - 1));   // four independent loads in flight
+        for (int u = 0; u < 8; ++u) b[u] = __ldg(gcirc + i0 + min(u, cnt - 1));
         unsigned hit = 0u;
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < 8; ++u) {
           const float dx = b[u].x - wbx, dy = b[u].y - wby;
           const float t = (wub + b[u].z) * 1.0001f + wrpad;
-          const bool ok = (i + u < e) && !(t < 0.f) && !(fmaf(dx, dx, dy * dy) > t * t) && (__float_as_int(b[u].w) != wseed);
+          const bool ok = (u < cnt) && !(t < 0.f) && !(fmaf(dx, dx, dy * dy) > t * t) && ((__float_as_int(b[u].w) & 0xffffff) != wseed);
           hit |= ok ? (1u << u) : 0u;
         }
         if (hit) {
-          const int cnt = __popc(hit);
-          const int at = atomicAdd(&s_n1, cnt);
-          if (at + cnt > kQueue) {                         // queue 1 full: these four entries again next round
-            for (int w = at; w < kQueue; ++w) s_q1[w] = make_int2(0, -1);   // reserved, not filled
+          const int c = __popc(hit);
+          const int at = atomicAdd(&s_n1, c);
+          if (at + c > kQ1) {                              // queue 1 full: this piece again next round
+            for (int w = at; w < kQ1; ++w) s_q1[w] = -1;   // reserved, not filled
             break;
           }
           int w = at;
-#pragma unroll
-          for (int u = 0; u < 4; ++u)
-            if (hit & (1u << u)) s_q1[w++] = make_int2(pose, i + u);
+          while (hit) {
+            const int u = __ffs(hit) - 1;
+            hit &= hit - 1;
+            s_q1[w++] = (pose << 24) | (i0 + u);
+          }
         }
-        i += 4;
       }
+      cdone = pc >= n_piece;
       __syncthreads();
       // (after the first failed reservation the counter is past the end, so every later one fails
       // too: valid entries, then the failed reservation's blanked slots up to the end)
-      const int n1 = min(s_n1, kQueue);
-      // ---- boxes: lane per circle survivor
-      for (int j = tid; j < n1; j += NP) {
-        const int2 it = s_q1[j];
-        if (it.y < 0) continue;                            // slot reserved by a failed push
-        const WalkPose& wp = s_walk[it.x];
-        const float4 c = __ldg(gcirc + it.y);
-        const float4 o = __ldg(gobb + it.y);               // (ux, uy, hx, hy)
-        const float dx = c.x - wp.bx, dy = c.y - wp.by, pcs = wp.cs, psn = wp.sn;
-        // box-box separating-axis bound: sd(boxes) = max over the four box axes of the gap of the
-        // projections (exact when they overlap, a lower bound of the distance otherwise), and
-        // sd(footprint, obstacle) >= sd(boxes) because each polygon lies inside its box
-        const float a1 = fabsf(fmaf(o.x, pcs, o.y * psn)), a2 = fabsf(fmaf(o.y, pcs, -o.x * psn));
-        const float g0 = fabsf(fmaf(dx, o.x, dy * o.y)) - (o.z + fmaf(fp.bhx, a1, fp.bhy * a2));
-        const float g1 = fabsf(fmaf(dy, o.x, -dx * o.y)) - (o.w + fmaf(fp.bhx, a2, fp.bhy * a1));
-        const float g2 = fabsf(fmaf(dx, pcs, dy * psn)) - (fp.bhx + fmaf(o.z, a1, o.w * a2));
-        const float g3 = fabsf(fmaf(dy, pcs, -dx * psn)) - (fp.bhy + fmaf(o.z, a2, o.w * a1));
-        if (fmaxf(fmaxf(g0, g1), fmaxf(g2, g3)) > wp.ub_pad) continue;
-        s_q2[atomicAdd(&s_n2, 1)] = make_int2(it.x, __float_as_int(c.w));   // (never more than n1 <= kQueue)
+      const int n1 = min(s_n1, kQ1);
+      // ---- boxes: lane per circle survivor, a slice of at most kQ2 survivors at a time -> pair queue
+      for (int base = 0; base < n1; base += kQ2) {
+        for (int j = base + tid; j < min(base + kQ2, n1); j += NP) {
+          const int it = s_q1[j];
+          if (it < 0) continue;                            // slot reserved by a failed push
+          const int q = (int)((unsigned)it >> 24), entry = it & 0xffffff;
+          const WalkPose& wp = s_walk[q];
+          const float4 c = __ldg(gcirc + entry);
+          const float4 o = __ldg(gobb + entry);            // (ux, uy, hx, hy)
+          const float dx = c.x - wp.bx, dy = c.y - wp.by, pcs = wp.cs, psn = wp.sn;
+          // box-box separating-axis bound: sd(boxes) = max over the four box axes of the gap of the
+          // projections (exact when they overlap, a lower bound of the distance otherwise), and
+          // sd(footprint, obstacle) >= sd(boxes) because each polygon lies inside its box
+          const float a1 = fabsf(fmaf(o.x, pcs, o.y * psn)), a2 = fabsf(fmaf(o.y, pcs, -o.x * psn));
+          const float g0 = fabsf(fmaf(dx, o.x, dy * o.y)) - (o.z + fmaf(fp.bhx, a1, fp.bhy * a2));
+          const float g1 = fabsf(fmaf(dy, o.x, -dx * o.y)) - (o.w + fmaf(fp.bhx, a2, fp.bhy * a1));
+          const float g2 = fabsf(fmaf(dx, pcs, dy * psn)) - (fp.bhx + fmaf(o.z, a1, o.w * a2));
+          const float g3 = fabsf(fmaf(dy, pcs, -dx * psn)) - (fp.bhy + fmaf(o.z, a2, o.w * a1));
+          if (fmaxf(fmaxf(g0, g1), fmaxf(g2, g3)) > wp.ub_pad) continue;
+          push_pair(q, __float_as_int(c.w), par);
+        }
+        __syncthreads();
+        drain(s_n2[par], s_nl[par]);
+        __syncthreads();                                   // (every lane has read the counters and its pairs)
+        if (tid == 0) { s_n2[par] = 0; s_nl[par] = 0; }
+        par ^= 1;
       }
-      __syncthreads();
-      drain(s_n2);
-      __syncthreads();
-      if (tid == 0) { s_n1 = 0; s_n2 = 0; }
+      if (tid == 0) s_n1 = 0;
       if (__syncthreads_and(cdone)) break;
     }
-    if (tid == 0) s_nseg = 0;
-    if (__syncthreads_and(n_rows == 0)) break;
+    if (tid == 0) s_npiece = 0;
+    if (__syncthreads_and(pdone)) break;
   }
 
   if (p.stats) {
@@ -425,7 +505,7 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
   if (MODE & (kGrad | kCoeff)) {
     const bool want = active && slot >= 0;
     if (want && !separated) {                              // queue this pose for the compacted pass
-      s_pen[atomicAdd(&s_npen, 1)] = (unsigned short)tid;
+      s_pen[atomicAdd(&s_npen, 1)] = tid;
       s_walk[tid].seed_rec = __float_as_int(__ldg(&p.bounds[2 * slot].w));   // (the walk is over: reuse the field)
     }
     if (want && separated) {
@@ -440,10 +520,10 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
       posed_of(q, Ps);
       float gp[3];
       witness_penetrating<V>(fp, Ps, recs, s_walk[q].seed_rec, gp);
-      s_g[q][0] = gp[0]; s_g[q][1] = gp[1]; s_g[q][2] = gp[2];
+      s_g[3 * q] = gp[0]; s_g[3 * q + 1] = gp[1]; s_g[3 * q + 2] = gp[2];
     }
     __syncthreads();
-    if (want && !separated) { g[0] = s_g[tid][0]; g[1] = s_g[tid][1]; g[2] = s_g[tid][2]; }
+    if (want && !separated) { g[0] = s_g[3 * tid]; g[1] = s_g[3 * tid + 1]; g[2] = s_g[3 * tid + 2]; }
   }
   if (k >= p.N) return;
   finalize_store<MODE>(fp, p, n, finite, value, slot, g);

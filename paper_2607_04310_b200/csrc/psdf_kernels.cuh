@@ -12,6 +12,15 @@ constexpr int kMaxChunks = 64;
 
 enum Mode : int { kGrad = 1, kPerObs = 2, kCoeff = 4 };
 
+// Obstacle grid of the culled path (psdf_cull_kernels.cuh): geometry, built on the device with the grid
+// and read back once per pack so that it travels in the launch parameters.
+struct GridHdr {
+  float x0, y0, sx, sy;    // cell(x) = clamp((int)((x - x0) * sx), 0, G-1)
+  float rmax;              // largest bounding-circle radius
+  float cell;              // larger cell edge [m]
+  int G, Mv;
+};
+
 struct EvalParams {
   const PairRec* pairs;        // [n_pairs] packed valid edges, two per record, grouped by obstacle
   const int* empty_rows;       // [n_empty] obstacle rows with no valid edge
@@ -20,7 +29,7 @@ struct EvalParams {
   const float4* bounds;        // [2 Mv] per packed obstacle: (circle, first pair record), oriented box
   const float4* gbounds;       // [2 Mv] obstacle bounds in grid order: circles, then boxes (culled path)
   const int* gcell;            // [G*G+1] obstacle-grid cell -> first entry of gbounds
-  const struct GridHdr* ghdr;  // obstacle-grid geometry
+  GridHdr grid;                // obstacle-grid geometry
   unsigned long long* stats;   // [2] culled path: evaluated (pose, obstacle) pairs, (pose, edge) steps; or null
   const float* poses;          // [N,3]
   float* value;                // [N]

@@ -48,7 +48,7 @@ def test_product_build_has_no_tuning_knobs(psdf):
     """The sweep knobs (PSDF_BD, PSDF_CHUNKS, PSDF_BRANCHES, PSDF_NO_ZERO_COPY) exist only in
     -DPSDF_TUNING measurement builds: the product library holds neither their names nor a getenv."""
     blob = open(psdf.LIB_PATH, "rb").read()
-    for knob in (b"PSDF_BD", b"PSDF_CHUNKS", b"PSDF_BRANCHES", b"PSDF_NO_ZERO_COPY"):
+    for knob in (b"PSDF_BD", b"PSDF_CHUNKS", b"PSDF_BRANCHES", b"PSDF_NO_ZERO_COPY", b"PSDF_CULL_NP", b"PSDF_GRID_PER_CELL"):
         assert knob not in blob, knob
     src = open(os.path.join(ROOT, "paper_2607_04310_b200", "csrc", "psdf_api.cu")).read()
     outside = re.sub(r"#ifdef PSDF_TUNING.*?#endif", "", src, flags=re.S)
