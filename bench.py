@@ -264,6 +264,18 @@ class DeviceRun:
         torch.cuda.synchronize()
         return [a.elapsed_time(b) for a, b in evs]
 
+    def timed_trajectories(self, n_steps, T, H, d_safe=0.5):
+        """As `timed`, for psdf_eval_trajectories (evaluation + per-trajectory reductions, one launch)."""
+        torch = self.torch
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_steps)]
+        for a, b in evs:
+            self.flush.zero_()
+            a.record(self.stream)
+            self.scene.eval_trajectories(self.poses, T, H, d_safe, grad=True, stream=self.stream)
+            b.record(self.stream)
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in evs]
+
     def e2e(self, n_steps, pin):
         """n_steps psdf_eval_host calls from HOST buffers (host clock; H2D and D2H inside).  Returns
         (seconds per step, value, grad) with the outputs of the last call."""
@@ -489,17 +501,25 @@ def main():
                 # roofline fraction of the other large configs (value+grad), same protocol as the headline
                 per = {}
                 for i in (3, 4, 5):
+                    r = run if i == args.workload else DeviceRun(torch, psdf, allw[i], flush)
                     if i == args.workload:
                         tk = t_kernel
                     else:
-                        r = DeviceRun(torch, psdf, allw[i], flush)
                         r.timed(5)
                         tk = float(np.mean(r.timed(max(args.steps // 2, 10)))) * 1e-3
-                        r.scene.close()
                     Fi = flops_per_launch(allw[i])
                     per[allw[i].name] = {"ms_per_step": tk * 1e3, "pairs_per_s": allw[i].n_pairs() / tk,
                                          "tflops": Fi / tk / 1e12, "frac": Fi / tk / 1e12 / peak_nominal,
                                          "N": allw[i].N, "M": allw[i].M, "V": allw[i].V, "what": "value+grad, dense"}
+                    tr = allw[i].meta.get("n_traj")
+                    if tr:          # trajectory batches: the same launch with the per-trajectory reductions fused in
+                        Hs = allw[i].N // tr
+                        r.timed_trajectories(3, tr, Hs)
+                        tt = float(np.mean(r.timed_trajectories(max(args.steps // 2, 10), tr, Hs)))
+                        per[allw[i].name]["with_fused_trajectory_reductions_ms"] = tt
+                        per[allw[i].name]["fused_over_plain"] = tt / (tk * 1e3)
+                    if i != args.workload:
+                        r.scene.close()
                 out["per_config"] = per
                 out["parity"] = parity_report(torch, psdf, O, allw, {1: 20, 2: 50, 3: 3000, 4: 1200, 5: 1000})
                 if not args.no_latency:

@@ -87,7 +87,7 @@ psdf_status psdf_update_scene(psdf_scene* scene, const float* A, const float* B,
  *   grad          device [N,3]  (d phi/dx, d phi/dy, d phi/dtheta), PLUS sign (the paper's
  *                               J_g = -grad);  NULL = value-only
  *   per_obstacle  device [N,M]  sd^i per obstacle row (eq.23), +INF for a row with no valid
- *                               edge;  NULL = not wanted
+ *                               edge ([N,n_obstacles] after psdf_set_components);  NULL = not wanted
  * No valid obstacle at all: value=+INF, grad=0.  Non-finite pose: NaN outputs.
  * At ties / kinks the gradient is that of one of the tied branches. */
 psdf_status psdf_eval(const psdf_scene* scene, const float* poses, int N, float* value, float* grad,
@@ -137,15 +137,34 @@ psdf_status psdf_mpc_coeffs_host(psdf_scene* scene, const float* poses, int N, f
  * branch-free evaluation). */
 psdf_status psdf_set_culling(psdf_scene* scene, int enable);
 
-/* Non-convex obstacles given as convex components (Assumption 1; eq.(6),
- * PAPER.md:93-97): folds the per-component values of psdf_eval's `per_obstacle` output,
+/* Non-convex obstacles given as convex components (Assumption 1: "non-convex = union of
+ * convex pieces"; eq.(6)), fused form: declares that the obstacle rows are components
+ * of n_obstacles obstacles, comp_to_obstacle host [M] giving the obstacle id of every row,
+ * non-decreasing and within [0, n_obstacles) (the components of one obstacle are consecutive rows;
+ * anything else is PSDF_ERR_INVALID_ARG).  From then on the `per_obstacle` output of psdf_eval and
+ * psdf_eval_host is [N, n_obstacles] with per_obstacle[n,o] = min over the valid rows of obstacle o
+ * (+INF if it has none), folded inside the evaluation kernels: no [N,M] array is formed.  value and
+ * grad are unaffected (eq.(6) is a minimum over all components anyway).  n_obstacles = 0 switches
+ * back to one value per row.  Synchronises the device. */
+psdf_status psdf_set_components(psdf_scene* scene, const int* comp_to_obstacle, int n_obstacles);
+
+/* Stand-alone form for any map: folds the per-component values of psdf_eval's `per_obstacle` output,
  * per_component device [N,M], into out device [N,n_obstacles] with
  * out[n,o] = min over rows i with comp_to_obstacle[i] == o (+INF if none); comp_to_obstacle is a
  * device [M] int32 array, ids outside [0,n_obstacles) are ignored.  Asynchronous on the stream. */
 psdf_status psdf_component_min(const float* per_component, int N, int M, const int* comp_to_obstacle,
                                int n_obstacles, float* out, void* cuda_stream);
 
-/* Sampled-trajectory batches (pose index = trajectory * H + stage): per trajectory the clearance
+/* Sampled-trajectory batches, fused form: psdf_eval on the T*H poses (pose index = trajectory * H +
+ * stage; value device [T*H], grad device [T*H,3] or NULL) with the per-trajectory reductions of
+ * psdf_trajectory_reduce computed by the same launch (the CTA that completes a trajectory reduces it:
+ * same routine, same bits as the stand-alone call).  Any of min_value / argmin_stage / penalty
+ * (device [T]) may be NULL.  T*H <= max_poses.  Asynchronous on the stream. */
+psdf_status psdf_eval_trajectories(const psdf_scene* scene, const float* poses, int T, int H, float d_safe,
+                                   float* value, float* grad, float* min_value, int* argmin_stage,
+                                   float* penalty, void* cuda_stream);
+
+/* Stand-alone form (pose index = trajectory * H + stage): per trajectory the clearance
  * min_value[t] = min_s phi, its first arg-min stage, and the soft penalty
  * penalty[t] = sum_s max(0, d_safe - phi_s)^2 (fixed summation order: deterministic).  value is
  * psdf_eval's device [T*H] output; any of the three device outputs may be NULL. */

@@ -11,7 +11,6 @@
 #include "psdf_cull_kernels.cuh"
 #include "psdf_pack.h"
 #include "psdf_pack_kernels.cuh"
-#include "psdf_reduce_kernels.cuh"
 
 using namespace psdf;
 
@@ -55,6 +54,7 @@ struct Workspace {
   unsigned long long* depth = nullptr;   // [max_poses] clean = 0
   unsigned long long* d2 = nullptr;      // [max_poses] clean = ~0
   unsigned int* count = nullptr;         // [max_poses + 1] clean = 0
+  unsigned int* traj = nullptr;          // [max_poses] per-trajectory arrival counters, clean = 0
   unsigned long long* stats = nullptr;   // [2]
 };
 
@@ -103,6 +103,12 @@ struct psdf_scene {
   int tune_bd = 0, tune_chunks = 0, tune_branches = 0, tune_cull_np = 0;   // measurement sweeps (PSDF_TUNING builds only)
   float grid_per_cell = 2.f;          // obstacles per cell of the culled path's grid (measured: DESIGN.md 6.7)
   int culling = 0;                    // psdf_set_culling
+  // psdf_set_components: obstacle rows are convex components of n_groups obstacles
+  int n_groups = 0;
+  std::vector<int> h_comp;            // [M] row -> obstacle id, non-decreasing
+  int* d_comp = nullptr;
+  std::vector<int> h_row_slot;        // [M+1] host copy of the live set's row_slot (component mode)
+  std::vector<int> h_slot_group;      // [Mv] packed obstacle -> obstacle id
   // host path
   bool host_ready = false;
   cudaStream_t gstream = nullptr;
@@ -251,6 +257,11 @@ struct EvalCall {
   const int* window = nullptr;        // per-pose obstacle row windows
   const PoseArgs* args = nullptr;     // poses travelling as a kernel parameter
   int which_ws = 0, ws_off = 0;
+  int traj_H = 0;                     // > 0: per-trajectory reductions fused into the tail
+  float d_safe = 0.f;
+  float* traj_min = nullptr;
+  int* traj_argmin = nullptr;
+  float* traj_penalty = nullptr;
 };
 
 // Launch plan: lane-split kernel for MPC-sized batches; otherwise the
@@ -288,6 +299,15 @@ psdf_status enqueue_eval(const psdf_scene* sc, const EvalCall& c, cudaStream_t s
   p.d_min = c.d_min;
   p.rho_p = c.rho_p;
   p.rho_theta = c.rho_theta;
+  const bool fold = per_obs != nullptr && sc->n_groups > 0;       // per-obstacle output folded over components
+  p.comp = fold ? sc->d_comp : nullptr;
+  p.n_groups = fold ? sc->n_groups : 0;
+  p.traj.H = c.traj_H;
+  p.traj.d_safe = c.d_safe;
+  p.traj.min_value = c.traj_min;
+  p.traj.argmin_stage = c.traj_argmin;
+  p.traj.penalty = c.traj_penalty;
+  p.traj.count = ws.traj + c.ws_off;
   const int mode = coeff ? kCoeff : ((grad ? kGrad : 0) | (per_obs ? kPerObs : 0));
 
   const bool lanes = lanes_plan(sc, N) || window != nullptr;
@@ -308,6 +328,7 @@ psdf_status enqueue_eval(const psdf_scene* sc, const EvalCall& c, cudaStream_t s
     const int K = L < 256 ? L : 256;
     int C = L / K;
     if (C > 16) C = 16;
+    if (fold) C = 1;                   // the lanes of a pose fold their components inside one CTA
     p.lanes = K;
     p.n_chunks = C;
     bd = K <= 64 ? 64 : K;
@@ -333,14 +354,20 @@ psdf_status enqueue_eval(const psdf_scene* sc, const EvalCall& c, cudaStream_t s
     if (C > kMaxChunks) C = kMaxChunks;
     const int tiles = (N + bd - 1) / bd;
     // chunk boundaries on obstacle boundaries, balanced by edge count
+    // (component mode: also between obstacles, so that every (pose, obstacle) entry has one writer)
     p.chunk_begin[0] = 0;
+    p.chunk_group[0] = 0;
     int o = 0;
     for (int c = 1; c < C; ++c) {
       const long long target = (long long)sc->n_pairs * c / C;
       while (o < sc->Mv && sc->h_pair_begin[o] < target) ++o;
+      if (fold)
+        while (o > 0 && o < sc->Mv && sc->h_slot_group[o] == sc->h_slot_group[o - 1]) ++o;
       p.chunk_begin[c] = sc->h_pair_begin[o];
+      p.chunk_group[c] = fold ? (o < sc->Mv ? sc->h_slot_group[o] : sc->n_groups) : 0;
     }
     p.chunk_begin[C] = sc->n_pairs;
+    p.chunk_group[C] = sc->n_groups;
     p.n_chunks = C;
     grid = dim3((unsigned)tiles, (unsigned)C);
   }
@@ -379,6 +406,20 @@ void note_eval_stream(const psdf_scene* csc, cudaStream_t st) {
   else if (sc->eval_stream != st) sc->eval_multi = true;
 }
 
+// Component mode (psdf_set_components): packed obstacle -> obstacle id on the host, for chunk plans
+// that end between obstacles.  `from_device`: the live set's row_slot has to be read back first.
+psdf_status rebuild_component_tables(psdf_scene* sc, bool from_device) {
+  if (sc->n_groups <= 0) return PSDF_OK;
+  if (from_device) {
+    sc->h_row_slot.resize((size_t)sc->M + 1);
+    CU_TRY(cudaMemcpy(sc->h_row_slot.data(), sc->pk[sc->cur].row_slot, sizeof(int) * ((size_t)sc->M + 1), cudaMemcpyDeviceToHost));
+  }
+  sc->h_slot_group.assign((size_t)sc->Mv, 0);
+  for (int i = 0; i < sc->M; ++i)
+    if (sc->h_row_slot[i + 1] > sc->h_row_slot[i]) sc->h_slot_group[sc->h_row_slot[i]] = sc->h_comp[i];
+  return PSDF_OK;
+}
+
 // Device-resident (A,B,S): pack on the GPU (count+validate -> scan -> write); only the
 // totals and the per-obstacle pair offsets (for the host launch plan) come back.
 psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const uint8_t* S, cudaStream_t st) {
@@ -414,7 +455,7 @@ psdf_status pack_on_device(psdf_scene* sc, const float* A, const float* B, const
   sc->n_empty = t.n_empty;
   sc->n_pairs = t.n_pairs;
   sc->cur ^= 1;
-  return PSDF_OK;
+  return rebuild_component_tables(sc, true);
 }
 
 psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const uint8_t* S, psdf_mem where,
@@ -441,8 +482,9 @@ psdf_status upload_scene(psdf_scene* sc, const float* A, const float* B, const u
   sc->n_empty = n_empty;
   sc->n_pairs = n_pairs;
   sc->h_pair_begin.swap(ps.pair_begin);
+  sc->h_row_slot.swap(ps.row_slot);
   sc->cur ^= 1;
-  return PSDF_OK;
+  return rebuild_component_tables(sc, false);
 }
 
 }  // namespace
@@ -468,7 +510,8 @@ void psdf_destroy_scene(psdf_scene* sc) {
   if (sc->h_totals) cudaFreeHost(sc->h_totals);
   if (sc->h_ghdr) cudaFreeHost(sc->h_ghdr);
   if (sc->h_win) cudaFreeHost(sc->h_win);
-  for (auto& w : sc->ws) { cudaFree(w.depth); cudaFree(w.d2); cudaFree(w.count); cudaFree(w.stats); }
+  for (auto& w : sc->ws) { cudaFree(w.depth); cudaFree(w.d2); cudaFree(w.count); cudaFree(w.traj); cudaFree(w.stats); }
+  cudaFree(sc->d_comp);
   cudaFree(sc->d_cnt); cudaFree(sc->d_offs); cudaFree(sc->d_totals);   // d_pair_begin lives inside d_totals' block
   cudaFree(sc->d_in); cudaFree(sc->d_out); cudaFree(sc->d_per);
   if (sc->h_in) cudaFreeHost(sc->h_in);
@@ -482,7 +525,9 @@ static psdf_status alloc_workspace(Workspace& w, int max_poses, cudaStream_t st)
   CU_TRY(cudaMalloc(&w.depth, sizeof(unsigned long long) * n));
   CU_TRY(cudaMalloc(&w.d2, sizeof(unsigned long long) * n));
   CU_TRY(cudaMalloc(&w.count, sizeof(unsigned int) * n_cnt));
+  CU_TRY(cudaMalloc(&w.traj, sizeof(unsigned int) * n));
   CU_TRY(cudaMalloc(&w.stats, sizeof(unsigned long long) * 2));
+  CU_TRY(cudaMemsetAsync(w.traj, 0x00, sizeof(unsigned int) * n, st));
   CU_TRY(cudaMemsetAsync(w.depth, 0x00, sizeof(unsigned long long) * n, st));
   CU_TRY(cudaMemsetAsync(w.d2, 0xff, sizeof(unsigned long long) * n, st));
   CU_TRY(cudaMemsetAsync(w.count, 0x00, sizeof(unsigned int) * n_cnt, st));
@@ -605,7 +650,7 @@ static psdf_status ensure_host_path(psdf_scene* sc, bool per_obs) {
         psdf_status s = alloc_workspace(sc->ws[1], sc->max_poses, sc->gstream);
         if (s != PSDF_OK) {                      // partial workspace: release it so that a retry starts clean
           Workspace& w = sc->ws[1];
-          cudaFree(w.depth); cudaFree(w.d2); cudaFree(w.count); cudaFree(w.stats);
+          cudaFree(w.depth); cudaFree(w.d2); cudaFree(w.count); cudaFree(w.traj); cudaFree(w.stats);
           w = Workspace();
           return s;
         }
@@ -687,7 +732,7 @@ static psdf_status run_zero_copy(psdf_scene* sc, const HostCall& h) {
       if (h.grad) { h.grad[3 * n] = sc->h_out[4 * n + 1]; h.grad[3 * n + 1] = sc->h_out[4 * n + 2]; h.grad[3 * n + 2] = sc->h_out[4 * n + 3]; }
     }
   }
-  if (h.per) std::memcpy(h.per, sc->h_per, sizeof(float) * (size_t)N * sc->M);
+  if (h.per) std::memcpy(h.per, sc->h_per, sizeof(float) * (size_t)N * (sc->n_groups > 0 ? sc->n_groups : sc->M));
   return PSDF_OK;
 }
 
@@ -707,7 +752,7 @@ static bool is_pinned_host(const void* ptr) {
 // Captured once per (N, outputs, constants, buffers); pinned caller buffers are used in place.
 static psdf_status run_graph(psdf_scene* sc, const HostCall& h) {
   const int N = h.N, mode = h.mode;
-  const size_t M = (size_t)sc->M;
+  const size_t M = (size_t)(sc->n_groups > 0 ? sc->n_groups : sc->M);   // row length of the per-obstacle output
   // sources / destinations of the copy nodes
   const bool pin_in = is_pinned_host(h.poses);
   const float* src = pin_in ? h.poses : sc->h_in;
@@ -906,14 +951,48 @@ psdf_status psdf_set_culling(psdf_scene* sc, int enable) {
   return PSDF_OK;
 }
 
+psdf_status psdf_set_components(psdf_scene* sc, const int* comp_to_obstacle, int n_obstacles) {
+  if (!sc || n_obstacles < 0 || (n_obstacles > 0 && !comp_to_obstacle)) return PSDF_ERR_INVALID_ARG;
+  PSDF_ENTER(sc);
+  if (n_obstacles > 0) {
+    if (n_obstacles > sc->M) return PSDF_ERR_INVALID_ARG;
+    for (int i = 0; i < sc->M; ++i)
+      if (comp_to_obstacle[i] < 0 || comp_to_obstacle[i] >= n_obstacles || (i > 0 && comp_to_obstacle[i] < comp_to_obstacle[i - 1]))
+        return PSDF_ERR_INVALID_ARG;                  // components of one obstacle are consecutive rows
+  }
+  if (sc->gstream) CU_TRY(cudaStreamSynchronize(sc->gstream));
+  drop_graphs(sc);
+  if (n_obstacles == 0) { sc->n_groups = 0; return PSDF_OK; }
+  if (!sc->d_comp) CU_TRY(cudaMalloc(&sc->d_comp, sizeof(int) * (size_t)sc->M));
+  CU_TRY(cudaDeviceSynchronize());                    // (evaluations in flight may still read the old map)
+  CU_TRY(cudaMemcpy(sc->d_comp, comp_to_obstacle, sizeof(int) * (size_t)sc->M, cudaMemcpyHostToDevice));
+  sc->h_comp.assign(comp_to_obstacle, comp_to_obstacle + sc->M);
+  sc->n_groups = n_obstacles;
+  const psdf_status s = rebuild_component_tables(sc, true);
+  if (s != PSDF_OK) sc->n_groups = 0;
+  return s;
+}
+
+psdf_status psdf_eval_trajectories(const psdf_scene* sc, const float* poses, int T, int H, float d_safe, float* value,
+                                   float* grad, float* min_value, int* argmin_stage, float* penalty, void* cuda_stream) {
+  if (!sc || T < 0 || H < 1 || (T > 0 && (!poses || !value))) return PSDF_ERR_INVALID_ARG;
+  if ((long long)T * H > sc->max_poses) return PSDF_ERR_CAPACITY;
+  if (T == 0) return PSDF_OK;
+  PSDF_ENTER(sc);
+  note_eval_stream(sc, (cudaStream_t)cuda_stream);
+  EvalCall c;
+  c.poses = poses; c.N = T * H; c.value = value; c.grad = grad;
+  c.traj_H = H; c.d_safe = d_safe; c.traj_min = min_value; c.traj_argmin = argmin_stage; c.traj_penalty = penalty;
+  return enqueue_eval(sc, c, (cudaStream_t)cuda_stream);
+}
+
 psdf_status psdf_component_min(const float* per_component, int N, int M, const int* comp_to_obstacle,
                                int n_obstacles, float* out, void* cuda_stream) {
   if (N < 0 || M < 1 || n_obstacles < 1 || (N > 0 && (!per_component || !comp_to_obstacle || !out)))
     return PSDF_ERR_INVALID_ARG;
   if (N == 0) return PSDF_OK;
-  const long long total = (long long)N * n_obstacles;
-  component_min_kernel<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(
-      per_component, N, M, comp_to_obstacle, n_obstacles, out);
+  component_min_kernel<<<(unsigned)N, 128, 0, (cudaStream_t)cuda_stream>>>(per_component, N, M, comp_to_obstacle,
+                                                                          n_obstacles, out);
   g_launches.fetch_add(1);
   CU_TRY(cudaGetLastError());
   return PSDF_OK;

@@ -525,8 +525,8 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
     __syncthreads();
     if (want && !separated) { g[0] = s_g[3 * tid]; g[1] = s_g[3 * tid + 1]; g[2] = s_g[3 * tid + 2]; }
   }
-  if (k >= p.N) return;
-  finalize_store<MODE>(fp, p, n, finite, value, slot, g);
+  if (k < p.N) finalize_store<MODE>(fp, p, n, finite, value, slot, g);
+  if (!(MODE & kCoeff)) trajectory_epilogue(p.traj, p.value, blockIdx.x * NP, min(NP, p.N - (int)blockIdx.x * NP));
 }
 
 }  // namespace psdf

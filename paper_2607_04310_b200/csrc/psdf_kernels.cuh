@@ -4,6 +4,7 @@
 // for MPC-sized batches.  See DESIGN.md §6.
 #pragma once
 #include "psdf_device.cuh"
+#include "psdf_reduce_kernels.cuh"
 
 namespace psdf {
 
@@ -34,7 +35,9 @@ struct EvalParams {
   const float* poses;          // [N,3]
   float* value;                // [N]
   float* grad;                 // [N,3] or null
-  float* per_obs;              // [N,M_rows] or null
+  float* per_obs;              // [N,M_rows], or [N,n_groups] when `comp` is set; or null
+  const int* comp;             // [M_rows] obstacle row -> obstacle id (psdf_set_components), or null
+  int n_groups;                // number of obstacles the components fold into
   float* coeff;                // [N,4] or null (kCoeff)
   float* packed;               // zero-copy host path: poses are [N,4], results one float4 (value, grad) per pose
   unsigned long long* ws_depth;  // [max_poses] cross-chunk arg-max keys (clean = 0)
@@ -45,6 +48,8 @@ struct EvalParams {
   int lanes;                   // lane-split kernel: lanes per pose (power of two <= 32)
   float d_min, rho_p, rho_theta;
   int chunk_begin[kMaxChunks + 1];   // pair-record offsets of the obstacle chunks
+  int chunk_group[kMaxChunks + 1];   // component mode: first obstacle id of each chunk (chunks end between obstacles)
+  TrajParams traj;                   // per-trajectory reductions fused into the tail (H = 0: none)
 };
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
@@ -128,6 +133,9 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
   acc.reset();
   float minD2 = kInf, prevD2 = kInf, maxDepth = -kInf;
   int idD2 = -1, idDepth = -1;
+  ComponentFold fold;
+  if ((MODE & kPerObs) && p.comp)
+    fold.begin(n_raw < p.N ? p.per_obs + (size_t)n * p.n_groups : nullptr, p.chunk_group[blockIdx.y]);
 
   if (n_tiles > 0) issue(0);
   for (int t = 0; t < n_tiles; ++t) {
@@ -152,8 +160,9 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
         const int slot = __float_as_int(q2.w);
         const float depth = acc.depth();
         if (MODE & kPerObs) {
-          if (n_raw < p.N)
-            p.per_obs[(size_t)n * p.M_rows + last] = depth >= 0.f ? -depth : sqrtf(minD2);
+          const float sd = depth >= 0.f ? -depth : sqrtf(minD2);            // eq.(23)
+          if (p.comp) fold.add(__ldg(p.comp + last), sd);
+          else if (n_raw < p.N) p.per_obs[(size_t)n * p.M_rows + last] = sd;
           if (minD2 < prevD2) { prevD2 = minD2; idD2 = slot; }
           minD2 = kInf;
         } else if (MODE & (kGrad | kCoeff)) {
@@ -167,7 +176,8 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
   }
   if (MODE & kPerObs) {
     minD2 = prevD2;
-    if (blockIdx.y == 0 && n_raw < p.N)
+    if (p.comp) fold.end(p.chunk_group[blockIdx.y + 1]);
+    else if (blockIdx.y == 0 && n_raw < p.N)
       for (int r = 0; r < p.n_empty; ++r) p.per_obs[(size_t)n * p.M_rows + __ldg(p.empty_rows + r)] = kInf;
   } else if (!(MODE & (kGrad | kCoeff))) {
     idD2 = minD2 < kInf ? 0 : -1;                  // value-only: winner id not tracked
@@ -188,21 +198,24 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
     if (!s_is_last) return;
     __threadfence();
     if (tid == 0) p.ws_count[blockIdx.x] = 0u;     // leave the workspace clean for the next call
-    if (n_raw >= p.N) return;
-    const unsigned long long kd = __ldcg(p.ws_depth + n), k2 = __ldcg(p.ws_d2 + n);
-    p.ws_depth[n] = 0ull;
-    p.ws_d2[n] = ~0ull;
-    maxDepth = kd ? fkey_inv((uint32_t)(kd >> 32)) : -kInf;
-    idDepth = kd ? (int)(0xffffffffu - (uint32_t)kd) : -1;
-    minD2 = (k2 != ~0ull) ? __uint_as_float((uint32_t)(k2 >> 32)) : kInf;
-    idD2 = (k2 != ~0ull) ? (int)(uint32_t)k2 : -1;
+    if (n_raw < p.N) {
+      const unsigned long long kd = __ldcg(p.ws_depth + n), k2 = __ldcg(p.ws_d2 + n);
+      p.ws_depth[n] = 0ull;
+      p.ws_d2[n] = ~0ull;
+      maxDepth = kd ? fkey_inv((uint32_t)(kd >> 32)) : -kInf;
+      idDepth = kd ? (int)(0xffffffffu - (uint32_t)kd) : -1;
+      minD2 = (k2 != ~0ull) ? __uint_as_float((uint32_t)(k2 >> 32)) : kInf;
+      idD2 = (k2 != ~0ull) ? (int)(uint32_t)k2 : -1;
+    }
   }
-  if (n_raw >= p.N) return;
-  const bool separated = !(maxDepth >= 0.f);
-  const float value = separated ? sqrtf(minD2) : -maxDepth;
-  Posed<V> Ps;
-  unpack_pose<V>(P, Ps);
-  finalize_pose<V, MODE>(fp, p, Ps, n, th, value, separated ? idD2 : idDepth, separated);
+  if (n_raw < p.N) {
+    const bool separated = !(maxDepth >= 0.f);
+    const float value = separated ? sqrtf(minD2) : -maxDepth;
+    Posed<V> Ps;
+    unpack_pose<V>(P, Ps);
+    finalize_pose<V, MODE>(fp, p, Ps, n, th, value, separated ? idD2 : idDepth, separated);
+  }
+  if (!(MODE & kCoeff)) trajectory_epilogue(p.traj, p.value, blockIdx.x * bd, min(bd, p.N - blockIdx.x * bd));
 }
 
 // ------------------------------------------------------------------------------------------
@@ -257,6 +270,15 @@ __device__ __forceinline__ void lanes_body(const Footprint& fp, const EvalParams
   pose_setup2<V>(fp, x, y, th, P);
   unsigned long long best = ~0ull;
   ObstacleAcc<V> acc;
+  // component mode (psdf_set_components; one CTA per pose group): the output row holds order-preserving
+  // keys while the lanes min-reduce their components into it, then is turned back into floats
+  const bool fold = (MODE & kPerObs) && p.comp != nullptr;
+  unsigned int* krow = fold ? reinterpret_cast<unsigned int*>(p.per_obs + (size_t)n * p.n_groups) : nullptr;
+  if (fold) {
+    if (n_raw < p.N)
+      for (int o = lane; o < p.n_groups; o += K) krow[o] = fkey(kInf);
+    __syncthreads();
+  }
   while (slot < s_end) {
     const int slot_next = slot + K * C;
     const int rec_next = slot_next < s_end ? __float_as_int(__ldg(&p.bounds[2 * slot_next].w)) : 0;
@@ -281,14 +303,22 @@ __device__ __forceinline__ void lanes_body(const Footprint& fp, const EvalParams
     }
     const float depth = acc.depth();
     const float sd = depth >= 0.f ? -depth : sqrtf(d2);            // eq.(23)
-    if ((MODE & kPerObs) && n_raw < p.N) p.per_obs[(size_t)n * p.M_rows + last] = sd;
+    if ((MODE & kPerObs) && n_raw < p.N) {
+      if (fold) atomicMin(krow + __ldg(p.comp + last), fkey(sd));
+      else p.per_obs[(size_t)n * p.M_rows + last] = sd;
+    }
     const unsigned long long key = ((unsigned long long)fkey(sd) << 32) | (unsigned)slot;
     best = key < best ? key : best;
     slot = slot_next;
     rec = rec_next;
   }
-  if ((MODE & kPerObs) && n_raw < p.N && blockIdx.y == 0)
+  if (fold) {
+    __syncthreads();
+    if (n_raw < p.N)
+      for (int o = lane; o < p.n_groups; o += K) p.per_obs[(size_t)n * p.n_groups + o] = fkey_inv(krow[o]);
+  } else if ((MODE & kPerObs) && n_raw < p.N && blockIdx.y == 0) {
     for (int r = lane; r < p.n_empty; r += K) p.per_obs[(size_t)n * p.M_rows + __ldg(p.empty_rows + r)] = kInf;
+  }
   // arg-min over the lanes of the group: within the warp ...
   for (int o = (K < 32 ? K : 32) >> 1; o > 0; o >>= 1) {
     const unsigned long long other = __shfl_xor_sync(0xffffffffu, best, o);
@@ -322,6 +352,8 @@ __device__ __forceinline__ void lanes_body(const Footprint& fp, const EvalParams
     unpack_pose<V>(P, Ps);
     finalize_pose<V, MODE>(fp, p, Ps, n, th, value, any ? (int)(uint32_t)best : -1, value > 0.f);
   }
+  if (!(MODE & kCoeff) && !p.packed)
+    trajectory_epilogue(p.traj, p.value, blockIdx.x * ppc, min(ppc, p.N - (int)blockIdx.x * ppc));
 }
 
 template <int V, int MODE>

@@ -27,7 +27,7 @@ PSDF_MEM_DEVICE = 1
 # include/psdf.h: the product ABI
 EXPORTS = ["psdf_create_scene", "psdf_update_scene", "psdf_eval", "psdf_eval_host",
            "psdf_eval_windows", "psdf_eval_windows_host", "psdf_mpc_coeffs_host", "psdf_component_min",
-           "psdf_trajectory_reduce", "psdf_set_culling", "psdf_destroy_scene", "psdf_scene_num_obstacles",
+           "psdf_trajectory_reduce", "psdf_set_components", "psdf_eval_trajectories", "psdf_set_culling", "psdf_destroy_scene", "psdf_scene_num_obstacles",
            "psdf_scene_num_edges", "psdf_last_cuda_error", "psdf_status_string", "psdf_version"]
 # include/psdf_bench.h: measurement instrumentation (bench.py, tests)
 BENCH_EXPORTS = ["psdf_kernel_launches", "psdf_cull_stats", "psdf_measure_fp32_peak", "psdf_bench_host_latency"]
@@ -68,6 +68,10 @@ def lib():
     L.psdf_eval_windows_host.argtypes = [vp, fp_, i, vp, fp_, fp_]
     L.psdf_mpc_coeffs_host.restype = i
     L.psdf_mpc_coeffs_host.argtypes = [vp, fp_, i, ctypes.c_float, ctypes.c_float, ctypes.c_float, fp_]
+    L.psdf_set_components.restype = i
+    L.psdf_set_components.argtypes = [vp, vp, i]
+    L.psdf_eval_trajectories.restype = i
+    L.psdf_eval_trajectories.argtypes = [vp, fp_, i, i, ctypes.c_float, fp_, fp_, fp_, vp, fp_, vp]
     L.psdf_set_culling.restype = i
     L.psdf_set_culling.argtypes = [vp, i]
     L.psdf_component_min.restype = i
@@ -167,6 +171,7 @@ class Scene:
             where = PSDF_MEM_HOST
             keep = (A_, B_, S_)
         self.M, self.E, self.max_poses = M, E, int(max_poses)
+        self.n_out = M                      # row length of the per-obstacle output (set_components changes it)
         h = ctypes.c_void_p()
         _check(lib().psdf_create_scene(fp_ptr, self.V, pa, pb, ps, M, E, where, int(max_poses),
                                        _stream_ptr(stream), ctypes.byref(h)), "psdf_create_scene")
@@ -198,6 +203,34 @@ class Scene:
         """psdf_set_culling: exact broad-phase culling for large batches (default off)."""
         _check(lib().psdf_set_culling(self._h, int(bool(enable))), "psdf_set_culling")
 
+    def set_components(self, comp_to_obstacle, n_obstacles: int):
+        """psdf_set_components: rows are convex components of n_obstacles obstacles (ids non-decreasing);
+        per_obstacle outputs become [N, n_obstacles].  n_obstacles = 0 switches back."""
+        if n_obstacles:
+            comp, pc = _host(comp_to_obstacle, np.int32)
+            assert comp.shape == (self.M,)
+        else:
+            pc = None
+        _check(lib().psdf_set_components(self._h, pc, int(n_obstacles)), "psdf_set_components")
+        self.n_out = int(n_obstacles) if n_obstacles else self.M
+
+    def eval_trajectories(self, poses, T, H, d_safe, grad=True, stream=None):
+        """psdf_eval_trajectories: device poses [T*H,3] -> (value, grad, min_value[T], argmin_stage[T], penalty[T])."""
+        import torch
+        N = int(T) * int(H)
+        assert int(poses.shape[0]) == N
+        dev = poses.device
+        value = torch.empty(N, dtype=torch.float32, device=dev)
+        g = torch.empty((N, 3), dtype=torch.float32, device=dev) if grad else None
+        mn = torch.empty(int(T), dtype=torch.float32, device=dev)
+        am = torch.empty(int(T), dtype=torch.int32, device=dev)
+        pen = torch.empty(int(T), dtype=torch.float32, device=dev)
+        _check(lib().psdf_eval_trajectories(self._h, _dev_ptr(poses, "float32"), int(T), int(H), float(d_safe),
+                                            _dev_ptr(value, "float32"), _dev_ptr(g, "float32") if grad else None,
+                                            _dev_ptr(mn, "float32"), _dev_ptr(am, "int32"), _dev_ptr(pen, "float32"),
+                                            _stream_ptr(stream)), "psdf_eval_trajectories")
+        return value, g, mn, am, pen
+
     def cull_stats(self, stream=None):
         """psdf_cull_stats: (evaluated (pose, obstacle) pairs, (pose, edge) steps) since the last call."""
         out = (ctypes.c_ulonglong * 2)()
@@ -227,7 +260,7 @@ class Scene:
         if grad is True:
             grad = torch.empty((N, 3), dtype=torch.float32, device=poses.device)
         if per_obstacle is True:
-            per_obstacle = torch.empty((N, self.M), dtype=torch.float32, device=poses.device)
+            per_obstacle = torch.empty((N, self.n_out), dtype=torch.float32, device=poses.device)
         want_g = grad is not False and grad is not None
         want_po = per_obstacle is not False and per_obstacle is not None
         pg = _dev_ptr(grad, "float32") if want_g else None
@@ -242,7 +275,7 @@ class Scene:
         N = int(poses.shape[0])
         value = np.empty(N, np.float32)
         g = np.empty((N, 3), np.float32) if grad else None
-        po = np.empty((N, self.M), np.float32) if per_obstacle else None
+        po = np.empty((N, self.n_out), np.float32) if per_obstacle else None
         _check(lib().psdf_eval_host(self._h, pp, N, value.ctypes.data,
                                     g.ctypes.data if g is not None else None,
                                     po.ctypes.data if po is not None else None), "psdf_eval_host")
@@ -291,7 +324,7 @@ class Scene:
         for a in (poses, value, grad, per_obstacle):
             assert a is None or (a.dtype == np.float32 and a.flags.c_contiguous)
         assert value.shape[0] == N and (grad is None or grad.shape == (N, 3))
-        assert per_obstacle is None or per_obstacle.shape == (N, self.M)
+        assert per_obstacle is None or per_obstacle.shape == (N, self.n_out)
         fn, h = lib().psdf_eval_host, self._h
         args = (h, poses.ctypes.data, N, value.ctypes.data, grad.ctypes.data if grad is not None else None,
                 per_obstacle.ctypes.data if per_obstacle is not None else None)
@@ -326,7 +359,7 @@ class Scene:
         N = int(poses.shape[0])
         value = np.empty(N, np.float32)
         g = np.empty((N, 3), np.float32) if grad else None
-        po = np.empty((N, self.M), np.float32) if per_obstacle else None
+        po = np.empty((N, self.n_out), np.float32) if per_obstacle else None
         c = np.empty((N, 4), np.float32) if coeffs else None
         d_min, rho_p, rho_theta = coeffs if coeffs else (0.0, 0.0, 0.0)
         out = (ctypes.c_double * int(reps))()
@@ -395,6 +428,14 @@ def psdf_trajectory_reduce(value, T, H, d_safe, stream=None):
                                         _dev_ptr(mn, "float32"), _dev_ptr(am, "int32"), _dev_ptr(pen, "float32"),
                                         _stream_ptr(stream)), "psdf_trajectory_reduce")
     return mn, am, pen
+
+
+def psdf_set_components(scene: Scene, comp_to_obstacle, n_obstacles: int):
+    return scene.set_components(comp_to_obstacle, n_obstacles)
+
+
+def psdf_eval_trajectories(scene: Scene, poses, T, H, d_safe, **kw):
+    return scene.eval_trajectories(poses, T, H, d_safe, **kw)
 
 
 def psdf_set_culling(scene: Scene, enable: bool):
