@@ -518,6 +518,25 @@ def main():
                         tt = float(np.mean(r.timed_trajectories(max(args.steps // 2, 10), tr, Hs)))
                         per[allw[i].name]["with_fused_trajectory_reductions_ms"] = tt
                         per[allw[i].name]["fused_over_plain"] = tt / (tk * 1e3)
+                    if i == 3:      # per-pose obstacle row windows (psdf_eval_windows, lane-split kernel at any N) at this size
+                        wi = allw[i]
+                        stage = np.arange(wi.N, dtype=np.int64) % 50
+                        w0 = (stage * (wi.M - 64) // 49).astype(np.int32)            # a 64-row window sliding with the stage
+                        win = torch.from_numpy(np.stack([w0, w0 + 64], 1).astype(np.int32)).cuda()
+                        full = torch.from_numpy(np.tile(np.array([[0, wi.M]], np.int32), (wi.N, 1))).cuda()
+                        for name, wt in (("eval_windows_64_rows_ms", win), ("eval_windows_all_rows_ms", full)):
+                            for _ in range(3):
+                                r.scene.eval_windows(r.poses, wt, grad=True)
+                            evs = []
+                            for _ in range(10):
+                                flush.zero_()
+                                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                                a.record(r.stream)
+                                r.scene.eval_windows(r.poses, wt, grad=True, stream=r.stream)
+                                b.record(r.stream)
+                                evs.append((a, b))
+                            torch.cuda.synchronize()
+                            per[wi.name][name] = float(np.mean([a.elapsed_time(b) for a, b in evs]))
                     if i != args.workload:
                         r.scene.close()
                 out["per_config"] = per
