@@ -140,7 +140,7 @@ psdf_status psdf_set_culling(psdf_scene* scene, int enable);
 /* Non-convex obstacles given as convex components (Assumption 1: "non-convex = union of
  * convex pieces"; eq.(6)), fused form: declares that the obstacle rows are components
  * of n_obstacles obstacles, comp_to_obstacle host [M] giving the obstacle id of every row,
- * non-decreasing and within [0, n_obstacles) (the components of one obstacle are consecutive rows;
+ * non-decreasing and within [0, n_obstacles), n_obstacles <= M (the components of one obstacle are consecutive rows;
  * anything else is PSDF_ERR_INVALID_ARG).  From then on the `per_obstacle` output of psdf_eval and
  * psdf_eval_host is [N, n_obstacles] with per_obstacle[n,o] = min over the valid rows of obstacle o
  * (+INF if it has none), folded inside the evaluation kernels: no [N,M] array is formed.  value and

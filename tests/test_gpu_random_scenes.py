@@ -107,6 +107,31 @@ def test_random_scenes_every_path(env, block):
             want = seg.min() if seg.size and np.isfinite(seg).any() else np.inf
             got = float(vw[n])
             assert (np.isinf(want) and np.isinf(got)) or abs(got - want) <= 1e-5 + 4 * abs(want) * 2.0 ** -23, (tag, n)
+        # NEXT-4 fused: random non-decreasing component map (rows in groups of 1..4), trajectories of a
+        # random length that divides N
+        sizes = []
+        while sum(sizes) < Mrows:
+            sizes.append(int(rng.integers(1, 5)))
+        ids = np.repeat(np.arange(len(sizes)), sizes)[:Mrows].astype(np.int32)
+        n_obs = min(int(ids.max()) + 1 + int(rng.integers(0, 2)), Mrows)      # (n_obstacles <= M)
+        scene.set_components(ids, n_obs)
+        vf_, gf_, pof = scene.eval(p, grad=True, per_obstacle=True)
+        assert torch.equal(vf_, v) and torch.equal(gf_, g), tag + " components: value/grad"
+        assert torch.equal(pof, psdf.psdf_component_min(po, torch.from_numpy(ids).cuda(), n_obs)), tag + " components: fused == stand-alone"
+        want = O.component_min(ref.per_obstacle, ids, n_obs)
+        got = pof.cpu().numpy().astype(np.float64)[idx]
+        assert np.array_equal(np.isposinf(got), np.isposinf(want)), tag
+        fin2 = np.isfinite(want)
+        assert (np.abs(got[fin2] - want[fin2]) <= 1e-5 + 4 * np.abs(want[fin2]) * 2.0 ** -23).all(), tag + " components vs oracle"
+        _, _, pofh = scene.eval_host(poses[idx], grad=True, per_obstacle=True)
+        assert np.array_equal(pofh, pof.cpu().numpy()[idx]), tag + " components: host path"
+        scene.set_components(None, 0)
+        divs = [h for h in (1, 2, 3, 5, 7, 10, 30, 60, 100, 600) if N % h == 0]
+        H = int(rng.choice(divs))
+        vt, gt, mn, am, pen = scene.eval_trajectories(p, N // H, H, 0.4, grad=True)
+        mn0, am0, pen0 = psdf.psdf_trajectory_reduce(v, N // H, H, 0.4)
+        assert torch.equal(vt, v) and torch.equal(gt, g), tag + " trajectories: value/grad"
+        assert torch.equal(mn, mn0) and torch.equal(am, am0) and torch.equal(pen, pen0), tag + f" trajectories H={H}"
         # update to shifted obstacles == fresh scene; device-resident update back == original
         sh = np.array([0.5, -0.25], np.float32)
         fresh = psdf.Scene(footprint, A + sh, B + sh, S, max_poses=max(N, 8))
