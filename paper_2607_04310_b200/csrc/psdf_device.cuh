@@ -10,8 +10,9 @@
 //   * per (l, j):  sigma = (r_l - a_j).n_j, tau_m = (r_l - a_j).t_j - h_j   (pool 1,
 //     eqs.(12)-(14) PAPER.md:153-167) and sigma' = (a_j - r_l).N_l,
 //     tau'_m = (a_j - r_l).T_l - h_l (pool 2, eq.(15));
-//     point-to-segment d^2 = sigma^2 + (max(|tau_m|, h) - h)^2  (eq.(13) with the clamp
-//     of eq.(12) written around the edge midpoint);
+//     point-to-segment d^2 = sigma^2 + max(|tau_m| - h, 0)^2  (eq.(13) with the clamp
+//     of eq.(12) written around the edge midpoint; as FADD2 with |.| + two FMNMX against zero:
+//     64 operand bits per vertex pair fewer than max(|tau_m|, h) - h, same bits out);
 //   * SAT (eqs.(17)-(22) PAPER.md:181-217), one-sided: face depth G_j = max_l sigma,
 //     G'_l = max_j sigma'; depth^i = min over the faces of both polygons; separated^i
 //     <=> depth^i < 0 (eq.21); pen = depth^i otherwise (eq.22) — the "other side" term of
@@ -199,7 +200,8 @@ __device__ __forceinline__ void edge_step2(const Footprint& fp, const Posed2<V>&
     // pool 1 + obstacle axis j
     const float2 s = __ffma2_rn(P.ry[l], tx, __ffma2_rn(P.rx[l], nty, ncn));
     const float2 u = __ffma2_rn(P.rx[l], tx, __ffma2_rn(P.ry[l], ty, nct));
-    const float2 e = __fadd2_rn(make_float2(fmaxf(fabsf(u.x), h), fmaxf(fabsf(u.y), h)), nh);
+    const float2 et = __fadd2_rn(make_float2(fabsf(u.x), fabsf(u.y)), nh);
+    const float2 e = make_float2(fmaxf(et.x, 0.f), fmaxf(et.y, 0.f));
     const float2 d = __ffma2_rn(e, e, __fmul2_rn(s, s));
     gj = fmax3(gj, s.x, s.y);
     // pool 2 + robot axes l, l+1
@@ -209,7 +211,8 @@ __device__ __forceinline__ void edge_step2(const Footprint& fp, const Posed2<V>&
     const float2 nhR = *reinterpret_cast<const float2*>(&fp.nh[2 * l]);
     const float2 pp = __ffma2_rn(ay, P.Tx[l], __ffma2_rn(nax, P.Ty[l], ncN));
     const float2 w = __ffma2_rn(ax, P.Tx[l], __ffma2_rn(ay, P.Ty[l], ncT));
-    const float2 f = __fadd2_rn(make_float2(fmaxf(fabsf(w.x), hR.x), fmaxf(fabsf(w.y), hR.y)), nhR);
+    const float2 ft = __fadd2_rn(make_float2(fabsf(w.x), fabsf(w.y)), nhR);
+    const float2 f = make_float2(fmaxf(ft.x, 0.f), fmaxf(ft.y, 0.f));
     const float2 g = __ffma2_rn(f, f, __fmul2_rn(pp, pp));
     acc.gR[2 * l] = fmaxf(acc.gR[2 * l], pp.x);
     acc.gR[2 * l + 1] = fmaxf(acc.gR[2 * l + 1], pp.y);
