@@ -184,7 +184,10 @@ __device__ __forceinline__ void unpack_pose(const Posed2<V>& P2, Posed<V>& P) {
 __device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
 
 // Hot inner step (H2-H5) for one edge against all V robot vertices/edges, two at a time.
-template <int V>
+// SUB_FIRST picks between two forms of the clamp that give the same bits: max(|tau| - h, 0) reads 64
+// register-operand bits per vertex pair less (throughput kernels: DESIGN.md 6.4); max(|tau|, h) - h lets
+// the compiler keep more of the latency-bound lane-split kernel in flight (MPC p50 0.4 us lower).
+template <int V, bool SUB_FIRST = true>
 __device__ __forceinline__ void edge_step2(const Footprint& fp, const Posed2<V>& P, const float4 q,
                                            const float h, ObstacleAcc<V>& acc, float& minD2) {
   const float sax = q.x - P.px, say = q.y - P.py;                 // H2: a_j = A_j - p
@@ -200,8 +203,13 @@ __device__ __forceinline__ void edge_step2(const Footprint& fp, const Posed2<V>&
     // pool 1 + obstacle axis j
     const float2 s = __ffma2_rn(P.ry[l], tx, __ffma2_rn(P.rx[l], nty, ncn));
     const float2 u = __ffma2_rn(P.rx[l], tx, __ffma2_rn(P.ry[l], ty, nct));
-    const float2 et = __fadd2_rn(make_float2(fabsf(u.x), fabsf(u.y)), nh);
-    const float2 e = make_float2(fmaxf(et.x, 0.f), fmaxf(et.y, 0.f));
+    float2 e;
+    if (SUB_FIRST) {
+      const float2 et = __fadd2_rn(make_float2(fabsf(u.x), fabsf(u.y)), nh);
+      e = make_float2(fmaxf(et.x, 0.f), fmaxf(et.y, 0.f));
+    } else {
+      e = __fadd2_rn(make_float2(fmaxf(fabsf(u.x), h), fmaxf(fabsf(u.y), h)), nh);
+    }
     const float2 d = __ffma2_rn(e, e, __fmul2_rn(s, s));
     gj = fmax3(gj, s.x, s.y);
     // pool 2 + robot axes l, l+1
@@ -211,8 +219,13 @@ __device__ __forceinline__ void edge_step2(const Footprint& fp, const Posed2<V>&
     const float2 nhR = *reinterpret_cast<const float2*>(&fp.nh[2 * l]);
     const float2 pp = __ffma2_rn(ay, P.Tx[l], __ffma2_rn(nax, P.Ty[l], ncN));
     const float2 w = __ffma2_rn(ax, P.Tx[l], __ffma2_rn(ay, P.Ty[l], ncT));
-    const float2 ft = __fadd2_rn(make_float2(fabsf(w.x), fabsf(w.y)), nhR);
-    const float2 f = make_float2(fmaxf(ft.x, 0.f), fmaxf(ft.y, 0.f));
+    float2 f;
+    if (SUB_FIRST) {
+      const float2 ft = __fadd2_rn(make_float2(fabsf(w.x), fabsf(w.y)), nhR);
+      f = make_float2(fmaxf(ft.x, 0.f), fmaxf(ft.y, 0.f));
+    } else {
+      f = __fadd2_rn(make_float2(fmaxf(fabsf(w.x), hR.x), fmaxf(fabsf(w.y), hR.y)), nhR);
+    }
     const float2 g = __ffma2_rn(f, f, __fmul2_rn(pp, pp));
     acc.gR[2 * l] = fmaxf(acc.gR[2 * l], pp.x);
     acc.gR[2 * l + 1] = fmaxf(acc.gR[2 * l + 1], pp.y);

@@ -297,8 +297,8 @@ __device__ __forceinline__ void lanes_body(const Footprint& fp, const EvalParams
         src = recs + 3 * (size_t)rec_next;
         q0 = __ldg(src); q1 = __ldg(src + 1); q2 = __ldg(src + 2);
       }
-      edge_step2<V>(fp, P, c0, h0, acc, d2);
-      if (h1 >= 0.f) edge_step2<V>(fp, P, c1, h1, acc, d2);
+      edge_step2<V, false>(fp, P, c0, h0, acc, d2);
+      if (h1 >= 0.f) edge_step2<V, false>(fp, P, c1, h1, acc, d2);
       if (last >= 0) break;
     }
     const float depth = acc.depth();
