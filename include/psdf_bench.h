@@ -15,6 +15,11 @@ extern "C" {
  * nodes): bench.py's `gpu_launches`. */
 long long psdf_kernel_launches(void);
 
+/* 1 if the scene's footprint was found centrally symmetric about its reference point at create
+ * (v_{l+V/2} == -v_l bitwise, V a multiple of 4): the kernels then take the edge step that derives half of
+ * the dot products from the other half.  Tests use it to know which variant ran. */
+int psdf_scene_footprint_symmetric(const psdf_scene* scene);
+
 /* Culled-path statistics (psdf_set_culling) accumulated since the last call (then reset):
  * out2[0] = number of evaluated (pose, obstacle) pairs, out2[1] = number of (pose, obstacle edge)
  * steps, over the stream-taking and the host entry points.  Synchronises `cuda_stream` and the

@@ -1029,6 +1029,7 @@ psdf_status psdf_cull_stats(psdf_scene* sc, void* cuda_stream, unsigned long lon
 
 int psdf_scene_num_obstacles(const psdf_scene* sc) { return sc ? sc->Mv : 0; }
 int psdf_scene_num_edges(const psdf_scene* sc) { return sc ? sc->n_edges : 0; }
+int psdf_scene_footprint_symmetric(const psdf_scene* sc) { return sc ? sc->fp.sym : 0; }
 int psdf_last_cuda_error(void) { return g_last_cuda_error.load(); }
 long long psdf_kernel_launches(void) { return g_launches.load(); }
 const char* psdf_version(void) { return "psdf-b200 0.2 (sm_100a)"; }

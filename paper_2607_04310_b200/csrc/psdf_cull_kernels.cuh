@@ -245,8 +245,13 @@ __global__ void __launch_bounds__(NP) psdf_cull_kernel(const __grid_constant__ F
           src += 3;
           q0 = __ldg(src); q1 = __ldg(src + 1); q2 = __ldg(src + 2);
         }
-        edge_step2<V>(fp, P, c0, h0, acc, minD2);
-        if (h1 >= 0.f) edge_step2<V>(fp, P, c1, h1, acc, minD2);
+        if (V % 4 == 0 && fp.sym) {                        // (uniform)
+          edge_step_any<V, true, true>(fp, P, c0, h0, acc, minD2);
+          if (h1 >= 0.f) edge_step_any<V, true, true>(fp, P, c1, h1, acc, minD2);
+        } else {
+          edge_step2<V>(fp, P, c0, h0, acc, minD2);
+          if (h1 >= 0.f) edge_step2<V>(fp, P, c1, h1, acc, minD2);
+        }
         n_edge += h1 >= 0.f ? 2u : 1u;
         if (last >= 0) break;
       }

@@ -50,6 +50,7 @@ struct __align__(16) Footprint {
   float rmax;                   // max_l |v_l|  (Prop.1)
   float bcx, bcy, bhx, bhy;     // robot-frame bounding box: centre, half extents (culled path)
   float rbox;                   // max_l |v_l - box centre|
+  int sym;                      // 1: centrally symmetric about the reference point, v_{l+V/2} == -v_l (edge_step2_sym)
 };
 
 // Per-pose state: posed footprint in registers (H1).
@@ -96,37 +97,6 @@ struct ObstacleAcc {
     return d;
   }
 };
-
-// Hot inner step H2-H5 for one packed edge against all V robot vertices/edges.
-// minD2 is min-updated with the 2V point-to-segment candidates of this edge.
-template <int V>
-__device__ __forceinline__ void edge_step(const Footprint& fp, const Posed<V>& P, const float4 e0,
-                                          const float h, ObstacleAcc<V>& acc, float& minD2) {
-  const float ax = e0.x - P.px, ay = e0.y - P.py;   // H2: a_j = A_j - p
-  const float tx = e0.z, ty = e0.w;
-  const float cn = fmaf(ay, tx, -ax * ty);          // a_j . n_j,  n_j = (-ty, tx)
-  const float ct = fmaf(ax, tx, fmaf(ay, ty, h));   // a_j . t_j + h_j
-  float gj = -kInf;
-  float m = minD2;
-#pragma unroll
-  for (int l = 0; l < V; ++l) {
-    // pool 1 + obstacle axis j
-    const float sig = fmaf(P.ry[l], tx, fmaf(-P.rx[l], ty, -cn));
-    const float tau = fmaf(P.rx[l], tx, fmaf(P.ry[l], ty, -ct));
-    const float e1 = fmaxf(fabsf(tau), h) - h;
-    const float d1 = fmaf(e1, e1, sig * sig);
-    gj = fmaxf(gj, sig);
-    // pool 2 + robot axis l
-    const float sigp = fmaf(ay, P.Tx[l], fmaf(-ax, P.Ty[l], -fp.cN[l]));
-    const float taup = fmaf(ax, P.Tx[l], fmaf(ay, P.Ty[l], -fp.cT[l]));
-    const float e2 = fmaxf(fabsf(taup), fp.h[l]) - fp.h[l];
-    const float d2 = fmaf(e2, e2, sigp * sigp);
-    acc.gR[l] = fmaxf(acc.gR[l], sigp);
-    m = fminf(fminf(m, d1), d2);
-  }
-  acc.gO = fminf(acc.gO, gj);
-  minD2 = m;
-}
 
 // Two packed edges of the same obstacle, 48 bytes (three float4): the tile-scan kernel's
 // record.  q2 = (h0, h1, last, slot): h1 < 0 marks a record whose second half is unused
@@ -234,6 +204,76 @@ __device__ __forceinline__ void edge_step2(const Footprint& fp, const Posed2<V>&
   }
   acc.gO = fminf(acc.gO, gj);
   minD2 = m;
+}
+
+// The same step for a footprint that is centrally symmetric about its reference point, v_{l+V/2} = -v_l
+// (rectangles, car outlines; V a multiple of 4; Footprint::sym, set at pack time when it holds bitwise).
+// Then r_{l+V/2} = -r_l, T_{l+V/2} = -T_l, and the constants c_N, c_T, h of edge l+V/2 equal those of edge
+// l, so the dot products of the far half follow from the near half by a sign:
+//     sigma_l  =  r_l.n_j - a_j.n_j        sigma_{l+V/2}  = -r_l.n_j - a_j.n_j        (same for tau)
+//     sigma'_l =  a_j.N_l - c_N,l          sigma'_{l+V/2} = -a_j.N_l - c_N,l          (same for tau')
+// i.e. per two vertex pairs eight FMUL2/FFMA2 and eight FADD2 instead of sixteen FFMA2: the same number
+// of instructions on the same pipe, 512 register-operand bits fewer (that is what bounds
+// the loop).  Every kernel of a scene takes the same variant, so they stay bit-identical to each other.
+template <int V, bool SUB_FIRST = true>
+__device__ __forceinline__ void edge_step2_sym(const Footprint& fp, const Posed2<V>& P, const float4 q,
+                                               const float h, ObstacleAcc<V>& acc, float& minD2) {
+  static_assert(V % 4 == 0, "symmetric variant: V must be a multiple of 4");
+  const float sax = q.x - P.px, say = q.y - P.py;                 // H2: a_j = A_j - p
+  const float sncn = fmaf(sax, q.w, -say * q.z);                  // -(a_j . n_j)
+  const float snct = -fmaf(sax, q.z, fmaf(say, q.w, h));          // -(a_j . t_j + h_j)
+  const float2 ax = bc2(sax), ay = bc2(say), nax = bc2(-sax);
+  const float2 tx = bc2(q.z), ty = bc2(q.w), nty = bc2(-q.w);
+  const float2 ncn = bc2(sncn), nct = bc2(snct), nh = bc2(-h);
+  float gj = -kInf;
+  float m = minD2;
+  auto neg2 = [](float2 a) { return make_float2(-a.x, -a.y); };
+  // H3-H5 for one vertex pair whose four dot products are known
+  auto tail = [&](const float2 s, const float2 u, const float2 pp, const float2 w, const float2 hR, const float2 nhR,
+                  float& gR0, float& gR1) {
+    float2 e, f;
+    if (SUB_FIRST) {
+      const float2 et = __fadd2_rn(make_float2(fabsf(u.x), fabsf(u.y)), nh);
+      e = make_float2(fmaxf(et.x, 0.f), fmaxf(et.y, 0.f));
+      const float2 ft = __fadd2_rn(make_float2(fabsf(w.x), fabsf(w.y)), nhR);
+      f = make_float2(fmaxf(ft.x, 0.f), fmaxf(ft.y, 0.f));
+    } else {
+      e = __fadd2_rn(make_float2(fmaxf(fabsf(u.x), h), fmaxf(fabsf(u.y), h)), nh);
+      f = __fadd2_rn(make_float2(fmaxf(fabsf(w.x), hR.x), fmaxf(fabsf(w.y), hR.y)), nhR);
+    }
+    const float2 d = __ffma2_rn(e, e, __fmul2_rn(s, s));
+    const float2 g = __ffma2_rn(f, f, __fmul2_rn(pp, pp));
+    gj = fmax3(gj, s.x, s.y);
+    gR0 = fmaxf(gR0, pp.x);
+    gR1 = fmaxf(gR1, pp.y);
+    m = fmin3(m, d.x, d.y);
+    m = fmin3(m, g.x, g.y);
+  };
+#pragma unroll
+  for (int b = 0; b < V / 4; ++b) {
+    const float2 pn = __ffma2_rn(P.ry[b], tx, __fmul2_rn(P.rx[b], nty));       // r_l . n_j,  l = 2b, 2b+1
+    const float2 pt = __ffma2_rn(P.rx[b], tx, __fmul2_rn(P.ry[b], ty));        // r_l . t_j
+    const float2 an = __ffma2_rn(ay, P.Tx[b], __fmul2_rn(nax, P.Ty[b]));       // a_j . N_l
+    const float2 at = __ffma2_rn(ax, P.Tx[b], __fmul2_rn(ay, P.Ty[b]));        // a_j . T_l
+    const float2 ncN = *reinterpret_cast<const float2*>(&fp.ncN[2 * b]);
+    const float2 ncT = *reinterpret_cast<const float2*>(&fp.ncT[2 * b]);
+    const float2 hR = *reinterpret_cast<const float2*>(&fp.h[2 * b]);
+    const float2 nhR = *reinterpret_cast<const float2*>(&fp.nh[2 * b]);
+    tail(__fadd2_rn(pn, ncn), __fadd2_rn(pt, nct), __fadd2_rn(an, ncN), __fadd2_rn(at, ncT), hR, nhR,
+         acc.gR[2 * b], acc.gR[2 * b + 1]);
+    tail(__fadd2_rn(neg2(pn), ncn), __fadd2_rn(neg2(pt), nct), __fadd2_rn(neg2(an), ncN), __fadd2_rn(neg2(at), ncT), hR, nhR,
+         acc.gR[2 * b + V / 2], acc.gR[2 * b + 1 + V / 2]);
+  }
+  acc.gO = fminf(acc.gO, gj);
+  minD2 = m;
+}
+
+// Compile-time / run-time choice of the variant: SYM instantiations exist for V % 4 == 0 only.
+template <int V, bool SUB_FIRST, bool SYM>
+__device__ __forceinline__ void edge_step_any(const Footprint& fp, const Posed2<V>& P, const float4 q, const float h,
+                                          ObstacleAcc<V>& acc, float& minD2) {
+  if constexpr (SYM && V % 4 == 0) edge_step2_sym<V, SUB_FIRST>(fp, P, q, h, acc, minD2);
+  else edge_step2<V, SUB_FIRST>(fp, P, q, h, acc, minD2);
 }
 
 // Order-preserving float -> uint32 key (works for negatives and +-inf).

@@ -3,6 +3,7 @@
 // lane-split kernel (K lanes per pose, obstacles split across lanes, warp-shuffle arg-min)
 // for MPC-sized batches.  See DESIGN.md §6.
 #pragma once
+#include <type_traits>
 #include "psdf_device.cuh"
 #include "psdf_reduce_kernels.cuh"
 
@@ -137,43 +138,50 @@ __global__ void __launch_bounds__(256) psdf_scan_kernel(const __grid_constant__ 
   if ((MODE & kPerObs) && p.comp)
     fold.begin(n_raw < p.N ? p.per_obs + (size_t)n * p.n_groups : nullptr, p.chunk_group[blockIdx.y]);
 
-  if (n_tiles > 0) issue(0);
-  for (int t = 0; t < n_tiles; ++t) {
-    if (t + 1 < n_tiles) {
-      issue(t + 1);
-      cp_async_wait<1>();
-    } else {
-      cp_async_wait<0>();
-    }
-    __syncthreads();
-    const float4* buf = tile[t & 1];
-    const int cnt = min(kTilePairs, ce - (cb + t * kTilePairs));
-#pragma unroll 1
-    for (int k = 0; k < cnt; ++k) {
-      const float4 q0 = buf[3 * k];
-      const float4 q1 = buf[3 * k + 1];
-      const float4 q2 = buf[3 * k + 2];
-      edge_step2<V>(fp, P, q0, q2.x, acc, minD2);
-      if (q2.y >= 0.f) edge_step2<V>(fp, P, q1, q2.y, acc, minD2);   // uniform: odd edge count
-      const int last = __float_as_int(q2.z);
-      if (last >= 0) {                             // uniform: end of an obstacle (H6, H7)
-        const int slot = __float_as_int(q2.w);
-        const float depth = acc.depth();
-        if (MODE & kPerObs) {
-          const float sd = depth >= 0.f ? -depth : sqrtf(minD2);            // eq.(23)
-          if (p.comp) fold.add(__ldg(p.comp + last), sd);
-          else if (n_raw < p.N) p.per_obs[(size_t)n * p.M_rows + last] = sd;
-          if (minD2 < prevD2) { prevD2 = minD2; idD2 = slot; }
-          minD2 = kInf;
-        } else if (MODE & (kGrad | kCoeff)) {
-          if (minD2 < prevD2) { prevD2 = minD2; idD2 = slot; }
-        }
-        if (depth > maxDepth) { maxDepth = depth; idDepth = slot; }
-        acc.reset();
+  // the whole scan in two variants, chosen once per kernel: symmetric footprints (Footprint::sym) take the
+  // edge step that derives the far half of the dot products from the near half (edge_step2_sym)
+  auto scan = [&](auto symc) {
+    constexpr bool SYM = decltype(symc)::value;
+    if (n_tiles > 0) issue(0);
+    for (int t = 0; t < n_tiles; ++t) {
+      if (t + 1 < n_tiles) {
+        issue(t + 1);
+        cp_async_wait<1>();
+      } else {
+        cp_async_wait<0>();
       }
+      __syncthreads();
+      const float4* buf = tile[t & 1];
+      const int cnt = min(kTilePairs, ce - (cb + t * kTilePairs));
+  #pragma unroll 1
+      for (int k = 0; k < cnt; ++k) {
+        const float4 q0 = buf[3 * k];
+        const float4 q1 = buf[3 * k + 1];
+        const float4 q2 = buf[3 * k + 2];
+        edge_step_any<V, true, SYM>(fp, P, q0, q2.x, acc, minD2);
+        if (q2.y >= 0.f) edge_step_any<V, true, SYM>(fp, P, q1, q2.y, acc, minD2);   // uniform: odd edge count
+        const int last = __float_as_int(q2.z);
+        if (last >= 0) {                             // uniform: end of an obstacle (H6, H7)
+          const int slot = __float_as_int(q2.w);
+          const float depth = acc.depth();
+          if (MODE & kPerObs) {
+            const float sd = depth >= 0.f ? -depth : sqrtf(minD2);            // eq.(23)
+            if (p.comp) fold.add(__ldg(p.comp + last), sd);
+            else if (n_raw < p.N) p.per_obs[(size_t)n * p.M_rows + last] = sd;
+            if (minD2 < prevD2) { prevD2 = minD2; idD2 = slot; }
+            minD2 = kInf;
+          } else if (MODE & (kGrad | kCoeff)) {
+            if (minD2 < prevD2) { prevD2 = minD2; idD2 = slot; }
+          }
+          if (depth > maxDepth) { maxDepth = depth; idDepth = slot; }
+          acc.reset();
+        }
+      }
+      __syncthreads();
     }
-    __syncthreads();
-  }
+  };
+  if (V % 4 == 0 && fp.sym) scan(std::true_type{});
+  else scan(std::false_type{});
   if (MODE & kPerObs) {
     minD2 = prevD2;
     if (p.comp) fold.end(p.chunk_group[blockIdx.y + 1]);
@@ -297,8 +305,13 @@ __device__ __forceinline__ void lanes_body(const Footprint& fp, const EvalParams
         src = recs + 3 * (size_t)rec_next;
         q0 = __ldg(src); q1 = __ldg(src + 1); q2 = __ldg(src + 2);
       }
-      edge_step2<V, false>(fp, P, c0, h0, acc, d2);
-      if (h1 >= 0.f) edge_step2<V, false>(fp, P, c1, h1, acc, d2);
+      if (V % 4 == 0 && fp.sym) {                      // (uniform)
+        edge_step_any<V, false, true>(fp, P, c0, h0, acc, d2);
+        if (h1 >= 0.f) edge_step_any<V, false, true>(fp, P, c1, h1, acc, d2);
+      } else {
+        edge_step2<V, false>(fp, P, c0, h0, acc, d2);
+        if (h1 >= 0.f) edge_step2<V, false>(fp, P, c1, h1, acc, d2);
+      }
       if (last >= 0) break;
     }
     const float depth = acc.depth();

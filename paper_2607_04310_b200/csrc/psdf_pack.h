@@ -267,6 +267,14 @@ inline int pack_footprint(const float* fpv, int V, Footprint& fp, int& Vp) {
     fp.cT[l] = (float)(x[a] * tx + y[a] * ty + h);
     fp.ncN[l] = -fp.cN[l]; fp.ncT[l] = -fp.cT[l]; fp.nh[l] = -fp.h[l];
   }
+  // centrally symmetric about the reference point (v_{l+V/2} == -v_l bitwise; no padding vertices; V a
+  // multiple of 4 so that mirrored vertices sit in mirrored f32x2 pairs): the kernels take edge_step2_sym
+  fp.sym = (V == Vp && V % 4 == 0) ? 1 : 0;
+  for (int l = 0; fp.sym && l < V / 2; ++l)
+    if (fpv[2 * (l + V / 2)] != -fpv[2 * l] || fpv[2 * (l + V / 2) + 1] != -fpv[2 * l + 1]) fp.sym = 0;
+  for (int l = 0; fp.sym && l < V / 2; ++l)      // (the derived constants mirror exactly; checked, not assumed)
+    if (fp.tx[l + V / 2] != -fp.tx[l] || fp.ty[l + V / 2] != -fp.ty[l] || fp.h[l + V / 2] != fp.h[l] ||
+        fp.cN[l + V / 2] != fp.cN[l] || fp.cT[l + V / 2] != fp.cT[l]) fp.sym = 0;
   for (int l = 0; l < V; ++l) rmax = std::fmax(rmax, std::hypot((double)fpv[2 * l], (double)fpv[2 * l + 1]));
   fp.rmax = (float)rmax;
   // robot-frame bounding box and the circle around its centre (culled path), rounded up

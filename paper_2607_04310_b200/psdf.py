@@ -30,7 +30,8 @@ EXPORTS = ["psdf_create_scene", "psdf_update_scene", "psdf_eval", "psdf_eval_hos
            "psdf_trajectory_reduce", "psdf_set_components", "psdf_eval_trajectories", "psdf_set_culling", "psdf_destroy_scene", "psdf_scene_num_obstacles",
            "psdf_scene_num_edges", "psdf_last_cuda_error", "psdf_status_string", "psdf_version"]
 # include/psdf_bench.h: measurement instrumentation (bench.py, tests)
-BENCH_EXPORTS = ["psdf_kernel_launches", "psdf_cull_stats", "psdf_measure_fp32_peak", "psdf_bench_host_latency"]
+BENCH_EXPORTS = ["psdf_kernel_launches", "psdf_cull_stats", "psdf_measure_fp32_peak", "psdf_bench_host_latency",
+                 "psdf_scene_footprint_symmetric"]
 
 _lib = None
 
@@ -86,6 +87,8 @@ def lib():
     L.psdf_scene_num_obstacles.argtypes = [vp]
     L.psdf_scene_num_edges.restype = i
     L.psdf_scene_num_edges.argtypes = [vp]
+    L.psdf_scene_footprint_symmetric.restype = i
+    L.psdf_scene_footprint_symmetric.argtypes = [vp]
     L.psdf_last_cuda_error.restype = i
     L.psdf_kernel_launches.restype = ctypes.c_longlong
     L.psdf_status_string.restype = ctypes.c_char_p
@@ -194,6 +197,11 @@ class Scene:
     @property
     def num_obstacles(self):
         return int(lib().psdf_scene_num_obstacles(self._h))
+
+    @property
+    def footprint_symmetric(self):
+        """psdf_scene_footprint_symmetric (include/psdf_bench.h)."""
+        return bool(lib().psdf_scene_footprint_symmetric(self._h))
 
     @property
     def num_edges(self):

@@ -41,6 +41,37 @@ def test_footprint_vertex_counts(env, V):
     scene.close()
 
 
+@pytest.mark.parametrize("V", [4, 8, 12, 16])
+def test_symmetric_footprints_take_the_mirrored_edge_step(env, V):
+    """Footprints that are centrally symmetric about the reference point (v_{l+V/2} == -v_l bitwise) are
+    evaluated by edge_step2_sym (half of the dot products derived from the other half); the same outline
+    with the reference point moved is not.  Both against the oracle, through the lane-split, the
+    tile-scan (chunked) and the culled kernel, which must agree bit for bit with each other."""
+    torch, O, psdf, W = env
+    rng = np.random.default_rng(300 + V)
+    ang = np.sort(rng.uniform(0.05, np.pi - 0.05, V // 2))            # half of a convex outline, then its mirror image
+    half = np.stack([0.8 * np.cos(ang), 0.45 * np.sin(ang)], 1).astype(np.float32)
+    fp_sym = np.concatenate([half, -half]).astype(np.float32)
+    fp_off = (fp_sym + np.float32(0.0625)).astype(np.float32)          # same outline, reference point moved
+    w = W.make_config(3).subsample(6000)
+    for fp, want_sym in ((fp_sym, True), (fp_off, False)):
+        scene = psdf.Scene(fp, w.A, w.B, w.S, max_poses=w.N)
+        assert scene.footprint_symmetric == want_sym
+        ref = O.evaluate(fp, w.A, w.B, w.S, w.poses[:1500], per_obstacle=False)
+        v, g, _ = _run(torch, scene, w.poses, grad=True)                # tile-scan kernel, chunked
+        print(V, want_sym, compare(ref, v[:1500], g[:1500], what=f"V={V} sym={want_sym} scan"))
+        vl, gl, pol = _run(torch, scene, w.poses[:100], grad=True, per_obstacle=True)   # lane-split kernel
+        assert np.array_equal(vl, v[:100]) and np.array_equal(gl, g[:100])
+        refp = O.evaluate(fp, w.A, w.B, w.S, w.poses[:100], per_obstacle=True)
+        compare(refp, vl, gl, pol, what=f"V={V} sym={want_sym} lanes")
+        scene.set_culling(True)
+        vc, gc, _ = _run(torch, scene, w.poses, grad=True)              # culled kernel
+        assert np.array_equal(vc, v) and np.array_equal(gc, g)
+        vh, gh, _ = scene.eval_host(w.poses[:40], grad=True)            # MPC host path
+        assert np.array_equal(vh, v[:40]) and np.array_equal(gh, g[:40])
+        scene.close()
+
+
 def test_empty_and_degenerate_inputs(env):
     torch, O, psdf, W = env
     w = W.make_config(2)
