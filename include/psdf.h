@@ -93,6 +93,21 @@ psdf_status psdf_update_scene(psdf_scene* scene, const float* A, const float* B,
 psdf_status psdf_eval(const psdf_scene* scene, const float* poses, int N, float* value, float* grad,
                       float* per_obstacle, void* cuda_stream);
 
+/* psdf_eval for callers that must not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the chunked tile-scan evaluation with its scratch memory (cross-chunk
+ * keys, arrival counters) in a file-scope static device array of the library, 1.03 MB, which every GPU
+ * that loads the library holds until exit.  Same outputs as psdf_eval (value [N], grad [N,3] or NULL:
+ * bit-identical), no per_obstacle output, no culling.  N > PSDF_STATIC_SCRATCH_MAX_POSES returns
+ * PSDF_ERR_CAPACITY and does nothing.  The call itself enqueues three memsets of the scratch it will use
+ * and one kernel on `cuda_stream`; it calls no cudaMalloc, cudaFree or allocating routine (the scene was
+ * created beforehand; the first call on a device also looks the array's device address up, once).
+ * ALL calls of the process on one GPU share the array, whatever scene they use: two such calls that overlap
+ * on the GPU (different streams without an ordering between them) race and give wrong results; calls
+ * ordered on one stream, or by events, are fine. */
+#define PSDF_STATIC_SCRATCH_MAX_POSES 65536
+psdf_status psdf_eval_static_scratch(const psdf_scene* scene, const float* poses, int N, float* value,
+                                     float* grad, void* cuda_stream);
+
 /* Same semantics with HOST buffers (Alg.1 l.5-11: upload the nominal states,
  * evaluate, bring the results back), on the scene's own stream; returns after synchronising it.
  * MPC-sized batches (N <= 512; with per_obstacle only up to 64 obstacles): ONE kernel launch; up

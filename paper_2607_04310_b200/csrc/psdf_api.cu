@@ -1093,3 +1093,96 @@ psdf_status psdf_measure_fp32_peak(int iters, void* cuda_stream, double* tflops_
 }
 
 }  // extern "C"
+
+// ====================================================================== no-allocation entry point
+// psdf_eval_static_scratch (include/psdf.h): the chunked tile-scan evaluation with its scratch (the
+// cross-chunk arg-max / arg-min keys and the per-tile arrival counters) in a file-scope device array
+// instead of a cudaMalloc'ed workspace.  Every GPU that loads the library holds the array until exit.
+namespace {
+
+constexpr int kStaticMaxPoses = PSDF_STATIC_SCRATCH_MAX_POSES;
+constexpr int kStaticTile = 64;                              // poses per CTA of the tile-scan kernel
+struct StaticScratch {
+  unsigned long long depth[kStaticMaxPoses];                 // must start at 0
+  unsigned long long d2[kStaticMaxPoses];                    // must start at ~0
+  unsigned int count[kStaticMaxPoses / kStaticTile + 64];    // must start at 0
+};
+static __device__ __align__(256) unsigned char g_static_scratch[sizeof(StaticScratch)];   // 1.03 MB
+
+// In host code `g_static_scratch` is a host-side stand-in, not a device address: the address the
+// kernels get comes from cudaGetSymbolAddress, once per device, with that device current.
+constexpr int kMaxDevices = 64;
+std::atomic<StaticScratch*> g_static_ptr[kMaxDevices];
+
+psdf_status static_scratch_ptr(StaticScratch** out) {
+  int dev = 0;
+  CU_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return PSDF_ERR_INVALID_ARG;
+  StaticScratch* ptr = g_static_ptr[dev].load(std::memory_order_acquire);
+  if (!ptr) {
+    void* sym = nullptr;
+    CU_TRY(cudaGetSymbolAddress(&sym, g_static_scratch));   // (allocates nothing; same answer from every thread)
+    if (!sym) return PSDF_ERR_CUDA;
+    ptr = static_cast<StaticScratch*>(sym);
+    g_static_ptr[dev].store(ptr, std::memory_order_release);
+  }
+  *out = ptr;
+  return PSDF_OK;
+}
+
+}  // namespace
+
+extern "C" psdf_status psdf_eval_static_scratch(const psdf_scene* sc, const float* poses, int N, float* value,
+                                                float* grad, void* cuda_stream) {
+  if (!sc || N < 0 || (N > 0 && (!poses || !value))) return PSDF_ERR_INVALID_ARG;
+  if (N > kStaticMaxPoses) return PSDF_ERR_CAPACITY;         // beyond the static array: rejected, nothing done
+  if (N == 0) return PSDF_OK;
+  PSDF_ENTER(sc);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  StaticScratch* ss = nullptr;
+  psdf_status s = static_scratch_ptr(&ss);
+  if (s != PSDF_OK) return s;
+  note_eval_stream(sc, st);
+  const int tiles = (N + kStaticTile - 1) / kStaticTile;
+  // the array is shared by every call and keeps the last call's contents (a call that failed or was
+  // overlapped may have left keys behind): what this call uses is put into its clean state first
+  CU_TRY(cudaMemsetAsync(ss->depth, 0x00, sizeof(unsigned long long) * (size_t)N, st));
+  CU_TRY(cudaMemsetAsync(ss->d2, 0xff, sizeof(unsigned long long) * (size_t)N, st));
+  CU_TRY(cudaMemsetAsync(ss->count, 0x00, sizeof(unsigned int) * (size_t)tiles, st));
+  EvalParams p{};
+  p.pairs = sc->pk[sc->cur].pairs;
+  p.row_slot = sc->pk[sc->cur].row_slot;
+  p.bounds = sc->pk[sc->cur].bounds;
+  p.empty_rows = sc->pk[sc->cur].empty;
+  p.poses = poses;
+  p.value = value;
+  p.grad = grad;
+  p.ws_depth = ss->depth;                                    // device addresses inside the static array
+  p.ws_d2 = ss->d2;
+  p.ws_count = ss->count;
+  p.n_edges = sc->n_edges;
+  p.Mv = sc->Mv;
+  p.M_rows = sc->M;
+  p.n_empty = sc->n_empty;
+  p.N = N;
+  // the tile-scan kernel's launch plan, always in chunks when the scene allows it
+  int C = 2;
+  const double warps_per_sm = (double)N / 32.0 / sc->sm_count;
+  if (warps_per_sm < 256.0) C = (int)std::ceil(256.0 / warps_per_sm);
+  const int maxC = sc->Mv / 16 > 0 ? sc->Mv / 16 : 1;
+  if (C < 2) C = 2;
+  if (C > maxC) C = maxC;
+  if (C > kMaxChunks) C = kMaxChunks;
+  p.chunk_begin[0] = 0;
+  int o = 0;
+  for (int c = 1; c < C; ++c) {
+    const long long target = (long long)sc->n_pairs * c / C;
+    while (o < sc->Mv && sc->h_pair_begin[o] < target) ++o;
+    p.chunk_begin[c] = sc->h_pair_begin[o];
+  }
+  p.chunk_begin[C] = sc->n_pairs;
+  p.n_chunks = C;
+  const cudaError_t e = launch_v(sc, p, grad ? kGrad : 0, false, dim3((unsigned)tiles, (unsigned)C), kStaticTile, st, nullptr);
+  if (e != cudaSuccess) return cuda_failed(e);
+  return PSDF_OK;
+}

@@ -21,11 +21,12 @@ PSDF_ERR_CAPACITY = -3
 PSDF_ERR_CUDA = -4
 PSDF_ERR_ALLOC = -5
 PSDF_ERR_BUSY = -6
+STATIC_SCRATCH_MAX_POSES = 65536      # PSDF_STATIC_SCRATCH_MAX_POSES of include/psdf.h
 PSDF_MEM_HOST = 0
 PSDF_MEM_DEVICE = 1
 
 # include/psdf.h: the product ABI
-EXPORTS = ["psdf_create_scene", "psdf_update_scene", "psdf_eval", "psdf_eval_host",
+EXPORTS = ["psdf_create_scene", "psdf_update_scene", "psdf_eval", "psdf_eval_static_scratch", "psdf_eval_host",
            "psdf_eval_windows", "psdf_eval_windows_host", "psdf_mpc_coeffs_host", "psdf_component_min",
            "psdf_trajectory_reduce", "psdf_set_components", "psdf_eval_trajectories", "psdf_set_culling", "psdf_destroy_scene", "psdf_scene_num_obstacles",
            "psdf_scene_num_edges", "psdf_last_cuda_error", "psdf_status_string", "psdf_version"]
@@ -61,6 +62,8 @@ def lib():
     L.psdf_update_scene.argtypes = [vp, fp_, fp_, u8p, i, vp]
     L.psdf_eval.restype = i
     L.psdf_eval.argtypes = [vp, fp_, i, fp_, fp_, fp_, vp]
+    L.psdf_eval_static_scratch.restype = i
+    L.psdf_eval_static_scratch.argtypes = [vp, fp_, i, fp_, fp_, vp]
     L.psdf_eval_host.restype = i
     L.psdf_eval_host.argtypes = [vp, fp_, i, fp_, fp_, fp_]
     L.psdf_eval_windows.restype = i
@@ -276,6 +279,22 @@ class Scene:
         _check(lib().psdf_eval(self._h, pp, N, _dev_ptr(value, "float32"), pg, po, _stream_ptr(stream)),
                "psdf_eval")
         return value, (grad if want_g else None), (per_obstacle if want_po else None)
+
+    def eval_static_scratch(self, poses, value=None, grad=True, stream=None):
+        """psdf_eval_static_scratch: psdf_eval without any allocation inside the library (scratch in a
+        static device array; N <= STATIC_SCRATCH_MAX_POSES).  Preallocated `value` / `grad` tensors may be
+        passed so that the binding allocates nothing either."""
+        import torch
+        N = int(poses.shape[0])
+        if value is None:
+            value = torch.empty(N, dtype=torch.float32, device=poses.device)
+        if grad is True:
+            grad = torch.empty((N, 3), dtype=torch.float32, device=poses.device)
+        want_g = grad is not False and grad is not None
+        _check(lib().psdf_eval_static_scratch(self._h, _dev_ptr(poses, "float32"), N, _dev_ptr(value, "float32"),
+                                              _dev_ptr(grad, "float32") if want_g else None, _stream_ptr(stream)),
+               "psdf_eval_static_scratch")
+        return value, (grad if want_g else None)
 
     def eval_host(self, poses, grad=True, per_obstacle=False):
         """psdf_eval_host on numpy arrays (CUDA-graph replay, returns after sync)."""
