@@ -158,6 +158,23 @@ def mpc_latency(torch, psdf, replays=2000):
         out["c_abi_clock"] = _pct(inlib)
         return out
 
+    def serve_lat(scene, w, n_rep, coeffs=None):
+        """psdf_serve_step (persistent kernel + mapped-memory mailbox): same clocks as host_lat."""
+        scene.serve_begin(w.N, coeffs=coeffs, idle_timeout_ms=200)
+        rows = np.empty((w.N, 4), np.float32)
+        call = scene.bind_serve_step(w.poses, rows)
+        for _ in range(500):
+            call()
+        ts = []
+        for _ in range(n_rep):
+            t0 = time.perf_counter_ns()
+            call()
+            ts.append((time.perf_counter_ns() - t0) * 1e-3)
+        out = _pct(ts)
+        out["c_abi_clock"] = _pct(scene.bench_serve_latency(w.poses, n_rep))
+        scene.serve_end()
+        return out
+
     def kernel_lat(scene, w, n_rep=300, per_obs=False):
         poses = torch.from_numpy(w.poses).cuda()
         value = torch.empty(w.N, dtype=torch.float32, device="cuda")
@@ -183,18 +200,25 @@ def mpc_latency(torch, psdf, replays=2000):
         if idx == 1:
             e["eval_host_value_grad_marshalled_per_call"] = host_lat(scene, w, replays, bound=False)
             e["mpc_coeffs_host"] = host_lat(scene, w, replays, coeffs=True)
+            e["serve_step_mpc_coeffs"] = serve_lat(scene, w, replays, coeffs=(0.3, 0.05, 0.05))
         else:
             e["eval_host_value_grad_per_obstacle"] = host_lat(scene, w, replays, per_obs=True)
+        e["serve_step_value_grad"] = serve_lat(scene, w, replays)
         out[w.name] = e
         scene.close()
-    t1 = {}
+    t1, t1s = {}, {}
     for M in (1, 10, 100):
         for B in (1, 15, 100):
             w = W.table1_case(M, B)
             scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=w.N)
             t1[f"M{M}_B{B}"] = host_lat(scene, w, 500)["p50_us"]
+            t1s[f"M{M}_B{B}"] = serve_lat(scene, w, 500)["p50_us"]
             scene.close()
     out["table1_shapes_eval_host_p50_us"] = t1
+    out["table1_shapes_serve_step_p50_us"] = t1s
+    out["serve_step"] = ("psdf_serve_begin / psdf_serve_step: persistent lane-split kernel polling a mailbox in pinned, "
+                         "device-mapped memory; no launch and no stream synchronisation per control cycle; rows "
+                         "bit-identical to psdf_eval_host / psdf_mpc_coeffs_host (tests/test_gpu_serve.py)")
     out["table1_paper_rtx4090_ms"] = {"M1_B1": 1.981, "M1_B15": 2.154, "M1_B100": 2.212, "M10_B1": 2.152,
                                       "M10_B15": 2.213, "M10_B100": 2.250, "M100_B1": 2.221, "M100_B15": 2.222,
                                       "M100_B100": 2.207,

@@ -120,6 +120,30 @@ psdf_status psdf_eval_static_scratch(const psdf_scene* scene, const float* poses
 psdf_status psdf_eval_host(psdf_scene* scene, const float* poses, int N, float* value, float* grad,
                            float* per_obstacle);
 
+/* Serving mode for one fixed MPC batch shape (Alg.1 l.5-11: every control cycle uploads
+ * the N nominal states and brings N coefficient rows back; N = 15 in the paper): a PERSISTENT
+ * kernel and a mailbox in pinned, device-mapped memory, so that a cycle costs neither a kernel launch nor a
+ * stream synchronisation.
+ *   psdf_serve_begin   starts the kernel on a stream of its own for batches of exactly N poses
+ *                      (N <= 512 and at most 64 pose groups, else PSDF_ERR_INVALID_ARG: use psdf_eval_host);
+ *                      want_coeffs = 0: rows (phi, d phi/dx, d phi/dy, d phi/dtheta) as psdf_eval_host;
+ *                      want_coeffs = 1: rows [h - gamma ; J_g] as psdf_mpc_coeffs_host with d_min, rho_p,
+ *                      rho_theta.  idle_timeout_ms in [1, 10000]: a kernel that sees no request for that
+ *                      long exits by itself (the next step starts it again, at the cost of one launch).
+ *   psdf_serve_step    poses host [N,3] -> out host [N,4]; posts the poses, spins until every CTA has
+ *                      acknowledged, copies the rows out.  Results are bit-identical to psdf_eval_host /
+ *                      psdf_mpc_coeffs_host.  Ordinary host memory is fine (N is small).
+ *   psdf_serve_end     stops the kernel (psdf_destroy_scene does it too).
+ * While the kernel runs it occupies a few CTAs and polls host memory over PCIe; a device-wide
+ * synchronisation (cudaDeviceSynchronize, cudaFree) issued meanwhile waits until it exits, i.e. until
+ * psdf_serve_end or the idle time-out.  psdf_update_scene, psdf_set_culling and psdf_set_components stop it
+ * themselves and the next psdf_serve_step restarts it on the new scene; every other call of this header may
+ * be used next to it.  Allocates pinned memory in psdf_serve_begin only. */
+psdf_status psdf_serve_begin(psdf_scene* scene, int N, int want_coeffs, float d_min, float rho_p, float rho_theta,
+                             int idle_timeout_ms);
+psdf_status psdf_serve_step(psdf_scene* scene, const float* poses, float* out);
+psdf_status psdf_serve_end(psdf_scene* scene);
+
 /* Time-varying environments ("batching {(x_{k+s}, E_{k+s})} instead"): the scene
  * holds the rows of all stage-wise edge sets one after another (e.g. M = H * M_stage rows) and
  * pose n is evaluated against the obstacle ROWS row_window[2n] <= i < row_window[2n+1] only

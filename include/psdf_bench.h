@@ -34,6 +34,10 @@ psdf_status psdf_bench_host_latency(psdf_scene* scene, const float* poses, int N
                                     float* per_obstacle, float* coeff, float d_min, float rho_p, float rho_theta,
                                     int reps, double* out_us);
 
+/* The same for psdf_serve_step (serving mode begun by psdf_serve_begin): `reps` steps on the same poses,
+ * one duration in microseconds per step. */
+psdf_status psdf_bench_serve_latency(psdf_scene* scene, const float* poses, float* out, int reps, double* out_us);
+
 /* FP32 FMA-only micro-kernel: achieved TFLOP/s on the current device (bench.py reports it beside
  * the nominal FP32 peak, MEASURED_PEAKS.json holding no FP32 figure). */
 psdf_status psdf_measure_fp32_peak(int iters, void* cuda_stream, double* tflops_out);

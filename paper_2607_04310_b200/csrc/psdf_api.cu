@@ -4,6 +4,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <new>
+#include <immintrin.h>
 
 #include "../../include/psdf.h"
 #include "../../include/psdf_bench.h"
@@ -124,7 +125,22 @@ struct psdf_scene {
   PoseArgs h_args;                    // the MPC host path's poses (N <= kArgPoses)
   GraphEntry graphs[kGraphCache];
   unsigned long long stamp = 0;
+  // serving mode (psdf_serve_begin): persistent kernel on its own stream, mailbox in mapped memory
+  struct Serve {
+    bool on = false, running = false;
+    int N = 0, mode = 0, K = 0, G = 0, bd = 0;
+    float d_min = 0.f, rho_p = 0.f, rho_theta = 0.f;
+    unsigned seq = 1;
+    unsigned long long idle_ns = 0;
+    cudaStream_t stream = nullptr;
+    float4* in = nullptr;               // mapped [N]   (x, y, theta, sequence number)
+    float4* out = nullptr;              // mapped [N]   (value, grad) or coefficient rows
+    unsigned* ack = nullptr;            // mapped [2 G] (served sequence number, exited flag) per CTA
+    int cap_N = 0, cap_G = 0;
+  } srv;
 };
+
+static psdf_status serve_pause(psdf_scene* sc);   // stops the serving kernel (it holds scene pointers by value)
 
 namespace {
 
@@ -494,6 +510,11 @@ extern "C" {
 
 void psdf_destroy_scene(psdf_scene* sc) {
   if (!sc) return;
+  (void)serve_pause(sc);
+  if (sc->srv.stream) cudaStreamDestroy(sc->srv.stream);
+  if (sc->srv.in) cudaFreeHost(sc->srv.in);
+  if (sc->srv.out) cudaFreeHost(sc->srv.out);
+  if (sc->srv.ack) cudaFreeHost(sc->srv.ack);
   for (auto& g : sc->graphs)
     if (g.exec) cudaGraphExecDestroy(g.exec);
   if (sc->gstream) cudaStreamDestroy(sc->gstream);
@@ -606,6 +627,7 @@ psdf_status psdf_update_scene(psdf_scene* sc, const float* A, const float* B, co
   // both paths validate before anything live changes (host: pack_scene; device: status word
   // checked before the buffer flip), so a bad update leaves the old scene in force
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  { const psdf_status sp = serve_pause(sc); if (sp != PSDF_OK) return sp; }   // (relaunched by the next psdf_serve_step)
   if (sc->gstream) CU_TRY(cudaStreamSynchronize(sc->gstream));
   psdf_status s = upload_scene(sc, A, B, S, where, st);
   if (s != PSDF_OK) return s;
@@ -940,6 +962,7 @@ psdf_status psdf_eval_windows_host(psdf_scene* sc, const float* poses, int N, co
 psdf_status psdf_set_culling(psdf_scene* sc, int enable) {
   if (!sc) return PSDF_ERR_INVALID_ARG;
   PSDF_ENTER(sc);
+  { const psdf_status sp = serve_pause(sc); if (sp != PSDF_OK) return sp; }
   if (sc->gstream) CU_TRY(cudaStreamSynchronize(sc->gstream));
   if (enable && !sc->pk[sc->cur].grid_ok) {      // built here, then kept current by every update
     CU_TRY(launch_grid(sc, sc->cur, nullptr, sc->Mv, sc->n_pairs, (cudaStream_t)0));
@@ -960,6 +983,7 @@ psdf_status psdf_set_components(psdf_scene* sc, const int* comp_to_obstacle, int
       if (comp_to_obstacle[i] < 0 || comp_to_obstacle[i] >= n_obstacles || (i > 0 && comp_to_obstacle[i] < comp_to_obstacle[i - 1]))
         return PSDF_ERR_INVALID_ARG;                  // components of one obstacle are consecutive rows
   }
+  { const psdf_status sp = serve_pause(sc); if (sp != PSDF_OK) return sp; }   // (cudaDeviceSynchronize below)
   if (sc->gstream) CU_TRY(cudaStreamSynchronize(sc->gstream));
   drop_graphs(sc);
   if (n_obstacles == 0) { sc->n_groups = 0; return PSDF_OK; }
@@ -1186,3 +1210,197 @@ extern "C" psdf_status psdf_eval_static_scratch(const psdf_scene* sc, const floa
   if (e != cudaSuccess) return cuda_failed(e);
   return PSDF_OK;
 }
+
+// ============================================================================== serving mode
+// psdf_serve_begin / psdf_serve_step / psdf_serve_end (include/psdf.h): a persistent kernel and a mailbox
+// in pinned, device-mapped memory for one fixed MPC batch shape (psdf_serve_kernel, psdf_kernels.cuh).
+namespace {
+
+constexpr int kServeMaxPoses = 512, kServeMaxCtas = 128;
+
+template <int V>
+cudaError_t launch_serve_v(const psdf_scene* sc, const EvalParams& p, unsigned last_seq) {
+  const psdf_scene::Serve& sv = sc->srv;
+  if (sv.mode & kCoeff)
+    psdf_serve_kernel<V, kCoeff><<<sv.G, sv.bd, 0, sv.stream>>>(sc->fp, p, sv.in, sv.ack, last_seq, sv.idle_ns);
+  else
+    psdf_serve_kernel<V, kGrad><<<sv.G, sv.bd, 0, sv.stream>>>(sc->fp, p, sv.in, sv.ack, last_seq, sv.idle_ns);
+  g_launches.fetch_add(1);
+  return cudaGetLastError();
+}
+
+// (re)launches the serving kernel on the live buffer set; `last_seq`: the request it must NOT answer
+psdf_status serve_launch(psdf_scene* sc, unsigned last_seq) {
+  psdf_scene::Serve& sv = sc->srv;
+  EvalParams p{};
+  p.pairs = sc->pk[sc->cur].pairs;
+  p.row_slot = sc->pk[sc->cur].row_slot;
+  p.bounds = sc->pk[sc->cur].bounds;
+  p.empty_rows = sc->pk[sc->cur].empty;
+  float* rows = reinterpret_cast<float*>(sv.out);            // mapped host rows
+  p.grad = (sv.mode & kGrad) ? rows : nullptr;               // (non-null = wanted; results go to `packed`)
+  p.coeff = (sv.mode & kCoeff) ? rows : nullptr;
+  p.packed = rows;
+  p.n_edges = sc->n_edges;
+  p.Mv = sc->Mv;
+  p.M_rows = sc->M;
+  p.n_empty = sc->n_empty;
+  p.N = sv.N;
+  p.lanes = sv.K;
+  p.n_chunks = 1;
+  p.d_min = sv.d_min; p.rho_p = sv.rho_p; p.rho_theta = sv.rho_theta;
+  for (int c = 0; c < sv.G; ++c) { sv.ack[2 * c] = last_seq; sv.ack[2 * c + 1] = 0u; }
+  cudaError_t e;
+  switch (sc->Vp) {
+    case 4: e = launch_serve_v<4>(sc, p, last_seq); break;
+    case 6: e = launch_serve_v<6>(sc, p, last_seq); break;
+    case 8: e = launch_serve_v<8>(sc, p, last_seq); break;
+    case 10: e = launch_serve_v<10>(sc, p, last_seq); break;
+    case 12: e = launch_serve_v<12>(sc, p, last_seq); break;
+    case 16: e = launch_serve_v<16>(sc, p, last_seq); break;
+    default: e = cudaErrorInvalidValue;
+  }
+  if (e != cudaSuccess) return cuda_failed(e);
+  sv.running = true;
+  return PSDF_OK;
+}
+
+inline void serve_post(psdf_scene::Serve& sv, int n, float x, float y, float th, unsigned seq) {
+  // one 16-byte store per slot: the polling lane sees either the old or the new request, never a mix
+  const __m128i v = _mm_set_epi32((int)seq, (int)__builtin_bit_cast(unsigned, th), (int)__builtin_bit_cast(unsigned, y),
+                                  (int)__builtin_bit_cast(unsigned, x));
+  _mm_store_si128(reinterpret_cast<__m128i*>(sv.in + n), v);
+}
+
+}  // namespace
+
+static psdf_status serve_pause(psdf_scene* sc) {
+  psdf_scene::Serve& sv = sc->srv;
+  if (!sv.running) return PSDF_OK;
+  for (int n = 0; n < sv.N; ++n) serve_post(sv, n, 0.f, 0.f, 0.f, kServeExit);
+  _mm_sfence();
+  sv.running = false;
+  CU_TRY(cudaStreamSynchronize(sv.stream));           // (at the latest after the idle timeout)
+  return PSDF_OK;
+}
+
+extern "C" {
+
+psdf_status psdf_serve_begin(psdf_scene* sc, int N, int want_coeffs, float d_min, float rho_p, float rho_theta,
+                             int idle_timeout_ms) {
+  if (!sc || N < 1 || N > kServeMaxPoses || idle_timeout_ms < 1 || idle_timeout_ms > 10000) return PSDF_ERR_INVALID_ARG;
+  if (N > sc->max_poses) return PSDF_ERR_CAPACITY;
+  PSDF_ENTER(sc);
+  psdf_status s = serve_pause(sc);
+  if (s != PSDF_OK) return s;
+  psdf_scene::Serve& sv = sc->srv;
+  sv.on = false;
+  // lanes per pose as in the lane-split plan, all inside one CTA per pose group (no cross-CTA reduction)
+  long long want = (long long)sc->sm_count * 1024 / N;
+  int L = 1;
+  // (fewer, fatter CTAs were measured and are far slower: ~1.7 us of dependent L2 round trips per obstacle and lane)
+  while (L < 256 && L < sc->Mv && L * 2 <= want) L <<= 1;
+  const int K = L, bd = K <= 64 ? 64 : K, ppc = bd / K, G = (N + ppc - 1) / ppc;
+  if (G > kServeMaxCtas) return PSDF_ERR_INVALID_ARG;       // not an MPC-sized shape: use psdf_eval_host
+  if (!sv.stream) CU_TRY(cudaStreamCreateWithFlags(&sv.stream, cudaStreamNonBlocking));
+  if (N > sv.cap_N || G > sv.cap_G) {
+    if (sv.in) cudaFreeHost(sv.in);
+    if (sv.out) cudaFreeHost(sv.out);
+    if (sv.ack) cudaFreeHost(sv.ack);
+    sv.in = sv.out = nullptr; sv.ack = nullptr; sv.cap_N = sv.cap_G = 0;
+    CU_TRY(cudaHostAlloc(&sv.in, sizeof(float4) * (size_t)N, cudaHostAllocMapped));
+    CU_TRY(cudaHostAlloc(&sv.out, sizeof(float4) * (size_t)N, cudaHostAllocMapped));
+    CU_TRY(cudaHostAlloc(&sv.ack, sizeof(unsigned) * 2 * (size_t)G, cudaHostAllocMapped));
+    sv.cap_N = N; sv.cap_G = G;
+  }
+  int dev = 0, uva = 0;
+  CU_TRY(cudaGetDevice(&dev));
+  CU_TRY(cudaDeviceGetAttribute(&uva, cudaDevAttrUnifiedAddressing, dev));
+  if (!uva) return PSDF_ERR_CUDA;                            // (mapped host pointers are used as device pointers)
+  sv.N = N; sv.K = K; sv.bd = bd; sv.G = G;
+  sv.mode = want_coeffs ? kCoeff : kGrad;
+  sv.d_min = d_min; sv.rho_p = rho_p; sv.rho_theta = rho_theta;
+  sv.idle_ns = (unsigned long long)idle_timeout_ms * 1000000ull;
+  sv.seq = 1;
+  for (int n = 0; n < N; ++n) serve_post(sv, n, 0.f, 0.f, 0.f, sv.seq);
+  _mm_sfence();
+  s = serve_launch(sc, sv.seq);
+  if (s != PSDF_OK) return s;
+  sv.on = true;
+  return PSDF_OK;
+}
+
+psdf_status psdf_serve_step(psdf_scene* sc, const float* poses, float* out) {
+  if (!sc || !poses || !out) return PSDF_ERR_INVALID_ARG;
+  PSDF_ENTER(sc);
+  psdf_scene::Serve& sv = sc->srv;
+  if (!sv.on) return PSDF_ERR_INVALID_ARG;                   // psdf_serve_begin first
+  unsigned seq = sv.seq + 1;
+  if (seq == kServeExit || seq == 0u) seq = 1u;
+  const unsigned prev = sv.seq;
+  sv.seq = seq;
+  for (int n = 0; n < sv.N; ++n) serve_post(sv, n, poses[3 * n], poses[3 * n + 1], poses[3 * n + 2], seq);
+  _mm_sfence();
+  if (!sv.running) {                                         // paused by an update, or first step after a time-out
+    const psdf_status s = serve_launch(sc, prev);
+    if (s != PSDF_OK) return s;
+  }
+  volatile unsigned* ack = sv.ack;
+  const auto t0 = std::chrono::steady_clock::now();
+  int relaunches = 0;
+  for (int c = 0; c < sv.G;) {
+    unsigned spins = 0;
+    bool restart = false;
+    while (ack[2 * c] != seq) {
+      _mm_pause();
+      if ((++spins & 0x3fu) != 0u) continue;
+      for (int k = 0; k < sv.G && !restart; ++k) restart = ack[2 * k + 1] != 0u;   // a CTA gave up (idle time-out)
+      if (restart) break;
+      if ((spins & 0xfffu) == 0u) {
+        if (cudaStreamQuery(sv.stream) != cudaErrorNotReady) {   // kernel gone without a word: an error
+          sv.running = false;
+          const cudaError_t e = cudaGetLastError();
+          return cuda_failed(e != cudaSuccess ? e : cudaErrorUnknown);
+        }
+        if (std::chrono::steady_clock::now() - t0 > std::chrono::seconds(5)) return PSDF_ERR_CUDA;
+      }
+    }
+    if (restart) {
+      // the kernel is on its way out: hurry the CTAs that are still polling, then every CTA answers the
+      // request again on a fresh launch (requests are idempotent)
+      psdf_status s = serve_pause(sc);
+      if (s != PSDF_OK) return s;
+      if (++relaunches > 3) return PSDF_ERR_CUDA;
+      for (int n = 0; n < sv.N; ++n) serve_post(sv, n, poses[3 * n], poses[3 * n + 1], poses[3 * n + 2], seq);
+      _mm_sfence();
+      s = serve_launch(sc, prev);
+      if (s != PSDF_OK) return s;
+      c = 0;
+      continue;
+    }
+    ++c;
+  }
+  std::memcpy(out, sv.out, sizeof(float4) * (size_t)sv.N);
+  return PSDF_OK;
+}
+
+psdf_status psdf_serve_end(psdf_scene* sc) {
+  if (!sc) return PSDF_ERR_INVALID_ARG;
+  PSDF_ENTER(sc);
+  sc->srv.on = false;
+  return serve_pause(sc);
+}
+
+psdf_status psdf_bench_serve_latency(psdf_scene* sc, const float* poses, float* out, int reps, double* out_us) {
+  if (!sc || !out_us || reps < 1) return PSDF_ERR_INVALID_ARG;
+  for (int r = 0; r < reps; ++r) {
+    const auto t0 = std::chrono::steady_clock::now();
+    const psdf_status s = psdf_serve_step(sc, poses, out);
+    const auto t1 = std::chrono::steady_clock::now();
+    if (s != PSDF_OK) return s;
+    out_us[r] = std::chrono::duration<double, std::micro>(t1 - t0).count();
+  }
+  return PSDF_OK;
+}
+
+}  // extern "C"

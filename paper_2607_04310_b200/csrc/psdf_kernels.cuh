@@ -382,6 +382,76 @@ __global__ void __launch_bounds__(256) psdf_lanes_args_kernel(const __grid_const
   lanes_body<V, MODE, true>(fp, p, a.q);
 }
 
+// ------------------------------------------------------------------------------------------
+// Serving kernel (psdf_serve_begin / psdf_serve_step, include/psdf.h): the lane-split evaluation as a
+// PERSISTENT kernel for one fixed MPC batch shape.  A control cycle then costs neither a kernel launch
+// nor a stream synchronisation: the host posts the N nominal states into pinned, device-mapped memory
+// (one 16-byte slot per pose: x, y, theta and the request's sequence number in the fourth word, stored
+// with one 16-byte store), the leader lane of every pose group polls ITS slot over PCIe, so the flag and
+// the data arrive in the same read, the CTA evaluates (lanes_body, poses handed over through shared
+// memory), writes one float4 per pose (value, gradient; or the coefficient row) back to mapped memory,
+// fences, and raises its acknowledgement word, on which the host spins.
+// Lifetime is bounded: a CTA that sees no request for `idle_ns` (or the exit code) marks itself exited
+// and returns; the host relaunches on the next step (requests are idempotent).
+constexpr unsigned kServeExit = 0xffffffffu;
+
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+__device__ __forceinline__ float4 ld_volatile_f4(const float4* ptr) {
+  float4 v;
+  asm volatile("ld.volatile.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(ptr));
+  return v;
+}
+
+// ack: mapped [2 * gridDim.x] = per CTA (last sequence number served, exited flag).  Only the lanes that wrote
+// a row fence at system scope before the CTA's acknowledgement (a fence by every thread cost 3-4 us on shapes
+// with many CTAs; collecting the rows on the device and letting the last CTA write them out was slower still).
+template <int V, int MODE>
+__global__ void __launch_bounds__(256) psdf_serve_kernel(const __grid_constant__ Footprint fp,
+                                                         const __grid_constant__ EvalParams p,
+                                                         const float4* __restrict__ in, volatile unsigned* ack,
+                                                         unsigned last_seq, unsigned long long idle_ns) {
+  __shared__ float4 s_pose[256];
+  __shared__ int s_exit;
+  const int K = p.lanes, ppc = blockDim.x / K;
+  const int g = threadIdx.x / K, lane = threadIdx.x % K;
+  const int n_raw = blockIdx.x * ppc + g;
+  unsigned last = last_seq;
+  if (threadIdx.x == 0) s_exit = 0;
+  __syncthreads();
+  unsigned long long t_idle = global_timer_ns();
+  while (true) {
+    if (lane == 0 && n_raw < p.N) {                  // leader of a pose group: wait for this pose's slot
+      float4 q;
+      unsigned s;
+      while (true) {
+        q = ld_volatile_f4(in + n_raw);
+        s = __float_as_uint(q.w);
+        if (s != last) break;                          // the next request (or the exit code)
+        if (*(volatile int*)&s_exit) break;
+        if (global_timer_ns() - t_idle > idle_ns) { *(volatile int*)&s_exit = 1; break; }
+      }
+      s_pose[g] = q;
+      if (s == kServeExit) *(volatile int*)&s_exit = 1;
+    }
+    __syncthreads();
+    if (s_exit) {                                      // (uniform: read after the barrier)
+      if (threadIdx.x == 0) { ack[2 * blockIdx.x + 1] = 1u; __threadfence_system(); }
+      return;
+    }
+    const unsigned seq = __float_as_uint(s_pose[0].w); // (group 0 of a CTA always owns a pose)
+    lanes_body<V, MODE, true>(fp, p, s_pose - (size_t)blockIdx.x * ppc);   // rows -> p.packed / p.coeff
+    if (lane == 0) __threadfence_system();             // this group's row before the acknowledgement
+    __syncthreads();
+    if (threadIdx.x == 0) ack[2 * blockIdx.x] = seq;
+    last = seq;
+    t_idle = global_timer_ns();
+  }
+}
+
 // FP32 FMA-only micro-kernel for the measured roofline denominator (bench.py).
 __global__ void fp32_peak_kernel(float* out, int iters, float a, float b) {
   float acc[16];

@@ -27,12 +27,13 @@ PSDF_MEM_DEVICE = 1
 
 # include/psdf.h: the product ABI
 EXPORTS = ["psdf_create_scene", "psdf_update_scene", "psdf_eval", "psdf_eval_static_scratch", "psdf_eval_host",
-           "psdf_eval_windows", "psdf_eval_windows_host", "psdf_mpc_coeffs_host", "psdf_component_min",
+           "psdf_eval_windows", "psdf_eval_windows_host", "psdf_mpc_coeffs_host", "psdf_serve_begin", "psdf_serve_step",
+           "psdf_serve_end", "psdf_component_min",
            "psdf_trajectory_reduce", "psdf_set_components", "psdf_eval_trajectories", "psdf_set_culling", "psdf_destroy_scene", "psdf_scene_num_obstacles",
            "psdf_scene_num_edges", "psdf_last_cuda_error", "psdf_status_string", "psdf_version"]
 # include/psdf_bench.h: measurement instrumentation (bench.py, tests)
 BENCH_EXPORTS = ["psdf_kernel_launches", "psdf_cull_stats", "psdf_measure_fp32_peak", "psdf_bench_host_latency",
-                 "psdf_scene_footprint_symmetric"]
+                 "psdf_scene_footprint_symmetric", "psdf_bench_serve_latency"]
 
 _lib = None
 
@@ -72,6 +73,14 @@ def lib():
     L.psdf_eval_windows_host.argtypes = [vp, fp_, i, vp, fp_, fp_]
     L.psdf_mpc_coeffs_host.restype = i
     L.psdf_mpc_coeffs_host.argtypes = [vp, fp_, i, ctypes.c_float, ctypes.c_float, ctypes.c_float, fp_]
+    L.psdf_serve_begin.restype = i
+    L.psdf_serve_begin.argtypes = [vp, i, i, ctypes.c_float, ctypes.c_float, ctypes.c_float, i]
+    L.psdf_serve_step.restype = i
+    L.psdf_serve_step.argtypes = [vp, fp_, fp_]
+    L.psdf_serve_end.restype = i
+    L.psdf_serve_end.argtypes = [vp]
+    L.psdf_bench_serve_latency.restype = i
+    L.psdf_bench_serve_latency.argtypes = [vp, fp_, fp_, i, ctypes.POINTER(ctypes.c_double)]
     L.psdf_set_components.restype = i
     L.psdf_set_components.argtypes = [vp, vp, i]
     L.psdf_eval_trajectories.restype = i
@@ -394,6 +403,46 @@ class Scene:
                                              po.ctypes.data if po is not None else None,
                                              c.ctypes.data if c is not None else None, float(d_min), float(rho_p),
                                              float(rho_theta), int(reps), out), "psdf_bench_host_latency")
+        return np.frombuffer(out, dtype=np.float64).copy()
+
+    def serve_begin(self, N, coeffs=None, idle_timeout_ms=200):
+        """psdf_serve_begin: persistent-kernel serving of batches of exactly N poses; coeffs = (d_min, rho_p,
+        rho_theta) for MPC coefficient rows, None for (value, grad) rows."""
+        d_min, rho_p, rho_theta = coeffs if coeffs else (0.0, 0.0, 0.0)
+        _check(lib().psdf_serve_begin(self._h, int(N), 1 if coeffs else 0, float(d_min), float(rho_p), float(rho_theta),
+                                      int(idle_timeout_ms)), "psdf_serve_begin")
+        self._serve_N = int(N)
+
+    def serve_step(self, poses, out=None):
+        """psdf_serve_step: host poses [N,3] -> host rows [N,4]."""
+        poses, pp = _host(poses, np.float32)
+        assert poses.shape == (self._serve_N, 3)
+        if out is None:
+            out = np.empty((self._serve_N, 4), np.float32)
+        _check(lib().psdf_serve_step(self._h, pp, out.ctypes.data), "psdf_serve_step")
+        return out
+
+    def bind_serve_step(self, poses, out):
+        """psdf_serve_step pre-marshalled (as bind_eval_host): zero-argument callable over fixed float32 arrays."""
+        assert poses.dtype == np.float32 and poses.flags.c_contiguous and poses.shape == (self._serve_N, 3)
+        assert out.dtype == np.float32 and out.flags.c_contiguous and out.shape == (self._serve_N, 4)
+        fn, args, keep = lib().psdf_serve_step, (self._h, poses.ctypes.data, out.ctypes.data), (poses, out)
+
+        def call(_keep=keep):
+            status = fn(*args)
+            if status != PSDF_OK:
+                raise PsdfError(status, "psdf_serve_step")
+        return call
+
+    def serve_end(self):
+        _check(lib().psdf_serve_end(self._h), "psdf_serve_end")
+
+    def bench_serve_latency(self, poses, reps):
+        """psdf_bench_serve_latency (include/psdf_bench.h): per-step microseconds, timed inside the library."""
+        poses, pp = _host(poses, np.float32)
+        out4 = np.empty((self._serve_N, 4), np.float32)
+        out = (ctypes.c_double * int(reps))()
+        _check(lib().psdf_bench_serve_latency(self._h, pp, out4.ctypes.data, int(reps), out), "psdf_bench_serve_latency")
         return np.frombuffer(out, dtype=np.float64).copy()
 
     def mpc_coeffs_host(self, poses, d_min, rho_p, rho_theta):

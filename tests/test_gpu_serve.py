@@ -1,0 +1,126 @@
+"""Serving mode (psdf_serve_begin / psdf_serve_step / psdf_serve_end, include/psdf.h): a persistent kernel
+with a mailbox in mapped memory for one fixed MPC batch shape (Alg.1 l.5-11).  Rows must
+be bit-identical to psdf_eval_host / psdf_mpc_coeffs_host and match the oracle; the kernel must survive its
+idle time-out (restart), perception updates (restart on the new scene) and other calls made next to it.
+Every wait is bounded (idle time-outs of <= 300 ms).  Need a B200: `pytest -m gpu`."""
+import time
+
+import numpy as np
+import pytest
+
+from tests.parity import compare
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    from oracle import psdf_oracle as O
+    from paper_2607_04310_b200 import psdf, workloads as W
+    assert torch.cuda.is_available()
+    return torch, O, psdf, W
+
+
+class _Ref:
+    def __init__(self, ref, sign=1.0):
+        self.value, self.grad, self.margin, self.per_obstacle = ref.value, sign * ref.grad, ref.margin, None
+
+
+@pytest.mark.parametrize("case", ["cfg1", "cfg2", "table1_M100_B15", "M1000_B3", "V6_B33"])
+def test_serve_rows_equal_host_path_and_oracle(env, case):
+    torch, O, psdf, W = env
+    if case == "cfg1":
+        w = W.make_config(1)
+    elif case == "cfg2":
+        w = W.make_config(2)
+    elif case == "table1_M100_B15":
+        w = W.table1_case(100, 15)
+    elif case == "M1000_B3":
+        w = W.table1_case(1000, 3)                      # K = 256 lanes per pose, one CTA per pose
+    else:
+        w = W.make_config(5).subsample(33)              # asymmetric 6-gon, 4096 obstacles
+    scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=w.N)
+    v, g, _ = scene.eval_host(w.poses, grad=True)
+    ref = O.evaluate(w.footprint, w.A, w.B, w.S, w.poses)
+    try:
+        scene.serve_begin(w.N, idle_timeout_ms=300)
+        for rep in range(50):
+            rows = scene.serve_step(w.poses)
+            assert np.array_equal(rows[:, 0], v) and np.array_equal(rows[:, 1:], g), (case, rep)
+        compare(ref, rows[:, 0], rows[:, 1:], what=case + " serve")
+        # new poses every step (an MPC loop): reversed order, shifted headings
+        for rep in range(10):
+            q = w.poses[::-1].copy()
+            q[:, 2] += np.float32(0.01 * rep)
+            rows = scene.serve_step(q)
+            vq, gq, _ = scene.eval_host(q, grad=True)   # the ordinary host path may be used next to the server
+            assert np.array_equal(rows[:, 0], vq) and np.array_equal(rows[:, 1:], gq), (case, rep)
+        # coefficient rows, eqs.(26)-(28)
+        scene.serve_begin(w.N, coeffs=(0.01, 0.1, 0.1), idle_timeout_ms=300)
+        c = scene.serve_step(w.poses)
+        assert np.array_equal(c, scene.mpc_coeffs_host(w.poses, 0.01, 0.1, 0.1))
+        want = O.mpc_coeffs(ref.value, ref.grad, w.footprint, 0.01, 0.1, 0.1)
+        fin = np.isfinite(want[:, 0])
+        assert (np.abs(c[fin, 0] - want[fin, 0]) <= 1e-5 + 4 * np.abs(want[fin, 0]) * 2.0 ** -23).all()
+        compare(_Ref(ref, -1.0), rows[:, 0] * 0 + ref.value.astype(np.float32), c[:, 1:], what=case + " J_g")
+    finally:
+        scene.serve_end()
+    torch.cuda.synchronize()                            # returns at once: the kernel is gone
+    scene.close()
+
+
+def test_serve_survives_timeout_update_and_errors(env):
+    torch, O, psdf, W = env
+    w = W.make_config(1)
+    scene = psdf.Scene(w.footprint, w.A, w.B, w.S, max_poses=64)
+    v, g, _ = scene.eval_host(w.poses, grad=True)
+    with pytest.raises(psdf.PsdfError):                 # step before begin
+        scene._serve_N = w.N
+        scene.serve_step(w.poses)
+    for bad_n in (0, 513):
+        with pytest.raises(psdf.PsdfError) as e:
+            scene.serve_begin(bad_n)
+        assert e.value.status == psdf.PSDF_ERR_INVALID_ARG
+    with pytest.raises(psdf.PsdfError) as e:
+        scene.serve_begin(65)                           # beyond the scene's max_poses
+    assert e.value.status == psdf.PSDF_ERR_CAPACITY
+    try:
+        scene.serve_begin(w.N, idle_timeout_ms=30)
+        rows = scene.serve_step(w.poses)
+        assert np.array_equal(rows[:, 0], v)
+        # idle time-out: the kernel exits by itself, the next step starts it again
+        time.sleep(0.12)
+        t0 = time.perf_counter()
+        torch.cuda.synchronize()                        # nothing left to wait for
+        assert time.perf_counter() - t0 < 0.02
+        for _ in range(3):
+            rows = scene.serve_step(w.poses)
+            assert np.array_equal(rows[:, 0], v) and np.array_equal(rows[:, 1:], g)
+        # perception update while serving: the server restarts on the new scene
+        sh = np.array([0.5, -0.25], np.float32)
+        scene.update(w.A + sh, w.B + sh, w.S)
+        v2, g2, _ = scene.eval_host(w.poses, grad=True)
+        rows = scene.serve_step(w.poses)
+        assert np.array_equal(rows[:, 0], v2) and np.array_equal(rows[:, 1:], g2) and not np.array_equal(v2, v)
+        scene.update(torch.from_numpy(w.A).cuda(), torch.from_numpy(w.B).cuda(), torch.from_numpy(w.S).cuda())
+        rows = scene.serve_step(w.poses)
+        assert np.array_equal(rows[:, 0], v) and np.array_equal(rows[:, 1:], g)
+        # an obstacle-free frame: +inf, zero gradient; a non-finite pose: NaN row, neighbours unaffected
+        scene.update(w.A, w.B, np.zeros_like(w.S))
+        rows = scene.serve_step(w.poses)
+        assert np.isposinf(rows[:, 0]).all() and (rows[:, 1:] == 0).all()
+        scene.update(w.A, w.B, w.S)
+        q = w.poses.copy()
+        q[3, 1] = np.nan
+        rows = scene.serve_step(q)
+        keep = np.arange(w.N) != 3
+        assert np.isnan(rows[3]).all() and np.array_equal(rows[keep, 0], v[keep])
+        # device path and culling switch next to the server
+        vd, gd, _ = scene.eval(torch.from_numpy(w.poses).cuda(), grad=True)
+        scene.set_culling(True)
+        rows = scene.serve_step(w.poses)
+        assert np.array_equal(rows[:, 0], v) and np.array_equal(vd.cpu().numpy(), v)
+    finally:
+        scene.serve_end()
+    scene.close()

@@ -29,7 +29,7 @@ def test_static_scratch_entry_point_matches_psdf_eval():
     # the entry point's code (everything behind its marker in psdf_api.cu) holds no allocating call
     import os, re
     src = open(os.path.join(os.path.dirname(psdf.LIB_PATH), "csrc", "psdf_api.cu")).read()
-    tail = src[src.index("no-allocation entry point"):]
+    tail = src[src.index("no-allocation entry point"):src.index("== serving mode")]
     tail = re.sub(r"//[^\n]*", "", tail)
     assert "psdf_eval_static_scratch" in tail and "cudaGetSymbolAddress" in tail
     assert not re.search(r"cudaMalloc|cudaFree|cudaHostAlloc|cudaMallocHost|\bnew\b|malloc\(|std::vector", tail)
