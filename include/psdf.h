@@ -130,8 +130,9 @@ psdf_status psdf_eval_host(psdf_scene* scene, const float* poses, int N, float* 
  *                      want_coeffs = 1: rows [h - gamma ; J_g] as psdf_mpc_coeffs_host with d_min, rho_p,
  *                      rho_theta.  idle_timeout_ms in [1, 10000]: a kernel that sees no request for that
  *                      long exits by itself (the next step starts it again, at the cost of one launch).
- *   psdf_serve_step    poses host [N,3] -> out host [N,4]; posts the poses, spins until every CTA has
- *                      acknowledged, copies the rows out.  Results are bit-identical to psdf_eval_host /
+ *   psdf_serve_step    poses host [N,3] -> out host [N,4]; posts the poses, spins until every row has
+ *                      arrived (the rows are blanked with a NaN pattern no result carries and watched
+ *                      word by word: no fence, no acknowledgement), copies the rows out.  Results are bit-identical to psdf_eval_host /
  *                      psdf_mpc_coeffs_host.  Ordinary host memory is fine (N is small).
  *   psdf_serve_end     stops the kernel (psdf_destroy_scene does it too).
  * While the kernel runs it occupies a few CTAs and polls host memory over PCIe; a device-wide

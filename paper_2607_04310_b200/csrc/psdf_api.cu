@@ -1217,6 +1217,7 @@ extern "C" psdf_status psdf_eval_static_scratch(const psdf_scene* sc, const floa
 namespace {
 
 constexpr int kServeMaxPoses = 512, kServeMaxCtas = 128;
+constexpr unsigned kServeSentinel = 0x7fa5a5a5u;   // a NaN payload no kernel result carries (theirs: 0x7fc00000, 0x7fffffff)
 
 template <int V>
 cudaError_t launch_serve_v(const psdf_scene* sc, const EvalParams& p, unsigned last_seq) {
@@ -1339,6 +1340,9 @@ psdf_status psdf_serve_step(psdf_scene* sc, const float* poses, float* out) {
   if (seq == kServeExit || seq == 0u) seq = 1u;
   const unsigned prev = sv.seq;
   sv.seq = seq;
+  const __m128i sentinel = _mm_set1_epi32((int)kServeSentinel);
+  for (int n = 0; n < sv.N; ++n) _mm_store_si128(reinterpret_cast<__m128i*>(sv.out + n), sentinel);
+  _mm_sfence();                                              // rows are blank before the request can be seen
   for (int n = 0; n < sv.N; ++n) serve_post(sv, n, poses[3 * n], poses[3 * n + 1], poses[3 * n + 2], seq);
   _mm_sfence();
   if (!sv.running) {                                         // paused by an update, or first step after a time-out
@@ -1348,10 +1352,13 @@ psdf_status psdf_serve_step(psdf_scene* sc, const float* poses, float* out) {
   volatile unsigned* ack = sv.ack;
   const auto t0 = std::chrono::steady_clock::now();
   int relaunches = 0;
-  for (int c = 0; c < sv.G;) {
+  // a row has arrived when none of its four words is the sentinel any more (the kernel writes a row with one
+  // 16-byte store; word-wise acceptance does not even rely on that store landing as a whole)
+  for (int n = 0; n < sv.N;) {
     unsigned spins = 0;
     bool restart = false;
-    while (ack[2 * c] != seq) {
+    const volatile __m128i* row = reinterpret_cast<const volatile __m128i*>(sv.out + n);
+    while (_mm_movemask_epi8(_mm_cmpeq_epi32(_mm_load_si128(const_cast<const __m128i*>(row)), sentinel)) != 0) {
       _mm_pause();
       if ((++spins & 0x3fu) != 0u) continue;
       for (int k = 0; k < sv.G && !restart; ++k) restart = ack[2 * k + 1] != 0u;   // a CTA gave up (idle time-out)
@@ -1371,14 +1378,16 @@ psdf_status psdf_serve_step(psdf_scene* sc, const float* poses, float* out) {
       psdf_status s = serve_pause(sc);
       if (s != PSDF_OK) return s;
       if (++relaunches > 3) return PSDF_ERR_CUDA;
-      for (int n = 0; n < sv.N; ++n) serve_post(sv, n, poses[3 * n], poses[3 * n + 1], poses[3 * n + 2], seq);
+      for (int k = 0; k < sv.N; ++k) _mm_store_si128(reinterpret_cast<__m128i*>(sv.out + k), sentinel);
+      _mm_sfence();
+      for (int k = 0; k < sv.N; ++k) serve_post(sv, k, poses[3 * k], poses[3 * k + 1], poses[3 * k + 2], seq);
       _mm_sfence();
       s = serve_launch(sc, prev);
       if (s != PSDF_OK) return s;
-      c = 0;
+      n = 0;
       continue;
     }
-    ++c;
+    ++n;
   }
   std::memcpy(out, sv.out, sizeof(float4) * (size_t)sv.N);
   return PSDF_OK;

@@ -389,8 +389,8 @@ __global__ void __launch_bounds__(256) psdf_lanes_args_kernel(const __grid_const
 // (one 16-byte slot per pose: x, y, theta and the request's sequence number in the fourth word, stored
 // with one 16-byte store), the leader lane of every pose group polls ITS slot over PCIe, so the flag and
 // the data arrive in the same read, the CTA evaluates (lanes_body, poses handed over through shared
-// memory), writes one float4 per pose (value, gradient; or the coefficient row) back to mapped memory,
-// fences, and raises its acknowledgement word, on which the host spins.
+// memory) and writes one float4 per pose (value, gradient; or the coefficient row) back to mapped memory,
+// where the host watches the rows arrive.
 // Lifetime is bounded: a CTA that sees no request for `idle_ns` (or the exit code) marks itself exited
 // and returns; the host relaunches on the next step (requests are idempotent).
 constexpr unsigned kServeExit = 0xffffffffu;
@@ -406,9 +406,7 @@ __device__ __forceinline__ float4 ld_volatile_f4(const float4* ptr) {
   return v;
 }
 
-// ack: mapped [2 * gridDim.x] = per CTA (last sequence number served, exited flag).  Only the lanes that wrote
-// a row fence at system scope before the CTA's acknowledgement (a fence by every thread cost 3-4 us on shapes
-// with many CTAs; collecting the rows on the device and letting the last CTA write them out was slower still).
+// ack: mapped [2 * gridDim.x] = per CTA (unused, exited flag).
 template <int V, int MODE>
 __global__ void __launch_bounds__(256) psdf_serve_kernel(const __grid_constant__ Footprint fp,
                                                          const __grid_constant__ EvalParams p,
@@ -444,9 +442,10 @@ __global__ void __launch_bounds__(256) psdf_serve_kernel(const __grid_constant__
     }
     const unsigned seq = __float_as_uint(s_pose[0].w); // (group 0 of a CTA always owns a pose)
     lanes_body<V, MODE, true>(fp, p, s_pose - (size_t)blockIdx.x * ppc);   // rows -> p.packed / p.coeff
-    if (lane == 0) __threadfence_system();             // this group's row before the acknowledgement
-    __syncthreads();
-    if (threadIdx.x == 0) ack[2 * blockIdx.x] = seq;
+    // no fence and no acknowledgement word: the host has filled every row with a sentinel pattern that no
+    // result can hold and watches the rows themselves (each is one 16-byte store; the host accepts a row
+    // only when none of its four words is the sentinel any more)
+    __syncthreads();                                   // (s_pose is rewritten by the next request)
     last = seq;
     t_idle = global_timer_ns();
   }

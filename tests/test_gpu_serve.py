@@ -56,6 +56,17 @@ def test_serve_rows_equal_host_path_and_oracle(env, case):
             rows = scene.serve_step(q)
             vq, gq, _ = scene.eval_host(q, grad=True)   # the ordinary host path may be used next to the server
             assert np.array_equal(rows[:, 0], vq) and np.array_equal(rows[:, 1:], gq), (case, rep)
+        # soak: rows are accepted by watching them arrive (no acknowledgement word): thousands of steps with
+        # alternating pose sets, every row of every step checked
+        qa, qb = w.poses.copy(), w.poses[::-1].copy()
+        va, ga, _ = scene.eval_host(qa, grad=True)
+        vb, gb, _ = scene.eval_host(qb, grad=True)
+        buf = np.empty((w.N, 4), np.float32)
+        for rep in range(2000):
+            scene.serve_step(qa, out=buf)
+            assert np.array_equal(buf[:, 0], va) and np.array_equal(buf[:, 1:], ga), (case, rep)
+            scene.serve_step(qb, out=buf)
+            assert np.array_equal(buf[:, 0], vb) and np.array_equal(buf[:, 1:], gb), (case, rep)
         # coefficient rows, eqs.(26)-(28)
         scene.serve_begin(w.N, coeffs=(0.01, 0.1, 0.1), idle_timeout_ms=300)
         c = scene.serve_step(w.poses)
