@@ -111,8 +111,8 @@ psdf_status psdf_eval_static_scratch(const psdf_scene* scene, const float* poses
 /* Same semantics with HOST buffers (Alg.1 l.5-11: upload the nominal states,
  * evaluate, bring the results back), on the scene's own stream; returns after synchronising it.
  * MPC-sized batches (N <= 512; with per_obstacle only up to 64 obstacles): ONE kernel launch; up
- * to 128 poses travel inside the launch, results are written to pinned, device-mapped staging and
- * copied out.  Larger batches: replay of a captured CUDA graph of up to four branches
+ * to 128 poses travel inside the launch, results are written to pinned, device-mapped staging, where
+ * the host watches the rows arrive (no stream synchronise unless per_obstacle is wanted), and copied out.  Larger batches: replay of a captured CUDA graph of up to four branches
  * {H2D pose chunk, kernel, D2H result chunk} that overlap copies and kernels.  Buffers in pinned
  * (page-locked) host memory are read and written in place by the copy engines; ordinary memory
  * goes through the scene's pinned staging (one extra host copy each way).  Results are

@@ -722,6 +722,32 @@ struct HostCall {
   float d_min = 0.f, rho_p = 0.f, rho_theta = 0.f;
 };
 
+// Result rows in mapped memory are watched as they arrive instead of waiting for the stream: the host blanks
+// them with a NaN bit pattern that no kernel result carries (the kernels' own NaNs are 0x7fc00000 and
+// 0x7fffffff) and accepts a row when none of its four words is the pattern any more.
+constexpr unsigned kRowSentinel = 0x7fa5a5a5u;
+
+// Spins until rows [0, N) of `rows` hold no sentinel word.  The stream is asked now and then: an error ends
+// the wait; a stream that has finished leaves at most one more pass (its writes are visible by then).
+static psdf_status wait_rows(const float4* rows, int N, cudaStream_t st) {
+  const __m128i sentinel = _mm_set1_epi32((int)kRowSentinel);
+  bool finished = false;
+  for (int n = 0; n < N; ++n) {
+    const __m128i* row = reinterpret_cast<const __m128i*>(rows + n);
+    unsigned spins = 0;
+    while (_mm_movemask_epi8(_mm_cmpeq_epi32(_mm_load_si128(const_cast<const __m128i*>(
+               reinterpret_cast<const volatile __m128i*>(row))), sentinel)) != 0) {
+      _mm_pause();
+      if ((++spins & 0x3ffu) != 0u) continue;
+      if (finished) return PSDF_ERR_CUDA;                     // the kernel is done and the row is still blank
+      const cudaError_t e = cudaStreamQuery(st);
+      if (e == cudaSuccess) finished = true;
+      else if (e != cudaErrorNotReady) return cuda_failed(e);
+    }
+  }
+  return PSDF_OK;
+}
+
 static psdf_status run_zero_copy(psdf_scene* sc, const HostCall& h) {
   // staging layout: h_in [N,4] poses (padded), h_out [N,4] = (value, grad) or coefficients;
   // up to kArgPoses poses go into the launch itself (kernel parameter) instead
@@ -743,9 +769,20 @@ static psdf_status run_zero_copy(psdf_scene* sc, const HostCall& h) {
   c.packed = sc->h_out;
   c.args = N <= kArgPoses ? &sc->h_args : nullptr;
   c.which_ws = 1;
+  const bool watch = !(h.mode & kPerObs);                     // ([N,M] per-obstacle output: wait for the stream)
+  if (watch) {
+    const __m128i sentinel = _mm_set1_epi32((int)kRowSentinel);
+    for (int n = 0; n < N; ++n) _mm_store_si128(reinterpret_cast<__m128i*>(sc->h_out) + n, sentinel);
+    _mm_sfence();
+  }
   psdf_status s = enqueue_eval(sc, c, sc->gstream);
   if (s != PSDF_OK) return s;
-  CU_TRY(cudaStreamSynchronize(sc->gstream));
+  if (watch) {
+    s = wait_rows(reinterpret_cast<const float4*>(sc->h_out), N, sc->gstream);
+    if (s != PSDF_OK) return s;
+  } else {
+    CU_TRY(cudaStreamSynchronize(sc->gstream));
+  }
   if (h.mode & kCoeff) {
     std::memcpy(h.coeff, sc->h_out, sizeof(float) * 4 * (size_t)N);
   } else {
@@ -1217,7 +1254,7 @@ extern "C" psdf_status psdf_eval_static_scratch(const psdf_scene* sc, const floa
 namespace {
 
 constexpr int kServeMaxPoses = 512, kServeMaxCtas = 128;
-constexpr unsigned kServeSentinel = 0x7fa5a5a5u;   // a NaN payload no kernel result carries (theirs: 0x7fc00000, 0x7fffffff)
+constexpr unsigned kServeSentinel = kRowSentinel;
 
 template <int V>
 cudaError_t launch_serve_v(const psdf_scene* sc, const EvalParams& p, unsigned last_seq) {
