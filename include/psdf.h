@@ -125,7 +125,10 @@ psdf_status psdf_eval_host(psdf_scene* scene, const float* poses, int N, float* 
  * kernel and a mailbox in pinned, device-mapped memory, so that a cycle costs neither a kernel launch nor a
  * stream synchronisation.
  *   psdf_serve_begin   starts the kernel on a stream of its own for batches of exactly N poses
- *                      (N <= 512 and at most 64 pose groups, else PSDF_ERR_INVALID_ARG: use psdf_eval_host);
+ *                      (N <= 512 and at most 128 pose groups, else PSDF_ERR_INVALID_ARG: use psdf_eval_host);
+ *                      row_window: NULL, or host [N,2] int32 obstacle ROW windows as in psdf_eval_windows,
+ *                      fixed for the session (time-varying environments: stage s sees the rows
+ *                      of E_{k+s}; the mapping stays, psdf_update_scene brings the new values);
  *                      want_coeffs = 0: rows (phi, d phi/dx, d phi/dy, d phi/dtheta) as psdf_eval_host;
  *                      want_coeffs = 1: rows [h - gamma ; J_g] as psdf_mpc_coeffs_host with d_min, rho_p,
  *                      rho_theta.  idle_timeout_ms in [1, 10000]: a kernel that sees no request for that
@@ -139,9 +142,9 @@ psdf_status psdf_eval_host(psdf_scene* scene, const float* poses, int N, float* 
  * synchronisation (cudaDeviceSynchronize, cudaFree) issued meanwhile waits until it exits, i.e. until
  * psdf_serve_end or the idle time-out.  psdf_update_scene, psdf_set_culling and psdf_set_components stop it
  * themselves and the next psdf_serve_step restarts it on the new scene; every other call of this header may
- * be used next to it.  Allocates pinned memory in psdf_serve_begin only. */
-psdf_status psdf_serve_begin(psdf_scene* scene, int N, int want_coeffs, float d_min, float rho_p, float rho_theta,
-                             int idle_timeout_ms);
+ * be used next to it.  Allocates (pinned memory, the window table) in psdf_serve_begin only. */
+psdf_status psdf_serve_begin(psdf_scene* scene, int N, const int* row_window, int want_coeffs, float d_min,
+                             float rho_p, float rho_theta, int idle_timeout_ms);
 psdf_status psdf_serve_step(psdf_scene* scene, const float* poses, float* out);
 psdf_status psdf_serve_end(psdf_scene* scene);
 

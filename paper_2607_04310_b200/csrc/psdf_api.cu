@@ -136,6 +136,8 @@ struct psdf_scene {
     float4* in = nullptr;               // mapped [N]   (x, y, theta, sequence number)
     float4* out = nullptr;              // mapped [N]   (value, grad) or coefficient rows
     unsigned* ack = nullptr;            // mapped [2 G] (served sequence number, exited flag) per CTA
+    int* d_win = nullptr;               // device [cap_N,2] per-pose obstacle row windows
+    bool windows = false;
     int cap_N = 0, cap_G = 0;
   } srv;
 };
@@ -515,6 +517,7 @@ void psdf_destroy_scene(psdf_scene* sc) {
   if (sc->srv.in) cudaFreeHost(sc->srv.in);
   if (sc->srv.out) cudaFreeHost(sc->srv.out);
   if (sc->srv.ack) cudaFreeHost(sc->srv.ack);
+  cudaFree(sc->srv.d_win);
   for (auto& g : sc->graphs)
     if (g.exec) cudaGraphExecDestroy(g.exec);
   if (sc->gstream) cudaStreamDestroy(sc->gstream);
@@ -1275,6 +1278,7 @@ psdf_status serve_launch(psdf_scene* sc, unsigned last_seq) {
   p.row_slot = sc->pk[sc->cur].row_slot;
   p.bounds = sc->pk[sc->cur].bounds;
   p.empty_rows = sc->pk[sc->cur].empty;
+  p.window = sv.windows ? sv.d_win : nullptr;
   float* rows = reinterpret_cast<float*>(sv.out);            // mapped host rows
   p.grad = (sv.mode & kGrad) ? rows : nullptr;               // (non-null = wanted; results go to `packed`)
   p.coeff = (sv.mode & kCoeff) ? rows : nullptr;
@@ -1324,8 +1328,8 @@ static psdf_status serve_pause(psdf_scene* sc) {
 
 extern "C" {
 
-psdf_status psdf_serve_begin(psdf_scene* sc, int N, int want_coeffs, float d_min, float rho_p, float rho_theta,
-                             int idle_timeout_ms) {
+psdf_status psdf_serve_begin(psdf_scene* sc, int N, const int* row_window, int want_coeffs, float d_min, float rho_p,
+                             float rho_theta, int idle_timeout_ms) {
   if (!sc || N < 1 || N > kServeMaxPoses || idle_timeout_ms < 1 || idle_timeout_ms > 10000) return PSDF_ERR_INVALID_ARG;
   if (N > sc->max_poses) return PSDF_ERR_CAPACITY;
   PSDF_ENTER(sc);
@@ -1345,10 +1349,12 @@ psdf_status psdf_serve_begin(psdf_scene* sc, int N, int want_coeffs, float d_min
     if (sv.in) cudaFreeHost(sv.in);
     if (sv.out) cudaFreeHost(sv.out);
     if (sv.ack) cudaFreeHost(sv.ack);
-    sv.in = sv.out = nullptr; sv.ack = nullptr; sv.cap_N = sv.cap_G = 0;
+    cudaFree(sv.d_win);
+    sv.in = sv.out = nullptr; sv.ack = nullptr; sv.d_win = nullptr; sv.cap_N = sv.cap_G = 0;
     CU_TRY(cudaHostAlloc(&sv.in, sizeof(float4) * (size_t)N, cudaHostAllocMapped));
     CU_TRY(cudaHostAlloc(&sv.out, sizeof(float4) * (size_t)N, cudaHostAllocMapped));
     CU_TRY(cudaHostAlloc(&sv.ack, sizeof(unsigned) * 2 * (size_t)G, cudaHostAllocMapped));
+    CU_TRY(cudaMalloc(&sv.d_win, sizeof(int) * 2 * (size_t)N));
     sv.cap_N = N; sv.cap_G = G;
   }
   int dev = 0, uva = 0;
@@ -1356,6 +1362,8 @@ psdf_status psdf_serve_begin(psdf_scene* sc, int N, int want_coeffs, float d_min
   CU_TRY(cudaDeviceGetAttribute(&uva, cudaDevAttrUnifiedAddressing, dev));
   if (!uva) return PSDF_ERR_CUDA;                            // (mapped host pointers are used as device pointers)
   sv.N = N; sv.K = K; sv.bd = bd; sv.G = G;
+  sv.windows = row_window != nullptr;
+  if (sv.windows) CU_TRY(cudaMemcpy(sv.d_win, row_window, sizeof(int) * 2 * (size_t)N, cudaMemcpyHostToDevice));
   sv.mode = want_coeffs ? kCoeff : kGrad;
   sv.d_min = d_min; sv.rho_p = rho_p; sv.rho_theta = rho_theta;
   sv.idle_ns = (unsigned long long)idle_timeout_ms * 1000000ull;

@@ -74,7 +74,7 @@ def lib():
     L.psdf_mpc_coeffs_host.restype = i
     L.psdf_mpc_coeffs_host.argtypes = [vp, fp_, i, ctypes.c_float, ctypes.c_float, ctypes.c_float, fp_]
     L.psdf_serve_begin.restype = i
-    L.psdf_serve_begin.argtypes = [vp, i, i, ctypes.c_float, ctypes.c_float, ctypes.c_float, i]
+    L.psdf_serve_begin.argtypes = [vp, i, vp, i, ctypes.c_float, ctypes.c_float, ctypes.c_float, i]
     L.psdf_serve_step.restype = i
     L.psdf_serve_step.argtypes = [vp, fp_, fp_]
     L.psdf_serve_end.restype = i
@@ -405,12 +405,17 @@ class Scene:
                                              float(rho_theta), int(reps), out), "psdf_bench_host_latency")
         return np.frombuffer(out, dtype=np.float64).copy()
 
-    def serve_begin(self, N, coeffs=None, idle_timeout_ms=200):
+    def serve_begin(self, N, coeffs=None, idle_timeout_ms=200, row_window=None):
         """psdf_serve_begin: persistent-kernel serving of batches of exactly N poses; coeffs = (d_min, rho_p,
-        rho_theta) for MPC coefficient rows, None for (value, grad) rows."""
+        rho_theta) for MPC coefficient rows, None for (value, grad) rows; row_window: optional [N,2] int32
+        per-pose obstacle row windows, fixed for the session."""
         d_min, rho_p, rho_theta = coeffs if coeffs else (0.0, 0.0, 0.0)
-        _check(lib().psdf_serve_begin(self._h, int(N), 1 if coeffs else 0, float(d_min), float(rho_p), float(rho_theta),
-                                      int(idle_timeout_ms)), "psdf_serve_begin")
+        pw = None
+        if row_window is not None:
+            win, pw = _host(row_window, np.int32)
+            assert win.shape == (int(N), 2)
+        _check(lib().psdf_serve_begin(self._h, int(N), pw, 1 if coeffs else 0, float(d_min), float(rho_p),
+                                      float(rho_theta), int(idle_timeout_ms)), "psdf_serve_begin")
         self._serve_N = int(N)
 
     def serve_step(self, poses, out=None):

@@ -81,6 +81,51 @@ def test_serve_rows_equal_host_path_and_oracle(env, case):
     scene.close()
 
 
+def test_serve_with_row_windows(env):
+    """Per-stage edge sets E_{k+s} under the server: the scene holds H stage-wise obstacle sets,
+    stage s sees its own rows; the window table is fixed at psdf_serve_begin, a perception update brings new
+    values for all stages.  Rows equal psdf_eval_windows_host bit for bit and the oracle per stage."""
+    torch, O, psdf, W = env
+    rng = np.random.default_rng(99)
+    base = W.table1_case(12, 1, seed=778)
+    H, Ms = 15, base.M
+    vel = rng.uniform(-1.0, 1.0, (Ms, 1, 2)).astype(np.float32)
+
+    def stacked(t0):
+        A = np.concatenate([(base.A + vel * np.float32(0.1 * (s + t0))).astype(np.float32) for s in range(H)])
+        B = A.copy()
+        S = np.concatenate([base.S] * H)
+        for i in range(H * Ms):
+            sl = np.nonzero(S[i])[0]
+            B[i, sl] = A[i, np.roll(sl, -1)]
+        return A, B, S
+
+    A, B, S = stacked(0)
+    poses = np.stack([rng.uniform(0, 20, H), rng.uniform(0, 20, H), rng.uniform(-3.2, 3.2, H)], 1).astype(np.float32)
+    win = np.stack([np.arange(H) * Ms, (np.arange(H) + 1) * Ms], 1).astype(np.int32)
+    scene = psdf.Scene(base.footprint, A, B, S, max_poses=H)
+    try:
+        scene.serve_begin(H, row_window=win, idle_timeout_ms=300)
+        for t0 in (0, 1, 2):                                   # control cycles: obstacles move, all stages updated
+            if t0:
+                A, B, S = stacked(t0)
+                scene.update(A, B, S)
+            vw, gw = scene.eval_windows_host(poses, win)
+            rows = scene.serve_step(poses)
+            assert np.array_equal(rows[:, 0], vw) and np.array_equal(rows[:, 1:], gw), t0
+            for s_ in range(H):
+                r = slice(s_ * Ms, (s_ + 1) * Ms)
+                ref = O.evaluate(base.footprint, A[r], B[r], S[r], poses[s_:s_ + 1])
+                compare(ref, rows[s_:s_ + 1, 0], rows[s_:s_ + 1, 1:], what=f"cycle {t0} stage {s_}")
+        scene.serve_begin(H, idle_timeout_ms=300)              # and back to all rows
+        v, g, _ = scene.eval_host(poses)
+        rows = scene.serve_step(poses)
+        assert np.array_equal(rows[:, 0], v) and np.array_equal(rows[:, 1:], g)
+    finally:
+        scene.serve_end()
+    scene.close()
+
+
 def test_serve_survives_timeout_update_and_errors(env):
     torch, O, psdf, W = env
     w = W.make_config(1)
