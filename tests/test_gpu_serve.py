@@ -117,6 +117,16 @@ def test_serve_with_row_windows(env):
                 r = slice(s_ * Ms, (s_ + 1) * Ms)
                 ref = O.evaluate(base.footprint, A[r], B[r], S[r], poses[s_:s_ + 1])
                 compare(ref, rows[s_:s_ + 1, 0], rows[s_:s_ + 1, 1:], what=f"cycle {t0} stage {s_}")
+        # coefficient rows under windows; a stage whose window is empty is an inactive row (reading G17)
+        win2 = win.copy()
+        win2[4] = (7, 7)
+        scene.serve_begin(H, coeffs=(0.01, 0.1, 0.1), row_window=win2, idle_timeout_ms=300)
+        c = scene.serve_step(poses)
+        vw, gw = scene.eval_windows_host(poses, win2)
+        keep = np.arange(H) != 4
+        want = O.mpc_coeffs(vw.astype(np.float64), gw.astype(np.float64), base.footprint, 0.01, 0.1, 0.1)
+        assert np.isposinf(c[4, 0]) and (c[4, 1:] == 0).all() and np.isposinf(vw[4])
+        assert np.array_equal(c[keep, 1:], -gw[keep]) and np.abs(c[keep, 0] - want[keep, 0]).max() <= 1e-5
         scene.serve_begin(H, idle_timeout_ms=300)              # and back to all rows
         v, g, _ = scene.eval_host(poses)
         rows = scene.serve_step(poses)
