@@ -86,6 +86,18 @@ def test_random_scenes_every_path(env, block):
         # host path (single zero-copy launch or graph), all outputs
         vh, gh, poh = scene.eval_host(poses[idx], grad=True, per_obstacle=True)
         compare(ref, vh, gh, poh, what=tag + " eval_host")
+        # serving mode (persistent kernel + mailbox): rows bit-equal to the host path, twice, then coefficients
+        if len(idx) <= 512:
+            try:
+                scene.serve_begin(len(idx), idle_timeout_ms=200)
+                for _ in range(2):
+                    rows = scene.serve_step(poses[idx])
+                    assert np.array_equal(rows[:, 0], vh) and np.array_equal(rows[:, 1:], gh), tag + " serve"
+                scene.serve_begin(len(idx), coeffs=(0.3, 0.05, 0.02), idle_timeout_ms=200)
+                rows = scene.serve_step(poses[idx])
+                assert np.array_equal(rows, scene.mpc_coeffs_host(poses[idx], 0.3, 0.05, 0.02)), tag + " serve coeffs"
+            finally:
+                scene.serve_end()
         # MPC coefficients, eqs.(26)-(28)
         d_min, rho_p, rho_t = 0.3, 0.05, 0.02
         c = scene.mpc_coeffs_host(poses[idx], d_min, rho_p, rho_t)
