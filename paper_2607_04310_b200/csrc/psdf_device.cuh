@@ -206,6 +206,57 @@ __device__ __forceinline__ void edge_step2(const Footprint& fp, const Posed2<V>&
   minD2 = m;
 }
 
+// Two edges of one pair record at once (tile-scan kernel, full records): the same arithmetic as two
+// edge_step2 calls, written vertex pair by vertex pair for both edges, so that consecutive instructions read the
+// same posed-vertex register pairs (operand reuse) and the two robot-face updates fold into one three-input
+// maximum.  min / max are exact, so the order of the updates does not change a bit.
+template <int V>
+__device__ __forceinline__ void edge_step2_two(const Footprint& fp, const Posed2<V>& P, const float4 qa, const float4 qb,
+                                               const float ha, const float hb, ObstacleAcc<V>& acc, float& minD2) {
+  const float saxa = qa.x - P.px, saya = qa.y - P.py, saxb = qb.x - P.px, sayb = qb.y - P.py;
+  const float sncna = fmaf(saxa, qa.w, -saya * qa.z), sncnb = fmaf(saxb, qb.w, -sayb * qb.z);
+  const float sncta = -fmaf(saxa, qa.z, fmaf(saya, qa.w, ha)), snctb = -fmaf(saxb, qb.z, fmaf(sayb, qb.w, hb));
+  const float2 axa = bc2(saxa), aya = bc2(saya), naxa = bc2(-saxa), axb = bc2(saxb), ayb = bc2(sayb), naxb = bc2(-saxb);
+  const float2 txa = bc2(qa.z), tya = bc2(qa.w), ntya = bc2(-qa.w), txb = bc2(qb.z), tyb = bc2(qb.w), ntyb = bc2(-qb.w);
+  const float2 ncna = bc2(sncna), ncta = bc2(sncta), nha = bc2(-ha), ncnb = bc2(sncnb), nctb = bc2(snctb), nhb = bc2(-hb);
+  float gja = -kInf, gjb = -kInf;
+  float m = minD2;
+#pragma unroll
+  for (int l = 0; l < V / 2; ++l) {
+    // pool 1 + obstacle axes a, b
+    const float2 sa = __ffma2_rn(P.ry[l], txa, __ffma2_rn(P.rx[l], ntya, ncna));
+    const float2 sb = __ffma2_rn(P.ry[l], txb, __ffma2_rn(P.rx[l], ntyb, ncnb));
+    const float2 ua = __ffma2_rn(P.rx[l], txa, __ffma2_rn(P.ry[l], tya, ncta));
+    const float2 ub = __ffma2_rn(P.rx[l], txb, __ffma2_rn(P.ry[l], tyb, nctb));
+    const float2 eta = __fadd2_rn(make_float2(fabsf(ua.x), fabsf(ua.y)), nha);
+    const float2 etb = __fadd2_rn(make_float2(fabsf(ub.x), fabsf(ub.y)), nhb);
+    const float2 ea = make_float2(fmaxf(eta.x, 0.f), fmaxf(eta.y, 0.f)), eb = make_float2(fmaxf(etb.x, 0.f), fmaxf(etb.y, 0.f));
+    const float2 da = __ffma2_rn(ea, ea, __fmul2_rn(sa, sa)), db = __ffma2_rn(eb, eb, __fmul2_rn(sb, sb));
+    gja = fmax3(gja, sa.x, sa.y);
+    gjb = fmax3(gjb, sb.x, sb.y);
+    // pool 2 + robot axes l, l+1
+    const float2 ncN = *reinterpret_cast<const float2*>(&fp.ncN[2 * l]);
+    const float2 ncT = *reinterpret_cast<const float2*>(&fp.ncT[2 * l]);
+    const float2 nhR = *reinterpret_cast<const float2*>(&fp.nh[2 * l]);
+    const float2 ppa = __ffma2_rn(aya, P.Tx[l], __ffma2_rn(naxa, P.Ty[l], ncN));
+    const float2 ppb = __ffma2_rn(ayb, P.Tx[l], __ffma2_rn(naxb, P.Ty[l], ncN));
+    const float2 wa = __ffma2_rn(axa, P.Tx[l], __ffma2_rn(aya, P.Ty[l], ncT));
+    const float2 wb = __ffma2_rn(axb, P.Tx[l], __ffma2_rn(ayb, P.Ty[l], ncT));
+    const float2 fta = __fadd2_rn(make_float2(fabsf(wa.x), fabsf(wa.y)), nhR);
+    const float2 ftb = __fadd2_rn(make_float2(fabsf(wb.x), fabsf(wb.y)), nhR);
+    const float2 fa = make_float2(fmaxf(fta.x, 0.f), fmaxf(fta.y, 0.f)), fb = make_float2(fmaxf(ftb.x, 0.f), fmaxf(ftb.y, 0.f));
+    const float2 ga = __ffma2_rn(fa, fa, __fmul2_rn(ppa, ppa)), gb = __ffma2_rn(fb, fb, __fmul2_rn(ppb, ppb));
+    acc.gR[2 * l] = fmax3(acc.gR[2 * l], ppa.x, ppb.x);
+    acc.gR[2 * l + 1] = fmax3(acc.gR[2 * l + 1], ppa.y, ppb.y);
+    m = fmin3(m, da.x, da.y);
+    m = fmin3(m, db.x, db.y);
+    m = fmin3(m, ga.x, ga.y);
+    m = fmin3(m, gb.x, gb.y);
+  }
+  acc.gO = fmin3(acc.gO, gja, gjb);
+  minD2 = m;
+}
+
 // The same step for a footprint that is centrally symmetric about its reference point, v_{l+V/2} = -v_l
 // (rectangles, car outlines; V a multiple of 4; Footprint::sym, set at pack time when it holds bitwise).
 // Then r_{l+V/2} = -r_l, T_{l+V/2} = -T_l, and the constants c_N, c_T, h of edge l+V/2 equal those of edge
