@@ -493,7 +493,7 @@ def main():
                                        "over_kernel": t_e2e_cull * 1e3 / float(np.mean(cull_times)),
                                        "outputs_checked": e2e_cull_checked,
                                        "from_pageable_buffers_ms_per_step": t_e2e_cull_pageable * 1e3,
-                                       "api": "psdf_eval_host with culling on, pinned host buffers"},
+                                       "api": "psdf_eval_host with culling on, pinned host buffers (one launch reading and writing them over PCIe)"},
                         "note": "pairs/s counts all pairs (SURVEY.md 8(d)); culled pairs cost at most two bound tests"},
             "gpu_launches": int(launches), "wall_s_timed_region": t_wall, "clocks": clocks,
             "paper_context": {"psdf_rtx4090_M100_B100_ms": 2.207, "implied_pairs_per_s": 4.5e6,

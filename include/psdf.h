@@ -115,7 +115,8 @@ psdf_status psdf_eval_static_scratch(const psdf_scene* scene, const float* poses
  * the host watches the rows arrive (no stream synchronise unless per_obstacle is wanted), and copied out.  Larger batches: replay of a captured CUDA graph of up to four branches
  * {H2D pose chunk, kernel, D2H result chunk} that overlap copies and kernels.  Buffers in pinned
  * (page-locked) host memory are read and written in place by the copy engines; ordinary memory
- * goes through the scene's pinned staging (one extra host copy each way).  Results are
+ * goes through the scene's pinned staging (one extra host copy each way); with culling on and pinned
+ * buffers one kernel reads and writes them itself, without the copy engines.  Results are
  * bit-identical to psdf_eval on the same poses.  grad / per_obstacle may be NULL. */
 psdf_status psdf_eval_host(psdf_scene* scene, const float* poses, int N, float* value, float* grad,
                            float* per_obstacle);

@@ -923,10 +923,53 @@ static psdf_status run_graph(psdf_scene* sc, const HostCall& h) {
   return PSDF_OK;
 }
 
+// Device-side address of a pinned (page-locked) host buffer, or null if the memory is not pinned.
+static void* pinned_device_ptr(const void* ptr) {
+  if (!ptr) return nullptr;
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, ptr) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+  return a.type == cudaMemoryTypeHost ? a.devicePointer : nullptr;
+}
+
+// Large batches on the culled path with PINNED caller buffers: one launch, no copy engine.  The culled kernel
+// reads every pose once and writes every result once, so it can do both over PCIe itself (coalesced 384-byte
+// reads / writes per warp), and transfer and evaluation overlap CTA by CTA instead of branch by branch.
+// (The dense tile-scan kernel reads a pose once per obstacle chunk: it keeps the copy-engine graph.)
+static bool takes_direct(const psdf_scene* sc, const HostCall& h, EvalCall& c) {
+  if (!sc->culling || (h.mode & kPerObs) || lanes_plan(sc, h.N) || h.N <= kCullMinPoses || sc->Mv < 64 ||
+      sc->n_pairs >= (1 << 24))
+    return false;                                           // (not the culled path: see enqueue_eval)
+  c.poses = static_cast<const float*>(pinned_device_ptr(h.poses));
+  if (!c.poses) return false;
+  if (h.mode & kCoeff) {
+    c.coeff = static_cast<float*>(pinned_device_ptr(h.coeff));
+    if (!c.coeff) return false;
+    c.value = c.coeff;                                      // (not written in coefficient mode)
+    c.d_min = h.d_min; c.rho_p = h.rho_p; c.rho_theta = h.rho_theta;
+  } else {
+    c.value = static_cast<float*>(pinned_device_ptr(h.value));
+    if (!c.value) return false;
+    if (h.mode & kGrad) {
+      c.grad = static_cast<float*>(pinned_device_ptr(h.grad));
+      if (!c.grad) return false;
+    }
+  }
+  c.N = h.N;
+  c.which_ws = 1;
+  return true;
+}
+
 static psdf_status run_host(psdf_scene* sc, const HostCall& h) {
   psdf_status s = ensure_host_path(sc, (h.mode & kPerObs) != 0);
   if (s != PSDF_OK) return s;
   if (use_zero_copy(sc, h.N, (h.mode & kPerObs) != 0)) return run_zero_copy(sc, h);
+  EvalCall direct;
+  if (takes_direct(sc, h, direct)) {
+    s = enqueue_eval(sc, direct, sc->gstream);
+    if (s != PSDF_OK) return s;
+    CU_TRY(cudaStreamSynchronize(sc->gstream));
+    return PSDF_OK;
+  }
   return run_graph(sc, h);
 }
 
