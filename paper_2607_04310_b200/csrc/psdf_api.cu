@@ -931,27 +931,38 @@ static void* pinned_device_ptr(const void* ptr) {
   return a.type == cudaMemoryTypeHost ? a.devicePointer : nullptr;
 }
 
-// Large batches on the culled path with PINNED caller buffers: one launch, no copy engine.  The culled kernel
+// Large batches on the culled path: one launch, no copy engine.  The culled kernel
 // reads every pose once and writes every result once, so it can do both over PCIe itself (coalesced 384-byte
 // reads / writes per warp), and transfer and evaluation overlap CTA by CTA instead of branch by branch.
 // (The dense tile-scan kernel reads a pose once per obstacle chunk: it keeps the copy-engine graph.)
-static bool takes_direct(const psdf_scene* sc, const HostCall& h, EvalCall& c) {
+// Buffers that are not pinned go through the scene's pinned, device-mapped staging (one host copy each way).
+struct DirectPlan {
+  EvalCall c;
+  bool stage_value = false, stage_grad = false, stage_coeff = false;
+};
+
+static bool takes_direct(psdf_scene* sc, const HostCall& h, DirectPlan& d) {
   if (!sc->culling || (h.mode & kPerObs) || lanes_plan(sc, h.N) || h.N <= kCullMinPoses || sc->Mv < 64 ||
-      sc->n_pairs >= (1 << 24))
+      sc->n_pairs >= (1 << 24) || !sc->zero_copy)
     return false;                                           // (not the culled path: see enqueue_eval)
+  EvalCall& c = d.c;
+  const size_t N = (size_t)h.N;
   c.poses = static_cast<const float*>(pinned_device_ptr(h.poses));
-  if (!c.poses) return false;
+  if (!c.poses) {
+    std::memcpy(sc->h_in, h.poses, sizeof(float) * 3 * N);
+    c.poses = sc->h_in;
+  }
   if (h.mode & kCoeff) {
     c.coeff = static_cast<float*>(pinned_device_ptr(h.coeff));
-    if (!c.coeff) return false;
+    if (!c.coeff) { c.coeff = sc->h_out; d.stage_coeff = true; }
     c.value = c.coeff;                                      // (not written in coefficient mode)
     c.d_min = h.d_min; c.rho_p = h.rho_p; c.rho_theta = h.rho_theta;
   } else {
     c.value = static_cast<float*>(pinned_device_ptr(h.value));
-    if (!c.value) return false;
+    if (!c.value) { c.value = sc->h_out; d.stage_value = true; }
     if (h.mode & kGrad) {
       c.grad = static_cast<float*>(pinned_device_ptr(h.grad));
-      if (!c.grad) return false;
+      if (!c.grad) { c.grad = sc->h_out + N; d.stage_grad = true; }
     }
   }
   c.N = h.N;
@@ -963,11 +974,15 @@ static psdf_status run_host(psdf_scene* sc, const HostCall& h) {
   psdf_status s = ensure_host_path(sc, (h.mode & kPerObs) != 0);
   if (s != PSDF_OK) return s;
   if (use_zero_copy(sc, h.N, (h.mode & kPerObs) != 0)) return run_zero_copy(sc, h);
-  EvalCall direct;
+  DirectPlan direct;
   if (takes_direct(sc, h, direct)) {
-    s = enqueue_eval(sc, direct, sc->gstream);
+    s = enqueue_eval(sc, direct.c, sc->gstream);
     if (s != PSDF_OK) return s;
     CU_TRY(cudaStreamSynchronize(sc->gstream));
+    const size_t N = (size_t)h.N;
+    if (direct.stage_coeff) std::memcpy(h.coeff, sc->h_out, sizeof(float) * 4 * N);
+    if (direct.stage_value) std::memcpy(h.value, sc->h_out, sizeof(float) * N);
+    if (direct.stage_grad) std::memcpy(h.grad, sc->h_out + N, sizeof(float) * 3 * N);
     return PSDF_OK;
   }
   return run_graph(sc, h);
